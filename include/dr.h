@@ -1,0 +1,183 @@
+/* dr.h — C-ABI of the B200-native Diffusion Restore hot path (arXiv 2605.08916).
+ *
+ * The per-frame step of N independent Markov chains in primary sample space (PSS):
+ * Alg. 1 Initialize/Accumulate, Alg. 2 Evolve (L530-L543),
+ * Alg. 3 Resolve (L545-L550), Alg. 4 LocalDynamics (L707-L723), for the five samplers of
+ * L733-L747.  Readings of everything the paper leaves open: DESIGN.md section 2 (Q1-Q20).
+ *
+ * Conventions
+ *  - plain C, no exceptions cross this boundary; every call returns a dr_status
+ *    (negative = failure and no state change where possible, positive = warning);
+ *    dr_last_error() gives a thread-local message for the last non-OK status.
+ *  - "host" / "dev" in a parameter name says where the pointer lives.  Host arrays given to
+ *    dr_scene_create* are copied (the caller may free them on return).  Chain state, the
+ *    accumulation buffer and the output image are CALLER-OWNED DEVICE MEMORY (e.g. torch
+ *    tensors); the library never frees them and they must outlive the dr_chains handle.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  All work is
+ *    asynchronous on that stream; only dr_chains_stats and the *_download / *_upload hooks
+ *    synchronise it.
+ *  - one GPU (the current device), fp32 arithmetic, sm_100a only, no CPU fallback.
+ */
+#ifndef DR_H_
+#define DR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  DR_OK = 0,
+  DR_WARN_NO_TOURS = 1,      /* resolve before any tour completed: zero image, no division */
+  DR_ERR_INVALID_ARG = -1,
+  DR_ERR_UNSUPPORTED = -2,
+  DR_ERR_CUDA = -3,
+  DR_ERR_NONFINITE = -4,     /* non-finite value in host input */
+  DR_ERR_OOM = -5
+} dr_status;
+
+/* the five samplers. */
+typedef enum {
+  DR_METROPOLIS = 0,
+  DR_MALA = 1,
+  DR_METROPOLIS_RESTORE = 2,
+  DR_MALA_RESTORE = 3,
+  DR_DIFFUSION_RESTORE = 4
+} dr_method;
+
+/* pbrt-v4 diffuse / dielectric / conductor + DiffuseAreaLight, simplified as in DESIGN.md Q6-Q7. */
+typedef enum { DR_MAT_LAMBERT = 0, DR_MAT_DIELECTRIC = 1, DR_MAT_GGX_CONDUCTOR = 2, DR_MAT_EMITTER = 3 } dr_mat_kind;
+
+typedef struct {
+  int32_t kind;             /* dr_mat_kind */
+  float albedo_or_f0[3];    /* Lambert albedo or conductor F0 */
+  float ior;                /* dielectric: inside / outside index ratio (> 0) */
+  float roughness;          /* GGX alpha in (0, 1] */
+  float emission[3];        /* emitter radiance on the front face (geometric normal side) */
+} dr_material;
+
+typedef struct {
+  const float* host_vertices;       /* 3 * nv */
+  uint32_t nv;
+  const uint32_t* host_indices;     /* 3 * nt, counter-clockwise = front */
+  uint32_t nt;
+  const uint32_t* host_tri_material;/* nt, index into materials */
+  const dr_material* host_materials;
+  uint32_t nm;
+  float env_radiance[3];            /* radiance of rays that escape */
+  float cam_pos[3], cam_look[3], cam_up[3];
+  float vfov_deg;                   /* pinhole camera, vertical field of view */
+  uint32_t width, height;           /* image W x H; pixel map DESIGN.md Q4 */
+  uint32_t max_path_len;            /* L segments, PSS dimension d = 2L (Q5); 1 <= L <= 16 */
+} dr_scene_desc;
+
+/* 2-D analytic target (d = 2): mixture of wrapped Gaussians, f = (p,p,p), closed-form score.
+ * Exercises the samplers without ray tracing (stationarity tests). */
+typedef struct {
+  uint32_t n_components;            /* 1..16 */
+  const float* host_weights;        /* n */
+  const float* host_means;          /* 2 n */
+  const float* host_stddevs;        /* n */
+  uint32_t width, height;
+} dr_analytic2d_desc;
+
+typedef struct {
+  int32_t method;            /* dr_method */
+  uint32_t n_chains;         /* N = dispatchCount */
+  float stddev;              /* L747: 1e-2 Metropolis*, 5e-3 Langevin-based; > 0 */
+  float c_tilde;             /* rotation strength c~ = dt c / 2 (L700), Diffusion Restore only; >= 0 */
+  float dt;                  /* L755: 1e-5; holding rate lambda = 1/dt (L659), Diffusion Restore only; > 0 */
+  float m;                   /* L754: expected local steps per tour, kappa0 = p_lambda / (m dt) (L752); > 0 */
+  float large_step_prob;     /* L747: 0.3 for plain Metropolis / MALA; ignored by Restore variants; in [0,1] */
+  float p_lambda_override;   /* > 0: use as p_lambda; <= 0: bootstrap from the init states (DESIGN.md a0) */
+  uint64_t seed;             /* Philox key (Q14) */
+  uint32_t chain_offset;     /* global id of chain 0: RNG streams are keyed by global chain id, so a run sharded
+                                over several GPUs draws the same numbers as the unsharded run */
+} dr_config;
+
+typedef struct {
+  uint64_t tours;            /* tourCount */
+  uint64_t mutations;        /* Accumulate calls = chain-iterations, init included */
+  uint64_t rays;             /* closest-hit queries */
+  uint64_t mh_accepts;       /* accepted Metropolis-Hastings proposals */
+  uint64_t nonfinite;        /* evaluations with non-finite f or score (treated as p = 0, Q18) */
+  uint32_t kills_last_step;  /* == regen_queue_len */
+  uint32_t regen_queue_len;
+  uint32_t iteration;        /* n of the last completed iteration (0 = init) */
+  float p_lambda, kappa0, lambda;
+} dr_stats;
+
+typedef struct {
+  uint32_t n_tris, n_nodes, depth, smem_nodes; /* BVH8 nodes, tree depth, nodes staged in shared memory */
+  float sah_cost;
+  float eps_ray;
+  size_t device_bytes;
+} dr_scene_info;
+
+typedef struct dr_scene dr_scene;   /* opaque */
+typedef struct dr_chains dr_chains; /* opaque */
+
+const char* dr_last_error(void);
+
+/* Validates the description (finite vertices, indices < nv, materials in range, 1 <= L <= 16, W,H >= 1),
+ * builds a SAH BVH2 on the host, collapses it to a BVH8, uploads.  The scene owns its device memory. */
+dr_status dr_scene_create(const dr_scene_desc* desc, dr_scene** out);
+dr_status dr_scene_create_analytic2d(const dr_analytic2d_desc* desc, dr_scene** out);
+dr_status dr_scene_destroy(dr_scene* scene);
+dr_status dr_scene_get_info(const dr_scene* scene, dr_scene_info* host_out);
+
+/* Bytes of device memory dr_chains_create needs for N chains on this scene (256-byte aligned). */
+size_t dr_chains_state_bytes(const dr_scene* scene, const dr_config* cfg);
+
+/* Validates cfg (stddev > 0, dt > 0, m > 0, probabilities in [0,1], N >= 1) and lays the chain state out in
+ * dev_state (SoA planes).  dev_accum_rgba: W*H float4 (RGB = sum w f/p_hat, A = sum w/p_hat). */
+dr_status dr_chains_create(const dr_scene* scene, const dr_config* cfg, void* dev_state, size_t state_bytes,
+                           float* dev_accum_rgba, dr_chains** out);
+dr_status dr_chains_destroy(dr_chains* chains);
+
+/* Alg. 1 for every chain (+ bootstrap of p_lambda and kappa0): zeroes the accumulation buffer and counters,
+ * x ~ U[0,1)^d keyed by (chain, iteration 0, frame_index), evaluate, Accumulate. */
+dr_status dr_chains_init(dr_chains* chains, uint32_t frame_index, void* stream);
+
+/* Alg. 2 for every chain, `iterations` times.  `method` must equal the method the chains were created with
+ * (DR_ERR_INVALID_ARG otherwise). */
+dr_status dr_step(dr_chains* chains, int32_t method, uint32_t iterations, void* stream);
+
+/* Alg. 3: dev_rgb_out[W*H*3] = N_pix * kappa0 / tourCount * accum (Restore) or N_pix * p_lambda / N_mut * accum
+ * (plain MH).  Returns DR_WARN_NO_TOURS and writes zeros if tourCount == 0 (the check synchronises the stream). */
+dr_status dr_resolve_image(dr_chains* chains, float* dev_rgb_out, void* stream);
+
+/* Synchronises the stream and copies the counters. */
+dr_status dr_chains_stats(dr_chains* chains, dr_stats* host_out, void* stream);
+
+/* ---- test hooks (parity harness; same library) ---------------------------------------------------------- */
+/* Host arrays, row-major: x[N*d], score[N*d], p[N], f_over_p[N*3], pix[N], killed[N], sig[N] (hash of the
+ * discrete decisions of the state's path).  Any output pointer may be NULL. */
+dr_status dr_chains_download(dr_chains* chains, float* host_x, float* host_p, float* host_f_over_p, uint32_t* host_pix,
+                             uint8_t* host_killed, float* host_score, uint32_t* host_sig, void* stream);
+/* Teacher forcing: overwrite the state and set the iteration counter; rebuilds the regeneration queue. */
+dr_status dr_chains_upload(dr_chains* chains, const float* host_x, const float* host_p, const float* host_f_over_p,
+                           const uint32_t* host_pix, const uint8_t* host_killed, const float* host_score,
+                           uint32_t iteration, void* stream);
+/* Per-chain record of the last iteration: accepted flag and sampled weight (dtau, or 1 for plain MH). */
+dr_status dr_chains_last_step(dr_chains* chains, uint8_t* host_accepted, float* host_weight, void* stream);
+/* Killed chain ids in ascending order; host_ids may be NULL to query the length. */
+dr_status dr_regen_queue_download(dr_chains* chains, uint32_t* host_ids, uint32_t* host_len, void* stream);
+/* Closest hit for n rays (device arrays o[3n], d[3n] -> t[n] (-1 = miss), prim[n] (0xFFFFFFFF = miss)). */
+dr_status dr_trace_rays(const dr_scene* scene, const float* dev_o, const float* dev_d, uint32_t n, float* dev_t,
+                        uint32_t* dev_prim, void* stream);
+/* Target evaluation for n states (device arrays, row-major x[n*d]) -> f[3n], p[n], pix[n], score[n*d] (if
+ * non-NULL), nrays[n], sig[n]. */
+dr_status dr_eval_states(const dr_scene* scene, const float* dev_x, uint32_t n, float* dev_f, float* dev_p,
+                         uint32_t* dev_pix, float* dev_score, uint32_t* dev_nrays, uint32_t* dev_sig, void* stream);
+/* Raw Philox blocks for n counters (device arrays ctr[4n] -> out[4n]) under key (seed lo, hi), and the stream
+ * transforms of DESIGN.md Q14 for n words pairs: out[4n] = u[0,1), u(0,1], Box-Muller z0, z1. */
+dr_status dr_philox_blocks(uint64_t seed, const uint32_t* dev_ctr, uint32_t n, uint32_t* dev_out, void* stream);
+dr_status dr_rng_transforms(const uint32_t* dev_words, uint32_t n, float* dev_out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DR_H_ */

@@ -35,6 +35,7 @@ struct Config {
   double large_step_prob;   // L747: 0.3 (plain Metropolis / MALA only)
   double p_lambda_override; // <= 0: bootstrap from the init states (Q-a0)
   uint64_t seed;
+  uint32_t chain_offset;    // global id of chain 0 (chains are keyed by global id: sharding-invariant, section 8e)
 };
 
 template <class Real> struct Eval {
@@ -127,14 +128,14 @@ template <class Real> struct Chains {
   void uniform_point(uint32_t chain, uint32_t iter, uint32_t purpose, Real* y) const {
     for (uint32_t j = 0; j < d; j += 4) {
       uint32_t w[4];
-      stream_block(cfg.seed, chain, iter, j / 4, purpose, epoch, w);
+      stream_block(cfg.seed, cfg.chain_offset + chain, iter, j / 4, purpose, epoch, w);
       for (uint32_t c = 0; c < 4 && j + c < d; ++c) y[j + c] = u01_co<Real>(w[c]);
     }
   }
   void normals(uint32_t chain, uint32_t iter, Real* xi) const {
     for (uint32_t j = 0; j < d; j += 4) {
       uint32_t w[4];
-      stream_block(cfg.seed, chain, iter, j / 4, PROP_N, epoch, w);
+      stream_block(cfg.seed, cfg.chain_offset + chain, iter, j / 4, PROP_N, epoch, w);
       Real z[4];
       box_muller<Real>(w[0], w[1], z[0], z[1]);
       box_muller<Real>(w[2], w[3], z[2], z[3]);
@@ -153,7 +154,7 @@ template <class Real> struct Chains {
   // Accumulate, Alg. 1 L506-L526.  The target was evaluated when the state was stored.
   void accumulate(uint32_t i, uint32_t n) {
     uint32_t w[4];
-    stream_block(cfg.seed, i, n, 0, DECIDE, epoch, w);
+    stream_block(cfg.seed, cfg.chain_offset + i, n, 0, DECIDE, epoch, w);
     const Real phat = p[i] + Real(kEps);
     Real weight = Real(1);
     if (restore) {
@@ -238,7 +239,7 @@ template <class Real> struct Chains {
         const Real* xi_ = &x[(size_t)i * d];
         const Real* gi = &g[(size_t)i * d];
         uint32_t w[4];
-        stream_block(cfg.seed, i, n, 0, DECIDE, epoch, w);
+        stream_block(cfg.seed, cfg.chain_offset + i, n, 0, DECIDE, epoch, w);
         if (restore && killed[i]) {                 // Alg. 2: re-initialise from nu
           kind[i] = 1;
           uniform_point(i, n, REGEN_U, y);
@@ -265,7 +266,7 @@ template <class Real> struct Chains {
       }
       for (uint32_t i = 0; i < N; ++i) {
         uint32_t w[4];
-        stream_block(cfg.seed, i, n, 0, DECIDE, epoch, w);
+        stream_block(cfg.seed, cfg.chain_offset + i, n, 0, DECIDE, epoch, w);
         const Real* y = &Y[(size_t)i * d];
         const Real* gy = &GY[(size_t)i * d];
         rays += E[i].nrays; nonfinite += E[i].nonfinite;

@@ -1,0 +1,477 @@
+// C-ABI entry points (include/dr.h): argument validation, scene upload, state layout, kernel launches.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/dr.h"
+#include "dr_kernels.cuh"
+
+using namespace dr;
+
+namespace {
+
+thread_local std::string g_err;
+
+dr_status fail(dr_status s, const std::string& msg) { g_err = msg; return s; }
+
+#define CUDA_TRY(expr)                                                                                   \
+  do {                                                                                                   \
+    cudaError_t e_ = (expr);                                                                             \
+    if (e_ != cudaSuccess)                                                                               \
+      return fail(e_ == cudaErrorMemoryAllocation ? DR_ERR_OOM : DR_ERR_CUDA,                            \
+                  std::string(#expr) + ": " + cudaGetErrorString(e_));                                   \
+  } while (0)
+
+size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+bool finite3(const float* v) { return std::isfinite(v[0]) && std::isfinite(v[1]) && std::isfinite(v[2]); }
+
+void normalize(float* v) {
+  const float n = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+  v[0] /= n; v[1] /= n; v[2] /= n;
+}
+void cross(const float* a, const float* b, float* c) {
+  c[0] = a[1] * b[2] - a[2] * b[1];
+  c[1] = a[2] * b[0] - a[0] * b[2];
+  c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+}  // namespace
+
+struct dr_scene {
+  DevScene dev{};
+  void* d_nodes = nullptr;
+  void* d_tris = nullptr;
+  void* d_mats = nullptr;
+  dr_scene_info info{};
+};
+
+struct dr_chains {
+  const dr_scene* scene = nullptr;
+  dr_config cfg{};
+  ChainParams cp{};
+  ChainState st{};
+  float4* accum = nullptr;
+  uint32_t npix = 0, nblocks = 0;
+  uint32_t iteration = 0;
+  bool initialised = false;
+  size_t state_bytes = 0;
+  void* state_base = nullptr;
+};
+
+namespace {
+
+struct Layout {
+  size_t x, g, fp, pix, sig, killed, y, gy, fy, pixy, sigy, kind, accepted, weight, order, blockcnt, blockoff, partial, ctr, total;
+};
+
+Layout make_layout(uint32_t N, uint32_t planes, bool grad) {
+  Layout L{};
+  size_t o = 0;
+  auto take = [&](size_t bytes) { const size_t at = o; o = align256(o + bytes); return at; };
+  const size_t nb = (N + kBlock - 1) / kBlock;
+  L.x = take(sizeof(float4) * planes * N);
+  L.g = take(grad ? sizeof(float4) * planes * N : 0);
+  L.fp = take(sizeof(float4) * N);
+  L.pix = take(4 * (size_t)N);
+  L.sig = take(4 * (size_t)N);
+  L.killed = take(N);
+  L.y = take(sizeof(float4) * planes * N);
+  L.gy = take(grad ? sizeof(float4) * planes * N : 0);
+  L.fy = take(sizeof(float4) * N);
+  L.pixy = take(4 * (size_t)N);
+  L.sigy = take(4 * (size_t)N);
+  L.kind = take(N);
+  L.accepted = take(N);
+  L.weight = take(4 * (size_t)N);
+  L.order = take(4 * (size_t)N);
+  L.blockcnt = take(4 * nb);
+  L.blockoff = take(4 * nb);
+  L.partial = take(8 * nb);
+  L.ctr = take(sizeof(Counters));
+  L.total = o;
+  return L;
+}
+
+dr_status check_config(const dr_config* c) {
+  if (!c) return fail(DR_ERR_INVALID_ARG, "config is null");
+  if (c->method < 0 || c->method > 4) return fail(DR_ERR_INVALID_ARG, "method out of range");
+  if (c->n_chains < 1) return fail(DR_ERR_INVALID_ARG, "n_chains must be >= 1");
+  if (!(c->stddev > 0.f) || !std::isfinite(c->stddev)) return fail(DR_ERR_INVALID_ARG, "stddev must be > 0");
+  if (!(c->c_tilde >= 0.f) || !std::isfinite(c->c_tilde)) return fail(DR_ERR_INVALID_ARG, "c_tilde must be >= 0");
+  if (!(c->dt > 0.f) || !std::isfinite(c->dt)) return fail(DR_ERR_INVALID_ARG, "dt must be > 0");
+  if (!(c->m > 0.f) || !std::isfinite(c->m)) return fail(DR_ERR_INVALID_ARG, "m must be > 0");
+  if (!(c->large_step_prob >= 0.f && c->large_step_prob <= 1.f)) return fail(DR_ERR_INVALID_ARG, "large_step_prob must be in [0,1]");
+  if (!std::isfinite(c->p_lambda_override)) return fail(DR_ERR_INVALID_ARG, "p_lambda_override must be finite");
+  return DR_OK;
+}
+
+size_t smem_bytes(const dr_scene* s) { return (size_t)s->dev.smem_nodes * sizeof(Node8); }
+
+// evaluation of all proposals (+ the kernels that must precede / follow it)
+dr_status launch_iteration(dr_chains* c, uint32_t n, bool init, cudaStream_t s) {
+  const ChainParams& cp = c->cp;
+  const uint32_t gb = c->nblocks, ge = (cp.N + kEvalBlock - 1) / kEvalBlock;
+  k_propose<<<gb, kBlock, 0, s>>>(cp, c->st, n, init ? 1 : 0);
+  const int use_order = (!init && cp.restore) ? 1 : 0;
+  const size_t sm = smem_bytes(c->scene);
+  if (cp.grad) k_eval<true><<<ge, kEvalBlock, sm, s>>>(c->scene->dev, cp, c->st, use_order);
+  else k_eval<false><<<ge, kEvalBlock, sm, s>>>(c->scene->dev, cp, c->st, use_order);
+  if (init) {
+    k_psum_partial<<<gb, kBlock, 0, s>>>(cp, c->st);
+    k_bootstrap<<<1, kBlock, 0, s>>>(cp, c->st, gb);
+  }
+  k_decide<<<gb, kBlock, 0, s>>>(cp, c->st, c->accum, n);
+  if (cp.restore) {
+    k_scan<<<1, 1024, 0, s>>>(c->st, gb);
+    k_scatter<<<gb, kBlock, 0, s>>>(cp, c->st);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* dr_last_error(void) { return g_err.c_str(); }
+
+dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
+  if (!d || !out) return fail(DR_ERR_INVALID_ARG, "null argument");
+  *out = nullptr;
+  if (!d->host_vertices || !d->host_indices || !d->host_tri_material || !d->host_materials)
+    return fail(DR_ERR_INVALID_ARG, "null array in scene description");
+  if (d->nv < 3 || d->nt < 1 || d->nm < 1) return fail(DR_ERR_INVALID_ARG, "empty scene");
+  if (d->nt >= (1u << 27)) return fail(DR_ERR_UNSUPPORTED, "more than 2^27 triangles");
+  if (d->width < 1 || d->height < 1) return fail(DR_ERR_INVALID_ARG, "image size must be >= 1");
+  if (d->max_path_len < 1 || d->max_path_len > (uint32_t)kMaxPathLen) return fail(DR_ERR_INVALID_ARG, "max_path_len must be in [1,16]");
+  if (!(d->vfov_deg > 0.f && d->vfov_deg < 180.f)) return fail(DR_ERR_INVALID_ARG, "vfov_deg must be in (0,180)");
+  for (size_t i = 0; i < 3 * (size_t)d->nv; ++i)
+    if (!std::isfinite(d->host_vertices[i])) return fail(DR_ERR_NONFINITE, "non-finite vertex");
+  for (size_t i = 0; i < 3 * (size_t)d->nt; ++i)
+    if (d->host_indices[i] >= d->nv) return fail(DR_ERR_INVALID_ARG, "vertex index out of range");
+  for (uint32_t i = 0; i < d->nt; ++i)
+    if (d->host_tri_material[i] >= d->nm) return fail(DR_ERR_INVALID_ARG, "material index out of range");
+  if (!finite3(d->env_radiance) || !finite3(d->cam_pos) || !finite3(d->cam_look) || !finite3(d->cam_up))
+    return fail(DR_ERR_NONFINITE, "non-finite camera or environment");
+  std::vector<MatPacked> mats(d->nm);
+  for (uint32_t i = 0; i < d->nm; ++i) {
+    const dr_material& m = d->host_materials[i];
+    if (m.kind < 0 || m.kind > 3) return fail(DR_ERR_INVALID_ARG, "material kind out of range");
+    if (!finite3(m.albedo_or_f0) || !finite3(m.emission) || !std::isfinite(m.ior) || !std::isfinite(m.roughness))
+      return fail(DR_ERR_NONFINITE, "non-finite material");
+    if (m.kind == DR_MAT_DIELECTRIC && !(m.ior > 0.f)) return fail(DR_ERR_INVALID_ARG, "dielectric ior must be > 0");
+    if (m.kind == DR_MAT_GGX_CONDUCTOR && !(m.roughness > 0.f && m.roughness <= 1.f))
+      return fail(DR_ERR_INVALID_ARG, "GGX roughness must be in (0,1]");
+    MatPacked& p = mats[i];
+    std::memset(&p, 0, sizeof(p));
+    p.kind = (uint32_t)m.kind;
+    for (int c = 0; c < 3; ++c) p.a[c] = m.albedo_or_f0[c];
+    p.ior = m.ior; p.alpha = m.roughness; p.le0 = m.emission[0]; p.le1 = m.emission[1]; p.le2 = m.emission[2];
+  }
+  BuiltBvh bvh;
+  build_bvh8(d->host_vertices, d->nv, d->host_indices, d->nt, d->host_tri_material, bvh);
+
+  dr_scene* s = new dr_scene();
+  DevScene& dev = s->dev;
+  const size_t nb = bvh.nodes.size() * sizeof(Node8), tb = bvh.tris.size() * sizeof(TriPacked), mb = mats.size() * sizeof(MatPacked);
+  cudaError_t e = cudaMalloc(&s->d_nodes, nb);
+  if (e == cudaSuccess) e = cudaMalloc(&s->d_tris, tb);
+  if (e == cudaSuccess) e = cudaMalloc(&s->d_mats, mb);
+  if (e == cudaSuccess) e = cudaMemcpy(s->d_nodes, bvh.nodes.data(), nb, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(s->d_tris, bvh.tris.data(), tb, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(s->d_mats, mats.data(), mb, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(s->d_nodes); cudaFree(s->d_tris); cudaFree(s->d_mats);
+    delete s;
+    return fail(e == cudaErrorMemoryAllocation ? DR_ERR_OOM : DR_ERR_CUDA, std::string("scene upload: ") + cudaGetErrorString(e));
+  }
+  dev.nodes = (const float4*)s->d_nodes; dev.tris = (const float4*)s->d_tris; dev.mats = (const float4*)s->d_mats;
+  dev.n_nodes = (uint32_t)bvh.nodes.size();
+  dev.smem_nodes = dev.n_nodes < (uint32_t)kSmemNodes ? dev.n_nodes : (uint32_t)kSmemNodes;
+  dev.n_tris = d->nt; dev.n_mats = d->nm;
+  for (int c = 0; c < 3; ++c) { dev.env[c] = d->env_radiance[c]; dev.cam_pos[c] = d->cam_pos[c]; }
+  // pinhole basis: w = normalize(look - pos), r = normalize(w x up), v = r x w
+  float w[3] = {d->cam_look[0] - d->cam_pos[0], d->cam_look[1] - d->cam_pos[1], d->cam_look[2] - d->cam_pos[2]};
+  normalize(w);
+  float r[3], v[3];
+  cross(w, d->cam_up, r);
+  normalize(r);
+  cross(r, w, v);
+  if (!finite3(w) || !finite3(r)) {
+    dr_scene_destroy(s);
+    return fail(DR_ERR_INVALID_ARG, "degenerate camera (look == pos or up parallel to view)");
+  }
+  for (int c = 0; c < 3; ++c) { dev.cam_w[c] = w[c]; dev.cam_r[c] = r[c]; dev.cam_v[c] = v[c]; }
+  dev.tan_half = std::tan(d->vfov_deg * (float)(3.14159265358979323846 / 360.0));
+  dev.tan_half_aspect = dev.tan_half * ((float)d->width / (float)d->height);
+  dev.W = d->width; dev.H = d->height; dev.L = d->max_path_len; dev.d = 2 * d->max_path_len; dev.planes = (dev.d + 3) / 4;
+  dev.eps_ray = 1e-5f * bvh.diag;  // Q8
+  dev.analytic = 0; dev.n_mix = 0;
+  s->info.n_tris = d->nt; s->info.n_nodes = dev.n_nodes; s->info.depth = bvh.depth; s->info.smem_nodes = dev.smem_nodes;
+  s->info.sah_cost = bvh.sah_cost; s->info.eps_ray = dev.eps_ray; s->info.device_bytes = nb + tb + mb;
+  *out = s;
+  return DR_OK;
+}
+
+dr_status dr_scene_create_analytic2d(const dr_analytic2d_desc* d, dr_scene** out) {
+  if (!d || !out) return fail(DR_ERR_INVALID_ARG, "null argument");
+  *out = nullptr;
+  if (d->n_components < 1 || d->n_components > (uint32_t)kMaxMix) return fail(DR_ERR_INVALID_ARG, "n_components must be in [1,16]");
+  if (!d->host_weights || !d->host_means || !d->host_stddevs) return fail(DR_ERR_INVALID_ARG, "null array");
+  if (d->width < 1 || d->height < 1) return fail(DR_ERR_INVALID_ARG, "image size must be >= 1");
+  dr_scene* s = new dr_scene();
+  DevScene& dev = s->dev;
+  for (uint32_t k = 0; k < d->n_components; ++k) {
+    const float w = d->host_weights[k], sd = d->host_stddevs[k], mx = d->host_means[2 * k], my = d->host_means[2 * k + 1];
+    if (!(std::isfinite(w) && std::isfinite(sd) && std::isfinite(mx) && std::isfinite(my))) { delete s; return fail(DR_ERR_NONFINITE, "non-finite mixture parameter"); }
+    if (!(w > 0.f) || !(sd > 0.f)) { delete s; return fail(DR_ERR_INVALID_ARG, "weights and stddevs must be > 0"); }
+    dev.mix_w[k] = w; dev.mix_s[k] = sd; dev.mix_mx[k] = mx; dev.mix_my[k] = my;
+  }
+  dev.analytic = 1; dev.n_mix = (int)d->n_components;
+  dev.W = d->width; dev.H = d->height; dev.L = 1; dev.d = 2; dev.planes = 1;
+  dev.smem_nodes = 0; dev.n_nodes = 0;
+  s->info = dr_scene_info{};
+  *out = s;
+  return DR_OK;
+}
+
+dr_status dr_scene_destroy(dr_scene* s) {
+  if (!s) return DR_OK;
+  cudaFree(s->d_nodes); cudaFree(s->d_tris); cudaFree(s->d_mats);
+  delete s;
+  return DR_OK;
+}
+
+dr_status dr_scene_get_info(const dr_scene* s, dr_scene_info* o) {
+  if (!s || !o) return fail(DR_ERR_INVALID_ARG, "null argument");
+  *o = s->info;
+  return DR_OK;
+}
+
+size_t dr_chains_state_bytes(const dr_scene* s, const dr_config* c) {
+  if (!s || check_config(c) != DR_OK) return 0;
+  const bool grad = c->method == DR_MALA || c->method == DR_MALA_RESTORE || c->method == DR_DIFFUSION_RESTORE;
+  return make_layout(c->n_chains, s->dev.planes, grad).total;
+}
+
+dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_state, size_t bytes, float* dev_accum, dr_chains** out) {
+  if (!s || !out || !dev_state || !dev_accum) return fail(DR_ERR_INVALID_ARG, "null argument");
+  *out = nullptr;
+  const dr_status cs = check_config(c);
+  if (cs != DR_OK) return cs;
+  if (((uintptr_t)dev_state & 255u) || ((uintptr_t)dev_accum & 15u)) return fail(DR_ERR_INVALID_ARG, "dev_state must be 256-byte and dev_accum 16-byte aligned");
+  const bool grad = c->method == DR_MALA || c->method == DR_MALA_RESTORE || c->method == DR_DIFFUSION_RESTORE;
+  const Layout L = make_layout(c->n_chains, s->dev.planes, grad);
+  if (bytes < L.total) return fail(DR_ERR_INVALID_ARG, "state buffer smaller than dr_chains_state_bytes");
+  dr_chains* h = new dr_chains();
+  h->scene = s; h->cfg = *c;
+  ChainParams& cp = h->cp;
+  cp.method = c->method; cp.restore = c->method >= DR_METROPOLIS_RESTORE; cp.grad = grad;
+  cp.N = c->n_chains; cp.d = s->dev.d; cp.planes = s->dev.planes;
+  cp.stddev = c->stddev; cp.half_s2 = 0.5f * c->stddev * c->stddev; cp.c_tilde = c->c_tilde; cp.dt = c->dt; cp.m = c->m;
+  cp.large_step_prob = cp.restore ? 0.f : c->large_step_prob;
+  cp.p_lambda_override = c->p_lambda_override; cp.seed = c->seed; cp.epoch = 0; cp.chain_offset = c->chain_offset;
+  char* b = (char*)dev_state;
+  ChainState& st = h->st;
+  st.x = (float4*)(b + L.x); st.g = (float4*)(b + L.g); st.fp = (float4*)(b + L.fp); st.pix = (uint32_t*)(b + L.pix);
+  st.sig = (uint32_t*)(b + L.sig); st.killed = (uint8_t*)(b + L.killed); st.y = (float4*)(b + L.y); st.gy = (float4*)(b + L.gy);
+  st.fy = (float4*)(b + L.fy); st.pixy = (uint32_t*)(b + L.pixy); st.sigy = (uint32_t*)(b + L.sigy); st.kind = (uint8_t*)(b + L.kind);
+  st.accepted = (uint8_t*)(b + L.accepted); st.weight = (float*)(b + L.weight); st.order = (uint32_t*)(b + L.order);
+  st.blockcnt = (uint32_t*)(b + L.blockcnt); st.blockoff = (uint32_t*)(b + L.blockoff); st.partial = (double*)(b + L.partial);
+  st.ctr = (Counters*)(b + L.ctr);
+  h->accum = (float4*)dev_accum;
+  h->npix = s->dev.W * s->dev.H;
+  h->nblocks = (cp.N + kBlock - 1) / kBlock;
+  h->state_bytes = L.total; h->state_base = dev_state;
+  const size_t sm = smem_bytes(s);
+  if (sm > 48 * 1024) {
+    CUDA_TRY(cudaFuncSetAttribute(k_eval<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    CUDA_TRY(cudaFuncSetAttribute(k_eval<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+  }
+  *out = h;
+  return DR_OK;
+}
+
+dr_status dr_chains_destroy(dr_chains* c) { delete c; return DR_OK; }
+
+dr_status dr_chains_init(dr_chains* c, uint32_t frame_index, void* stream) {
+  if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
+  if (frame_index >= (1u << 24)) return fail(DR_ERR_INVALID_ARG, "frame_index must be < 2^24");
+  cudaStream_t s = (cudaStream_t)stream;
+  c->cp.epoch = frame_index;
+  c->iteration = 0;
+  CUDA_TRY(cudaMemsetAsync(c->state_base, 0, c->state_bytes, s));
+  CUDA_TRY(cudaMemsetAsync(c->accum, 0, sizeof(float4) * (size_t)c->npix, s));
+  const dr_status r = launch_iteration(c, 0, true, s);
+  if (r == DR_OK) c->initialised = true;
+  return r;
+}
+
+dr_status dr_step(dr_chains* c, int32_t method, uint32_t iterations, void* stream) {
+  if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
+  if (method != c->cfg.method) return fail(DR_ERR_INVALID_ARG, "method differs from the one the chains were created with");
+  if (!c->initialised) return fail(DR_ERR_INVALID_ARG, "dr_chains_init has not been called");
+  for (uint32_t k = 0; k < iterations; ++k) {
+    const dr_status r = launch_iteration(c, ++c->iteration, false, (cudaStream_t)stream);
+    if (r != DR_OK) return r;
+  }
+  return DR_OK;
+}
+
+dr_status dr_resolve_image(dr_chains* c, float* dev_rgb, void* stream) {
+  if (!c || !dev_rgb) return fail(DR_ERR_INVALID_ARG, "null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  k_resolve<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, s>>>(c->cp, c->st.ctr, c->accum, dev_rgb, c->npix);
+  CUDA_TRY(cudaGetLastError());
+  if (c->cp.restore) {
+    unsigned long long tours = 0;
+    CUDA_TRY(cudaMemcpyAsync(&tours, &c->st.ctr->tours, sizeof(tours), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    if (tours == 0) { g_err = "no tour has completed yet: zero image"; return DR_WARN_NO_TOURS; }
+  }
+  return DR_OK;
+}
+
+dr_status dr_chains_stats(dr_chains* c, dr_stats* o, void* stream) {
+  if (!c || !o) return fail(DR_ERR_INVALID_ARG, "null argument");
+  Counters h;
+  CUDA_TRY(cudaMemcpyAsync(&h, c->st.ctr, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+  o->tours = h.tours; o->mutations = h.mutations; o->rays = h.rays; o->mh_accepts = h.mh_accepts; o->nonfinite = h.nonfinite;
+  o->kills_last_step = h.kills_last; o->regen_queue_len = h.queue_len; o->iteration = c->iteration;
+  o->p_lambda = h.p_lambda; o->kappa0 = h.kappa0; o->lambda = h.lambda;
+  return DR_OK;
+}
+
+// ---- test hooks ---------------------------------------------------------------------------------------------
+dr_status dr_chains_download(dr_chains* c, float* hx, float* hp, float* hfop, uint32_t* hpix, uint8_t* hkilled, float* hscore,
+                             uint32_t* hsig, void* stream) {
+  if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
+  cudaStream_t s = (cudaStream_t)stream;
+  const uint32_t N = c->cp.N, d = c->cp.d, g = (N + 255) / 256;
+  float* tmp = nullptr;
+  CUDA_TRY(cudaMalloc(&tmp, sizeof(float) * (size_t)N * (d > 4 ? d : 4)));
+  dr_status r = DR_OK;
+  auto rows = [&](const float4* planes, float* host) -> cudaError_t {
+    k_planes_to_rows<<<g, 256, 0, s>>>(planes, tmp, N, d, c->cp.planes);
+    return cudaMemcpyAsync(host, tmp, sizeof(float) * (size_t)N * d, cudaMemcpyDeviceToHost, s);
+  };
+  cudaError_t e = cudaSuccess;
+  if (hx) e = rows(c->st.x, hx);
+  if (e == cudaSuccess && hscore) {
+    if (c->cp.grad) e = rows(c->st.g, hscore);
+    else { e = cudaStreamSynchronize(s); std::memset(hscore, 0, sizeof(float) * (size_t)N * d); }
+  }
+  if (e == cudaSuccess && hp) { k_fp_split<<<g, 256, 0, s>>>(c->st.fp, tmp, nullptr, N); e = cudaMemcpyAsync(hp, tmp, 4 * (size_t)N, cudaMemcpyDeviceToHost, s); }
+  if (e == cudaSuccess && hfop) { k_fp_split<<<g, 256, 0, s>>>(c->st.fp, nullptr, tmp, N); e = cudaMemcpyAsync(hfop, tmp, 12 * (size_t)N, cudaMemcpyDeviceToHost, s); }
+  if (e == cudaSuccess && hpix) e = cudaMemcpyAsync(hpix, c->st.pix, 4 * (size_t)N, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess && hsig) e = cudaMemcpyAsync(hsig, c->st.sig, 4 * (size_t)N, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess && hkilled) e = cudaMemcpyAsync(hkilled, c->st.killed, N, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(tmp);
+  if (e != cudaSuccess) r = fail(DR_ERR_CUDA, std::string("download: ") + cudaGetErrorString(e));
+  return r;
+}
+
+dr_status dr_chains_upload(dr_chains* c, const float* hx, const float* hp, const float* hfop, const uint32_t* hpix,
+                           const uint8_t* hkilled, const float* hscore, uint32_t iteration, void* stream) {
+  if (!c || !hx || !hp || !hfop || !hpix || !hkilled) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (c->cp.grad && !hscore) return fail(DR_ERR_INVALID_ARG, "score required for gradient methods");
+  if (!c->initialised) return fail(DR_ERR_INVALID_ARG, "dr_chains_init has not been called");
+  cudaStream_t s = (cudaStream_t)stream;
+  const uint32_t N = c->cp.N, d = c->cp.d, g = (N + 255) / 256;
+  float *t0 = nullptr, *t1 = nullptr;
+  CUDA_TRY(cudaMalloc(&t0, sizeof(float) * (size_t)N * (d > 4 ? d : 4)));
+  cudaError_t e = cudaMalloc(&t1, sizeof(float) * (size_t)N * 4);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(t0, hx, sizeof(float) * (size_t)N * d, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) k_rows_to_planes<<<g, 256, 0, s>>>(t0, c->st.x, N, d, c->cp.planes);
+  if (e == cudaSuccess && c->cp.grad) {
+    e = cudaMemcpyAsync(t0, hscore, sizeof(float) * (size_t)N * d, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) k_rows_to_planes<<<g, 256, 0, s>>>(t0, c->st.g, N, d, c->cp.planes);
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(t0, hp, 4 * (size_t)N, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(t1, hfop, 12 * (size_t)N, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) k_fp_join<<<g, 256, 0, s>>>(t0, t1, c->st.fp, N);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(c->st.pix, hpix, 4 * (size_t)N, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(c->st.killed, hkilled, N, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess && c->cp.restore) {
+    k_count_killed<<<c->nblocks, kBlock, 0, s>>>(c->cp, c->st);
+    k_scan<<<1, 1024, 0, s>>>(c->st, c->nblocks);
+    k_scatter<<<c->nblocks, kBlock, 0, s>>>(c->cp, c->st);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(t0); cudaFree(t1);
+  if (e != cudaSuccess) return fail(DR_ERR_CUDA, std::string("upload: ") + cudaGetErrorString(e));
+  c->iteration = iteration;
+  return DR_OK;
+}
+
+dr_status dr_chains_last_step(dr_chains* c, uint8_t* hacc, float* hw, void* stream) {
+  if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
+  cudaStream_t s = (cudaStream_t)stream;
+  if (hacc) CUDA_TRY(cudaMemcpyAsync(hacc, c->st.accepted, c->cp.N, cudaMemcpyDeviceToHost, s));
+  if (hw) CUDA_TRY(cudaMemcpyAsync(hw, c->st.weight, 4 * (size_t)c->cp.N, cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(cudaStreamSynchronize(s));
+  return DR_OK;
+}
+
+dr_status dr_regen_queue_download(dr_chains* c, uint32_t* hids, uint32_t* hlen, void* stream) {
+  if (!c || !hlen) return fail(DR_ERR_INVALID_ARG, "null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  *hlen = 0;
+  if (!c->cp.restore) return DR_OK;
+  uint32_t q = 0;
+  CUDA_TRY(cudaMemcpyAsync(&q, &c->st.ctr->queue_len, 4, cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(cudaStreamSynchronize(s));
+  *hlen = q;
+  if (hids && q) {
+    CUDA_TRY(cudaMemcpyAsync(hids, c->st.order + (c->cp.N - q), 4 * (size_t)q, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+  }
+  return DR_OK;
+}
+
+dr_status dr_trace_rays(const dr_scene* sc, const float* o, const float* d, uint32_t n, float* t, uint32_t* prim, void* stream) {
+  if (!sc || !o || !d || !t || !prim) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (sc->dev.analytic) return fail(DR_ERR_UNSUPPORTED, "analytic scene has no geometry");
+  if (!n) return DR_OK;
+  const size_t sm = smem_bytes(sc);
+  k_trace<<<(n + kEvalBlock - 1) / kEvalBlock, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, o, d, n, t, prim);
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;
+}
+
+dr_status dr_eval_states(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score,
+                         uint32_t* nrays, uint32_t* sig, void* stream) {
+  if (!sc || !x || !f || !p || !pix || !nrays || !sig) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (!n) return DR_OK;
+  const size_t sm = smem_bytes(sc);
+  const uint32_t g = (n + kEvalBlock - 1) / kEvalBlock;
+  if (score) k_eval_states<true><<<g, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, x, n, f, p, pix, score, nrays, sig);
+  else k_eval_states<false><<<g, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, x, n, f, p, pix, nullptr, nrays, sig);
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;
+}
+
+dr_status dr_philox_blocks(uint64_t seed, const uint32_t* ctr, uint32_t n, uint32_t* out, void* stream) {
+  if (!ctr || !out) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (!n) return DR_OK;
+  k_philox_blocks<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(seed, ctr, n, out);
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;
+}
+
+dr_status dr_rng_transforms(const uint32_t* words, uint32_t n, float* out, void* stream) {
+  if (!words || !out) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (!n) return DR_OK;
+  k_rng_transforms<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(words, n, out);
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;
+}
+
+}  // extern "C"
