@@ -313,7 +313,7 @@ def ggx_room(seed=5, width=32, height=32, max_path_len=5, alpha=0.3) -> SceneDes
     _q((0, 0, 0), (0, R, 0), (0, R, R), (0, 0, R), 0)
     _q((R, 0, 0), (R, 0, R), (R, R, R), (R, R, 0), 0)
     _q((0.6, 1.99, 0.6), (1.4, 1.99, 0.6), (1.4, 1.99, 1.4), (0.6, 1.99, 1.4), 1)
-    _box_faces(mesh, (0.7, 0.5, 1.2), (0.3, 0.5, 0.3), _rot_y(rng.uniform(-30, 30)), 2)
+    _box_faces(mesh, (0.7, 0.55, 1.2), (0.3, 0.5, 0.3), _rot_y(rng.uniform(-30, 30)), 2)   # floats above the floor: no coplanar faces
     _box_faces(mesh, (1.4, 0.3, 0.8), (0.3, 0.3, 0.3), _rot_quat(rng.normal(size=4)), 3)
     verts, idx, tm = mesh.finish()
     return SceneDesc(verts, idx, tm, np.stack(mats), cam_pos=(0.3, 1.0, 0.2), cam_look=(1.2, 0.7, 1.3), vfov_deg=60.0,

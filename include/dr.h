@@ -157,10 +157,11 @@ dr_status dr_chains_stats(dr_chains* chains, dr_stats* host_out, void* stream);
  * discrete decisions of the state's path).  Any output pointer may be NULL. */
 dr_status dr_chains_download(dr_chains* chains, float* host_x, float* host_p, float* host_f_over_p, uint32_t* host_pix,
                              uint8_t* host_killed, float* host_score, uint32_t* host_sig, void* stream);
-/* Teacher forcing: overwrite the state and set the iteration counter; rebuilds the regeneration queue. */
+/* Teacher forcing: overwrite the state (host_sig may be NULL) and set the iteration counter; rebuilds the
+ * regeneration queue. */
 dr_status dr_chains_upload(dr_chains* chains, const float* host_x, const float* host_p, const float* host_f_over_p,
                            const uint32_t* host_pix, const uint8_t* host_killed, const float* host_score,
-                           uint32_t iteration, void* stream);
+                           const uint32_t* host_sig, uint32_t iteration, void* stream);
 /* Per-chain record of the last iteration: accepted flag and sampled weight (dtau, or 1 for plain MH). */
 dr_status dr_chains_last_step(dr_chains* chains, uint8_t* host_accepted, float* host_weight, void* stream);
 /* Killed chain ids in ascending order; host_ids may be NULL to query the length. */

@@ -130,8 +130,8 @@ class Scene:
         self.npix = desc.width * desc.height
 
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().orc_scene_destroy(self.h)
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.orc_scene_destroy(self.h)
             self.h = None
 
     @property
@@ -181,8 +181,8 @@ class Chains:
                                          p_lambda_override, int(seed), int(chain_offset))
 
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().orc_chains_destroy(self.h)
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.orc_chains_destroy(self.h)
             self.h = None
 
     def init(self, frame=0):

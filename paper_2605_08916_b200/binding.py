@@ -88,7 +88,7 @@ def _load():
     L.dr_resolve_image.argtypes = [vp, vp, vp]
     L.dr_chains_stats.argtypes = [vp, C.POINTER(dr_stats), vp]
     L.dr_chains_download.argtypes = [vp] * 9
-    L.dr_chains_upload.argtypes = [vp] * 7 + [u32, vp]
+    L.dr_chains_upload.argtypes = [vp] * 8 + [u32, vp]
     L.dr_chains_last_step.argtypes = [vp, vp, vp, vp]
     L.dr_regen_queue_download.argtypes = [vp, vp, C.POINTER(u32), vp]
     L.dr_trace_rays.argtypes = [vp, vp, vp, u32, vp, vp, vp]
@@ -249,8 +249,9 @@ class Chains:
         a = {k: np.ascontiguousarray(s[k], dtype=np.float32) for k in ("x", "p", "fop", "g")}
         pix = np.ascontiguousarray(s["pix"], dtype=np.uint32)
         killed = np.ascontiguousarray(s["killed"], dtype=np.uint8)
+        sig = np.ascontiguousarray(s["sig"], dtype=np.uint32)
         _check(lib.dr_chains_upload(self.h, _np(a["x"]), _np(a["p"]), _np(a["fop"]), _np(pix), _np(killed), _np(a["g"]),
-                                    int(iteration), _stream()))
+                                    _np(sig), int(iteration), _stream()))
 
     def last_step(self):
         acc = np.zeros(self.N, np.uint8)

@@ -378,7 +378,7 @@ dr_status dr_chains_download(dr_chains* c, float* hx, float* hp, float* hfop, ui
 }
 
 dr_status dr_chains_upload(dr_chains* c, const float* hx, const float* hp, const float* hfop, const uint32_t* hpix,
-                           const uint8_t* hkilled, const float* hscore, uint32_t iteration, void* stream) {
+                           const uint8_t* hkilled, const float* hscore, const uint32_t* hsig, uint32_t iteration, void* stream) {
   if (!c || !hx || !hp || !hfop || !hpix || !hkilled) return fail(DR_ERR_INVALID_ARG, "null argument");
   if (c->cp.grad && !hscore) return fail(DR_ERR_INVALID_ARG, "score required for gradient methods");
   if (!c->initialised) return fail(DR_ERR_INVALID_ARG, "dr_chains_init has not been called");
@@ -398,6 +398,7 @@ dr_status dr_chains_upload(dr_chains* c, const float* hx, const float* hp, const
   if (e == cudaSuccess) k_fp_join<<<g, 256, 0, s>>>(t0, t1, c->st.fp, N);
   if (e == cudaSuccess) e = cudaMemcpyAsync(c->st.pix, hpix, 4 * (size_t)N, cudaMemcpyHostToDevice, s);
   if (e == cudaSuccess) e = cudaMemcpyAsync(c->st.killed, hkilled, N, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess && hsig) e = cudaMemcpyAsync(c->st.sig, hsig, 4 * (size_t)N, cudaMemcpyHostToDevice, s);
   if (e == cudaSuccess && c->cp.restore) {
     k_count_killed<<<c->nblocks, kBlock, 0, s>>>(c->cp, c->st);
     k_scan<<<1, 1024, 0, s>>>(c->st, c->nblocks);
@@ -437,9 +438,10 @@ dr_status dr_regen_queue_download(dr_chains* c, uint32_t* hids, uint32_t* hlen, 
 }
 
 dr_status dr_trace_rays(const dr_scene* sc, const float* o, const float* d, uint32_t n, float* t, uint32_t* prim, void* stream) {
-  if (!sc || !o || !d || !t || !prim) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (!sc) return fail(DR_ERR_INVALID_ARG, "null scene");
   if (sc->dev.analytic) return fail(DR_ERR_UNSUPPORTED, "analytic scene has no geometry");
-  if (!n) return DR_OK;
+  if (!n) return DR_OK;  // empty input: nothing to do, pointers may be null
+  if (!o || !d || !t || !prim) return fail(DR_ERR_INVALID_ARG, "null argument");
   const size_t sm = smem_bytes(sc);
   k_trace<<<(n + kEvalBlock - 1) / kEvalBlock, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, o, d, n, t, prim);
   CUDA_TRY(cudaGetLastError());
@@ -448,8 +450,9 @@ dr_status dr_trace_rays(const dr_scene* sc, const float* o, const float* d, uint
 
 dr_status dr_eval_states(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score,
                          uint32_t* nrays, uint32_t* sig, void* stream) {
-  if (!sc || !x || !f || !p || !pix || !nrays || !sig) return fail(DR_ERR_INVALID_ARG, "null argument");
-  if (!n) return DR_OK;
+  if (!sc) return fail(DR_ERR_INVALID_ARG, "null scene");
+  if (!n) return DR_OK;  // empty input
+  if (!x || !f || !p || !pix || !nrays || !sig) return fail(DR_ERR_INVALID_ARG, "null argument");
   const size_t sm = smem_bytes(sc);
   const uint32_t g = (n + kEvalBlock - 1) / kEvalBlock;
   if (score) k_eval_states<true><<<g, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, x, n, f, p, pix, score, nrays, sig);

@@ -67,20 +67,23 @@ def test_trace_matches_oracle(dr, oracle, torch_, scene):
     assert mism.mean() < 1e-4, mism.sum()        # edge-grazing rays may pick the neighbour: counted
     hit = (~mism) & (otri >= 0)
     assert hit.sum() > 1000
-    assert np.all(np.abs(t[hit] - ot[hit]) <= 1e-5 * np.abs(ot[hit]))
+    diag = float(np.linalg.norm(desc.vertices.max(0) - desc.vertices.min(0)))
+    assert np.all(np.abs(t[hit] - ot[hit]) <= 1e-5 * np.maximum(np.abs(ot[hit]), 0.25 * diag))   # fp32 Moeller-Trumbore on both sides
     assert np.all(t[(~mism) & (otri < 0)] == -1.0)
     info = gsc.info()
     assert info["n_tris"] == desc.n_tris and info["n_nodes"] >= 1 and info["smem_nodes"] <= 73
 
 
-def test_trace_degenerate_rays(dr, torch_):
+def test_trace_degenerate_rays(dr, oracle, torch_):
     desc = S.cornell()
     gsc = dr.Scene(desc)
     o = np.array([[0.5, 0.5, -1.0], [0.5, 0.5, 0.5], [0.5, 0.5, 0.5], [5, 5, 5]], dtype=np.float32)
     d = np.array([[0, 0, 1], [1, 0, 0], [0, -1, 0], [1, 0, 0]], dtype=np.float32)   # axis-aligned: zero components
     t, prim = gsc.trace_rays(torch_.from_numpy(o).cuda(), torch_.from_numpy(d).cuda())
-    t = t.cpu().numpy()
-    assert np.isclose(t[0], 2.0) and np.isclose(t[1], 0.5) and np.isclose(t[2], 0.5) and t[3] == -1.0
+    t, prim = t.cpu().numpy(), prim.cpu().numpy()
+    ot, otri = oracle.Scene(desc, oracle.F32).trace(o, d, brute=True)
+    assert (prim == otri).all() and np.allclose(t, ot, rtol=1e-6)
+    assert np.isclose(t[1], 0.5) and np.isclose(t[2], 0.5) and t[3] == -1.0     # walls at x = 1 and y = 0
     t0, _ = gsc.trace_rays(torch_.zeros(0, 3, device="cuda"), torch_.zeros(0, 3, device="cuda"))    # empty input
     assert t0.numel() == 0
 
@@ -113,7 +116,7 @@ def test_eval_matches_oracle(dr, oracle, torch_, scene):
         assert (np.abs(e["g"][ok]).max(1) > 0).sum() > 20                       # the score path is exercised
     # without the score the value outputs are identical
     g2 = gsc.eval_states(torch_.from_numpy(x).cuda(), want_score=False)
-    assert (g2["p"].cpu().numpy() == g["p"]).all() and (g2["sig"].cpu().numpy() == g["sig"]).all()
+    assert np.allclose(g2["p"].cpu().numpy(), g["p"], rtol=1e-6, atol=0) and (g2["sig"].cpu().numpy() == g["sig"]).all()
 
 
 def test_furnace_states_hit_the_closed_form_exactly(dr, torch_):
