@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the Diffusion Restore hot path on B200 (BASELINE.json metric).
+
+A "step" is one frame of BASELINE.json configs[3] (the 1024x576 'transparent machines' scene, 589 824 chains,
+one chain per pixel): dr_step(1 iteration) + dr_resolve_image, i.e. every row a1-a12 of SURVEY.md section 8(a).
+Prints ONE JSON line (see the contract in the task statement).  `--impl reference` times the CPU oracle instead.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "chain mutations/s at 1024x576 (Diffusion Restore, transparent-machines scene)"
+UNIT = "mutations/s"
+# Algorithmic FLOPs of the path evaluation: one BVH8 node visit = 8 slab tests of
+# 6 FMA + 12 min/max = 192 FLOP; one Moeller-Trumbore test = 50 FLOP; shading one vertex = 150 FLOP.
+F_NODE, F_TRI, F_SHADE = 192.0, 50.0, 150.0
+# Algorithmic bytes per mutation of the state-streaming kernels (propose + decide + scan + scatter), d = 2L:
+# read x, score (2 * 4d) + write x, score (2 * 4d) + p, f/p_hat, pixel, flags read and written (2 * 21).
+def stream_bytes_per_mutation(d, grad):
+    return (4 if grad else 2) * 4 * d + 42
+
+
+def make_desc(name):
+    from dr_inputs import scenes as S
+    return {"machines": S.machines, "cornell": S.cornell, "caustic": S.caustic, "furnace": S.furnace,
+            "mini_machines": S.mini_machines}[name]()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for t, line in self.rows:
+            f = [c.strip() for c in line.split(",")]
+            if len(f) < 9 or not (t0 - 0.05 <= t <= t1 + 0.15):
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no sample inside the timed region"], samples=0)
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(np.max(mx)), reasons=sorted(reasons), samples=len(sm))
+
+
+def cpu_baseline(desc, method, n_chains, iterations, seed):
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    from oracle import oracle as O
+    sc = O.Scene(desc, O.F32)
+    ch = O.Chains(sc, method, n_chains, seed=seed)
+    ch.init(0)
+    r0 = ch.stats()["rays"]
+    t = time.perf_counter()
+    ch.step(iterations)
+    dt = time.perf_counter() - t
+    st = ch.stats()
+    return dict(value=n_chains * iterations / dt, unit=UNIT, cores=O.max_threads(), kind="oracle",
+                sample=f"{desc.name}: {n_chains} chains x {iterations} iterations after init, {method}, fp32 oracle, OpenMP",
+                mrays_per_s=(st["rays"] - r0) / dt / 1e6, seconds=dt)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, one bounded step = 8192 chains x 1 iteration of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    desc = make_desc(args.scene)
+    n = 8192
+    sc = O.Scene(desc, O.F32)
+    ch = O.Chains(sc, args.method, n, seed=4)
+    ch.init(0)
+    ch.step(args.warmup)
+    r0 = ch.stats()["rays"]
+    t = time.perf_counter()
+    ch.step(args.steps)
+    dt = time.perf_counter() - t
+    val = n * args.steps / dt
+    sample = f"{desc.name}: {n} chains x 1 iteration per step, {args.method}, fp32 oracle, OpenMP"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"configs[3] {desc.name} {desc.width}x{desc.height}, {desc.n_tris} triangles, L={desc.max_path_len}",
+                   "method": args.method, "chains_per_step": n},
+        "mrays_per_s": (ch.stats()["rays"] - r0) / dt / 1e6,
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=120)       # configs[3]: 120 frames after init
+    ap.add_argument("--warmup", type=int, default=8)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--method", default="diffusion_restore")
+    ap.add_argument("--scene", default="machines")
+    ap.add_argument("--chains", type=int, default=0, help="chains per GPU (default: one per pixel)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2605_08916_b200 import build as gpu_build
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if rank == 0:
+        gpu_build.build()
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    import paper_2605_08916_b200 as dr
+    from paper_2605_08916_b200 import sharding
+
+    desc = make_desc(args.scene)
+    scene = dr.Scene(desc)
+    n_local = args.chains or desc.width * desc.height            # weak scaling: every GPU runs one chain per pixel
+    offset = sharding.shard_offset(n_local, rank)
+    # sharded runs need the same p_lambda on every shard: fix it from a rank-0 bootstrap
+    p_override = 0.0
+    if world > 1:
+        probe = dr.Chains(scene, args.method, n_local, seed=4, chain_offset=0)
+        probe.init(0)
+        t = torch.tensor([probe.stats()["p_lambda"]], device="cuda")
+        dist.broadcast(t, 0)
+        p_override = float(t.item())
+        del probe
+    chains = dr.Chains(scene, args.method, n_local, seed=4, chain_offset=offset, p_lambda_override=p_override)
+    stream = torch.cuda.current_stream()
+
+    def frame():
+        chains.step(1)
+        if world > 1:
+            acc, tours, muts = sharding.allreduce_frame(chains.accum, chains)
+            chains.resolve_sharded(acc, tours, muts)
+        else:
+            chains.resolve()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    e0, e1 = ev(), ev()
+    e0.record(stream); chains.init(0); e1.record(stream); torch.cuda.synchronize()
+    init_ms = e0.elapsed_time(e1)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    for _ in range(args.warmup):
+        frame()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    st0 = chains.stats()
+    chains.profile_enable(True)
+    per = [(ev(), ev()) for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    t_wall0 = time.time()
+    e0.record(stream)
+    for a, b in per:
+        a.record(stream); frame(); b.record(stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t_wall1 = time.time()
+    total_ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    prof = chains.profile_read()
+    chains.profile_enable(False)
+    st1 = chains.stats()
+    frame_ms = sorted(a.elapsed_time(b) for a, b in per)
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    work = chains.work_stats()
+
+    rays_local = st1["rays"] - st0["rays"]
+    rays_total = rays_local
+    if world > 1:
+        t = torch.tensor([rays_local], device="cuda", dtype=torch.int64)
+        dist.all_reduce(t)
+        rays_total = int(t.item())
+    mutations = n_local * world * args.steps
+    value = mutations / (total_ms * 1e-3)
+
+    # ---- end to end: host owns the chain state; every step uploads it, steps, resolves, and reads image + state back
+    e2e = None
+    if rank == 0:
+        st = chains.download()
+        host = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in st.items()}
+        img_host = torch.empty(desc.height, desc.width, 3, dtype=torch.float32).pin_memory()
+        h2d = sum(host[k].numel() * host[k].element_size() for k in ("x", "p", "fop", "pix", "killed", "g", "sig"))
+        d2h = h2d + img_host.numel() * 4
+        it = st1["iteration"]
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for k in range(args.e2e_steps):
+            chains.upload({kk: vv.numpy() for kk, vv in host.items()}, it + k)
+            chains.step(1)
+            img, _ = chains.resolve()
+            img_host.copy_(img, non_blocking=True)
+            st = chains.download()
+            for kk in host:
+                host[kk].copy_(torch.from_numpy(st[kk]))
+        e1.record(stream)
+        torch.cuda.synchronize()
+        e2e_ms = e0.elapsed_time(e1)
+        e2e = {"value": n_local * args.e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.e2e_steps, "steps": args.e2e_steps,
+               "what": "host-owned chain state: dr_chains_upload (pinned host -> device) + dr_step(1) + dr_resolve_image + "
+                       "image and dr_chains_download back to host, every step, N = 1 GPU"}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    nodes_per_ray = work["node_visits"] / max(work["rays"], 1)
+    tris_per_ray = work["tri_tests"] / max(work["rays"], 1)
+    flop_per_ray = F_NODE * nodes_per_ray + F_TRI * tris_per_ray + F_SHADE
+    eval_ms = prof["eval"]["ms"] / max(prof["eval"]["launches"], 1)
+    rays_per_launch = rays_local / max(prof["eval"]["launches"], 1)
+    alu_peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+    achieved = flop_per_ray * rays_per_launch / (eval_ms * 1e-3) / 1e12
+    grad = args.method in ("mala", "mala_restore", "diffusion_restore")
+    stream_ms = sum(prof[k]["ms"] for k in ("propose", "decide", "scan", "scatter")) / args.steps
+    stream_gbs = stream_bytes_per_mutation(desc.dim, grad) * n_local / (stream_ms * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "r01_eval_traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get("dram_bytes_per_launch")
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"configs[3] {desc.name} {desc.width}x{desc.height}, {desc.n_tris} triangles, L={desc.max_path_len} (d={desc.dim})",
+                   "method": args.method, "chains_per_gpu": n_local, "iterations_per_frame": 1,
+                   "l2": "chain state (%.0f MB) larger than L2; no flush" % (chains.state.numel() / 1e6),
+                   "seed": 4, "stddev": float(chains.cfg.stddev), "c_tilde": float(chains.cfg.c_tilde), "dt": float(chains.cfg.dt),
+                   "m": float(chains.cfg.m)},
+        "mrays_per_s": rays_total / (total_ms * 1e-3) / 1e6,
+        "ms_per_frame": {"mean": total_ms / args.steps, "median": frame_ms[len(frame_ms) // 2], "min": frame_ms[0], "max": frame_ms[-1]},
+        "init_ms": init_ms,
+        "workload_stats": {"rays_per_mutation": rays_local / (n_local * args.steps), "nodes_per_ray": nodes_per_ray,
+                           "tris_per_ray": tris_per_ray, "kill_fraction_last": st1["kills_last_step"] / n_local,
+                           "tours": st1["tours"], "p_lambda": st1["p_lambda"], "nonfinite": st1["nonfinite"]},
+        "kernels_ms_per_frame": {k: v["ms"] / args.steps for k, v in prof.items()},
+        "gpu_launches": int(sum(v["launches"] for v in prof.values())),
+        "clocks": clocks,
+        "roofline": {"kernel": "k_eval<GRAD>" if grad else "k_eval", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+                     "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": traffic,
+                     "peak_source": f"148 SM x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
+                     "flop_per_ray": flop_per_ray, "rays_per_launch": rays_per_launch, "launch_ms": eval_ms},
+        "roofline_streaming": {"kernels": "k_propose+k_decide+k_scan+k_scatter", "bound": "hbm", "achieved": stream_gbs,
+                               "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": stream_gbs / pk["hbm_gbs"],
+                               "bytes_per_mutation": stream_bytes_per_mutation(desc.dim, grad), "ms_per_frame": stream_ms,
+                               "peak_source": pk["source"]},
+        "e2e": e2e,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(desc, args.method, 32768, 6, 4)
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

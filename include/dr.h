@@ -149,6 +149,24 @@ dr_status dr_step(dr_chains* chains, int32_t method, uint32_t iterations, void* 
  * (plain MH).  Returns DR_WARN_NO_TOURS and writes zeros if tourCount == 0 (the check synchronises the stream). */
 dr_status dr_resolve_image(dr_chains* chains, float* dev_rgb_out, void* stream);
 
+/* Alg. 3 for a run sharded over several GPUs: dev_accum_sum is the all-reduced accumulation buffer
+ * (W*H float4), tours_total / mutations_total the all-reduced counters (mutations_total > 0).  p_lambda and kappa0
+ * are this shard's; they are identical on every shard when p_lambda_override is used.  Asynchronous. */
+dr_status dr_resolve_image_sharded(dr_chains* chains, const float* dev_accum_sum, uint64_t tours_total,
+                                   uint64_t mutations_total, float* dev_rgb_out, void* stream);
+
+/* Per-kernel timing with CUDA events on the caller's stream (bench.py's roofline).  dr_profile_enable(on) resets
+ * the totals; while on, every kernel launch of dr_chains_init / dr_step / dr_resolve_image* is bracketed by two
+ * events.  dr_profile_read synchronises the stream and returns, per kernel class, the summed device time in ms and
+ * the number of launches (arrays of DR_PROF_COUNT entries). */
+enum { DR_PROF_PROPOSE = 0, DR_PROF_EVAL = 1, DR_PROF_DECIDE = 2, DR_PROF_SCAN = 3, DR_PROF_SCATTER = 4,
+       DR_PROF_RESOLVE = 5, DR_PROF_COUNT = 6 };
+dr_status dr_profile_enable(dr_chains* chains, int32_t on, void* stream);
+dr_status dr_profile_read(dr_chains* chains, double* host_ms, uint64_t* host_launches, void* stream);
+/* Work of the last evaluation launch: host_out3 = {rays, BVH8 node visits, triangle tests} of the chains' last
+ * proposals (re-evaluated with counters; values only).  Synchronises. */
+dr_status dr_chains_work_stats(dr_chains* chains, uint64_t* host_out3, void* stream);
+
 /* Synchronises the stream and copies the counters. */
 dr_status dr_chains_stats(dr_chains* chains, dr_stats* host_out, void* stream);
 
@@ -173,6 +191,9 @@ dr_status dr_trace_rays(const dr_scene* scene, const float* dev_o, const float* 
  * non-NULL), nrays[n], sig[n]. */
 dr_status dr_eval_states(const dr_scene* scene, const float* dev_x, uint32_t n, float* dev_f, float* dev_p,
                          uint32_t* dev_pix, float* dev_score, uint32_t* dev_nrays, uint32_t* dev_sig, void* stream);
+/* Work statistics for n states (device x[n*d], values only): dev_out3[0..2] += {rays, BVH8 node visits, triangle
+ * tests}.  bench.py derives the algorithmic FLOPs per ray of its roofline from these. */
+dr_status dr_eval_work_stats(const dr_scene* scene, const float* dev_x, uint32_t n, uint64_t* dev_out3, void* stream);
 /* Raw Philox blocks for n counters (device arrays ctr[4n] -> out[4n]) under key (seed lo, hi), and the stream
  * transforms of DESIGN.md Q14 for n words pairs: out[4n] = u[0,1), u(0,1], Box-Muller z0, z1. */
 dr_status dr_philox_blocks(uint64_t seed, const uint32_t* dev_ctr, uint32_t n, uint32_t* dev_out, void* stream);

@@ -23,8 +23,10 @@ EXPORTS = [
     "dr_last_error", "dr_scene_create", "dr_scene_create_analytic2d", "dr_scene_destroy", "dr_scene_get_info",
     "dr_chains_state_bytes", "dr_chains_create", "dr_chains_destroy", "dr_chains_init", "dr_step", "dr_resolve_image",
     "dr_chains_stats", "dr_chains_download", "dr_chains_upload", "dr_chains_last_step", "dr_regen_queue_download",
-    "dr_trace_rays", "dr_eval_states", "dr_philox_blocks", "dr_rng_transforms",
+    "dr_trace_rays", "dr_eval_states", "dr_philox_blocks", "dr_rng_transforms", "dr_resolve_image_sharded",
+    "dr_eval_work_stats", "dr_profile_enable", "dr_profile_read", "dr_chains_work_stats",
 ]
+PROF_NAMES = ["propose", "eval", "decide", "scan", "scatter", "resolve"]
 
 
 class dr_material(C.Structure):
@@ -93,6 +95,11 @@ def _load():
     L.dr_regen_queue_download.argtypes = [vp, vp, C.POINTER(u32), vp]
     L.dr_trace_rays.argtypes = [vp, vp, vp, u32, vp, vp, vp]
     L.dr_eval_states.argtypes = [vp, vp, u32, vp, vp, vp, vp, vp, vp, vp]
+    L.dr_resolve_image_sharded.argtypes = [vp, vp, u64, u64, vp, vp]
+    L.dr_eval_work_stats.argtypes = [vp, vp, u32, vp, vp]
+    L.dr_profile_enable.argtypes = [vp, i32, vp]
+    L.dr_profile_read.argtypes = [vp, vp, vp, vp]
+    L.dr_chains_work_stats.argtypes = [vp, vp, vp]
     L.dr_philox_blocks.argtypes = [u64, vp, u32, vp, vp]
     L.dr_rng_transforms.argtypes = [vp, u32, vp, vp]
     for name in EXPORTS:
@@ -176,6 +183,12 @@ class Scene:
         _check(lib.dr_trace_rays(self.h, _dp(o.contiguous()), _dp(d.contiguous()), n, _dp(t), _dp(prim), _stream()))
         return t, prim
 
+    def eval_work_stats(self, x: torch.Tensor) -> dict:
+        out = torch.zeros(3, dtype=torch.int64, device="cuda")
+        _check(lib.dr_eval_work_stats(self.h, _dp(x.contiguous()), x.shape[0], _dp(out), _stream()))
+        r, n, t = (int(v) for v in out.cpu())
+        return dict(rays=r, node_visits=n, tri_tests=t)
+
     def eval_states(self, x: torch.Tensor, want_score=True):
         x = x.contiguous()
         n = x.shape[0]
@@ -228,6 +241,25 @@ class Chains:
     def resolve(self):
         status = _check(lib.dr_resolve_image(self.h, _dp(self.image), _stream()), allow_warn=True)
         return self.image, status
+
+    def resolve_sharded(self, accum_sum: torch.Tensor, tours_total: int, mutations_total: int):
+        status = _check(lib.dr_resolve_image_sharded(self.h, _dp(accum_sum), int(tours_total), int(mutations_total),
+                                                     _dp(self.image), _stream()), allow_warn=True)
+        return self.image, status
+
+    def profile_enable(self, on=True):
+        _check(lib.dr_profile_enable(self.h, int(on), _stream()))
+
+    def profile_read(self) -> dict:
+        ms = np.zeros(len(PROF_NAMES), np.float64)
+        n = np.zeros(len(PROF_NAMES), np.uint64)
+        _check(lib.dr_profile_read(self.h, _np(ms), _np(n), _stream()))
+        return {k: dict(ms=float(a), launches=int(b)) for k, a, b in zip(PROF_NAMES, ms, n)}
+
+    def work_stats(self) -> dict:
+        o = np.zeros(3, np.uint64)
+        _check(lib.dr_chains_work_stats(self.h, _np(o), _stream()))
+        return dict(rays=int(o[0]), node_visits=int(o[1]), tri_tests=int(o[2]))
 
     def stats(self) -> dict:
         o = dr_stats()

@@ -59,6 +59,14 @@ struct dr_chains {
   bool initialised = false;
   size_t state_bytes = 0;
   void* state_base = nullptr;
+  // optional per-kernel timing (dr_profile_*): cudaEvent pairs recorded around every launch
+  bool profiling = false;
+  std::vector<cudaEvent_t> ev;     // pool
+  std::vector<int> ev_kind;        // kernel class of pair k (events 2k, 2k+1)
+  size_t ev_used = 0;              // pairs in use
+  double prof_ms[DR_PROF_COUNT] = {0, 0, 0, 0, 0, 0};
+  uint64_t prof_launches[DR_PROF_COUNT] = {0, 0, 0, 0, 0, 0};
+  ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
 };
 
 namespace {
@@ -110,23 +118,54 @@ dr_status check_config(const dr_config* c) {
 
 size_t smem_bytes(const dr_scene* s) { return (size_t)s->dev.smem_nodes * sizeof(Node8); }
 
+constexpr size_t kMaxPairs = 8192;
+
+// Folds finished event pairs into the per-class totals (requires the stream to be idle).
+void prof_drain(dr_chains* c) {
+  for (size_t k = 0; k < c->ev_used; ++k) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->ev[2 * k], c->ev[2 * k + 1]) == cudaSuccess) {
+      c->prof_ms[c->ev_kind[k]] += ms;
+      c->prof_launches[c->ev_kind[k]] += 1;
+    }
+  }
+  c->ev_used = 0;
+}
+
+struct ProfScope {
+  dr_chains* c; cudaStream_t s; size_t k; bool on;
+  ProfScope(dr_chains* c_, int kind, cudaStream_t s_) : c(c_), s(s_), k(0), on(c_->profiling) {
+    if (!on) return;
+    if (c->ev_used == kMaxPairs) { cudaStreamSynchronize(s); prof_drain(c); }
+    k = c->ev_used++;
+    while (c->ev.size() < 2 * (k + 1)) { cudaEvent_t e; cudaEventCreate(&e); c->ev.push_back(e); }
+    if (c->ev_kind.size() <= k) c->ev_kind.resize(k + 1);
+    c->ev_kind[k] = kind;
+    cudaEventRecord(c->ev[2 * k], s);
+  }
+  ~ProfScope() { if (on) cudaEventRecord(c->ev[2 * k + 1], s); }
+};
+
 // evaluation of all proposals (+ the kernels that must precede / follow it)
 dr_status launch_iteration(dr_chains* c, uint32_t n, bool init, cudaStream_t s) {
   const ChainParams& cp = c->cp;
   const uint32_t gb = c->nblocks, ge = (cp.N + kEvalBlock - 1) / kEvalBlock;
-  k_propose<<<gb, kBlock, 0, s>>>(cp, c->st, n, init ? 1 : 0);
+  { ProfScope ps(c, DR_PROF_PROPOSE, s); k_propose<<<gb, kBlock, 0, s>>>(cp, c->st, n, init ? 1 : 0); }
   const int use_order = (!init && cp.restore) ? 1 : 0;
   const size_t sm = smem_bytes(c->scene);
-  if (cp.grad) k_eval<true><<<ge, kEvalBlock, sm, s>>>(c->scene->dev, cp, c->st, use_order);
-  else k_eval<false><<<ge, kEvalBlock, sm, s>>>(c->scene->dev, cp, c->st, use_order);
+  {
+    ProfScope ps(c, DR_PROF_EVAL, s);
+    if (cp.grad) k_eval<true><<<ge, kEvalBlock, sm, s>>>(c->scene->dev, cp, c->st, use_order);
+    else k_eval<false><<<ge, kEvalBlock, sm, s>>>(c->scene->dev, cp, c->st, use_order);
+  }
   if (init) {
     k_psum_partial<<<gb, kBlock, 0, s>>>(cp, c->st);
     k_bootstrap<<<1, kBlock, 0, s>>>(cp, c->st, gb);
   }
-  k_decide<<<gb, kBlock, 0, s>>>(cp, c->st, c->accum, n);
+  { ProfScope ps(c, DR_PROF_DECIDE, s); k_decide<<<gb, kBlock, 0, s>>>(cp, c->st, c->accum, n); }
   if (cp.restore) {
-    k_scan<<<1, 1024, 0, s>>>(c->st, gb);
-    k_scatter<<<gb, kBlock, 0, s>>>(cp, c->st);
+    { ProfScope ps(c, DR_PROF_SCAN, s); k_scan<<<1, 1024, 0, s>>>(c->st, gb); }
+    { ProfScope ps(c, DR_PROF_SCATTER, s); k_scatter<<<gb, kBlock, 0, s>>>(cp, c->st); }
   }
   CUDA_TRY(cudaGetLastError());
   return DR_OK;
@@ -324,7 +363,7 @@ dr_status dr_step(dr_chains* c, int32_t method, uint32_t iterations, void* strea
 dr_status dr_resolve_image(dr_chains* c, float* dev_rgb, void* stream) {
   if (!c || !dev_rgb) return fail(DR_ERR_INVALID_ARG, "null argument");
   cudaStream_t s = (cudaStream_t)stream;
-  k_resolve<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, s>>>(c->cp, c->st.ctr, c->accum, dev_rgb, c->npix);
+  { ProfScope ps(c, DR_PROF_RESOLVE, s); k_resolve<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, s>>>(c->cp, c->st.ctr, c->accum, dev_rgb, c->npix, 0ull, 0ull); }
   CUDA_TRY(cudaGetLastError());
   if (c->cp.restore) {
     unsigned long long tours = 0;
@@ -332,6 +371,55 @@ dr_status dr_resolve_image(dr_chains* c, float* dev_rgb, void* stream) {
     CUDA_TRY(cudaStreamSynchronize(s));
     if (tours == 0) { g_err = "no tour has completed yet: zero image"; return DR_WARN_NO_TOURS; }
   }
+  return DR_OK;
+}
+
+dr_status dr_resolve_image_sharded(dr_chains* c, const float* dev_accum_sum, uint64_t tours_total, uint64_t mutations_total,
+                                   float* dev_rgb, void* stream) {
+  if (!c || !dev_rgb || !dev_accum_sum) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (!mutations_total) return fail(DR_ERR_INVALID_ARG, "mutations_total must be > 0");
+  {
+    ProfScope ps(c, DR_PROF_RESOLVE, (cudaStream_t)stream);
+    k_resolve<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, (cudaStream_t)stream>>>(
+        c->cp, c->st.ctr, (const float4*)dev_accum_sum, dev_rgb, c->npix, (unsigned long long)tours_total,
+        (unsigned long long)mutations_total);
+  }
+  CUDA_TRY(cudaGetLastError());
+  if (c->cp.restore && tours_total == 0) { g_err = "no tour has completed yet: zero image"; return DR_WARN_NO_TOURS; }
+  return DR_OK;
+}
+
+dr_status dr_profile_enable(dr_chains* c, int32_t on, void* stream) {
+  if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
+  CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+  prof_drain(c);
+  for (int k = 0; k < DR_PROF_COUNT; ++k) { c->prof_ms[k] = 0; c->prof_launches[k] = 0; }
+  c->profiling = on != 0;
+  return DR_OK;
+}
+
+dr_status dr_profile_read(dr_chains* c, double* host_ms, uint64_t* host_launches, void* stream) {
+  if (!c || !host_ms || !host_launches) return fail(DR_ERR_INVALID_ARG, "null argument");
+  CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+  prof_drain(c);
+  for (int k = 0; k < DR_PROF_COUNT; ++k) { host_ms[k] = c->prof_ms[k]; host_launches[k] = c->prof_launches[k]; }
+  return DR_OK;
+}
+
+dr_status dr_chains_work_stats(dr_chains* c, uint64_t* host_out3, void* stream) {
+  if (!c || !host_out3) return fail(DR_ERR_INVALID_ARG, "null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  unsigned long long* d = nullptr;
+  CUDA_TRY(cudaMalloc(&d, 24));
+  cudaError_t e = cudaMemsetAsync(d, 0, 24, s);
+  if (e == cudaSuccess) {
+    k_chain_stats<<<(c->cp.N + kEvalBlock - 1) / kEvalBlock, kEvalBlock, smem_bytes(c->scene), s>>>(c->scene->dev, c->cp, c->st, d);
+    e = cudaMemcpyAsync(host_out3, d, 24, cudaMemcpyDeviceToHost, s);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(d);
+  if (e != cudaSuccess) return fail(DR_ERR_CUDA, std::string("work stats: ") + cudaGetErrorString(e));
   return DR_OK;
 }
 
@@ -457,6 +545,16 @@ dr_status dr_eval_states(const dr_scene* sc, const float* x, uint32_t n, float* 
   const uint32_t g = (n + kEvalBlock - 1) / kEvalBlock;
   if (score) k_eval_states<true><<<g, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, x, n, f, p, pix, score, nrays, sig);
   else k_eval_states<false><<<g, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, x, n, f, p, pix, nullptr, nrays, sig);
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;
+}
+
+dr_status dr_eval_work_stats(const dr_scene* sc, const float* x, uint32_t n, uint64_t* dev_out3, void* stream) {
+  if (!sc) return fail(DR_ERR_INVALID_ARG, "null scene");
+  if (!n) return DR_OK;
+  if (!x || !dev_out3) return fail(DR_ERR_INVALID_ARG, "null argument");
+  k_eval_stats<<<(n + kEvalBlock - 1) / kEvalBlock, kEvalBlock, smem_bytes(sc), (cudaStream_t)stream>>>(
+      sc->dev, x, n, (unsigned long long*)dev_out3);
   CUDA_TRY(cudaGetLastError());
   return DR_OK;
 }

@@ -324,14 +324,16 @@ __global__ void __launch_bounds__(kBlock) k_scatter(ChainParams cp, ChainState s
   }
 }
 
-// a12: Alg. 3 with the pixel-count factor (Q2); plain MH: p_lambda / N_mut.
+// a12: Alg. 3 with the pixel-count factor (Q2); plain MH: p_lambda / N_mut.  ext_* != 0: use externally
+// reduced totals (sharded runs) instead of this shard's counters.
 __global__ void __launch_bounds__(kBlock) k_resolve(ChainParams cp, const Counters* c, const float4* accum, float* rgb,
-                                                    uint32_t npix) {
+                                                    uint32_t npix, unsigned long long ext_tours, unsigned long long ext_mut) {
   const uint32_t q = blockIdx.x * kBlock + threadIdx.x;
   if (q >= npix) return;
+  const unsigned long long tours = ext_mut ? ext_tours : c->tours, mut = ext_mut ? ext_mut : c->mutations;
   float scale;
-  if (cp.restore) scale = c->tours ? (float)npix * c->kappa0 / (float)c->tours : 0.f;
-  else scale = c->mutations ? (float)npix * c->p_lambda / (float)c->mutations : 0.f;
+  if (cp.restore) scale = tours ? (float)npix * c->kappa0 / (float)tours : 0.f;
+  else scale = mut ? (float)npix * c->p_lambda / (float)mut : 0.f;
   const float4 a = accum[q];
   rgb[3 * q] = scale * a.x; rgb[3 * q + 1] = scale * a.y; rgb[3 * q + 2] = scale * a.z;
 }
@@ -365,6 +367,47 @@ __global__ void __launch_bounds__(kEvalBlock) k_eval_states(DevScene sc, const f
   else eval_path<GRAD>(sc, snodes, xv, e, gv);
   f[3 * i] = e.f[0]; f[3 * i + 1] = e.f[1]; f[3 * i + 2] = e.f[2];
   p[i] = e.p; pix[i] = e.pix; nrays[i] = e.nrays; sig[i] = e.sig;
+}
+
+// Work statistics of the evaluation of n states: totals of rays, BVH8 node visits and triangle tests
+// (the algorithmic work the roofline of bench.py is computed from).  out[0..2] += totals.
+__global__ void __launch_bounds__(kEvalBlock) k_eval_stats(DevScene sc, const float* x, uint32_t n, unsigned long long* out) {
+  extern __shared__ float4 snodes[];
+  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 16u; k += kEvalBlock) snodes[k] = sc.nodes[k];
+  __syncthreads();
+  const uint32_t i = blockIdx.x * kEvalBlock + threadIdx.x;
+  uint32_t nr = 0, nn = 0, nt = 0;
+  if (i < n && !sc.analytic) {
+    XView xv{nullptr, x + (size_t)i * sc.d, 0, 0};
+    GView gv{nullptr, nullptr, 0, 0};
+    EvalOut e;
+    eval_path<false, true>(sc, snodes, xv, e, gv, &nn, &nt);
+    nr = e.nrays;
+  }
+  nr = __reduce_add_sync(0xFFFFFFFFu, nr); nn = __reduce_add_sync(0xFFFFFFFFu, nn); nt = __reduce_add_sync(0xFFFFFFFFu, nt);
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&out[0], (unsigned long long)nr); atomicAdd(&out[1], (unsigned long long)nn); atomicAdd(&out[2], (unsigned long long)nt);
+  }
+}
+
+// Same statistics for the chains' last proposals (the states the last k_eval launch evaluated).
+__global__ void __launch_bounds__(kEvalBlock) k_chain_stats(DevScene sc, ChainParams cp, ChainState st, unsigned long long* out) {
+  extern __shared__ float4 snodes[];
+  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 16u; k += kEvalBlock) snodes[k] = sc.nodes[k];
+  __syncthreads();
+  const uint32_t i = blockIdx.x * kEvalBlock + threadIdx.x;
+  uint32_t nr = 0, nn = 0, nt = 0;
+  if (i < cp.N && !sc.analytic) {
+    XView xv{st.y, nullptr, cp.N, i};
+    GView gv{nullptr, nullptr, 0, 0};
+    EvalOut e;
+    eval_path<false, true>(sc, snodes, xv, e, gv, &nn, &nt);
+    nr = e.nrays;
+  }
+  nr = __reduce_add_sync(0xFFFFFFFFu, nr); nn = __reduce_add_sync(0xFFFFFFFFu, nn); nt = __reduce_add_sync(0xFFFFFFFFu, nt);
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&out[0], (unsigned long long)nr); atomicAdd(&out[1], (unsigned long long)nn); atomicAdd(&out[2], (unsigned long long)nt);
+  }
 }
 
 __global__ void k_philox_blocks(uint64_t seed, const uint32_t* ctr, uint32_t n, uint32_t* out) {

@@ -112,7 +112,9 @@ __device__ __forceinline__ void test_tri(const float4* __restrict__ tris, uint32
 }
 
 // One lane = one ray.  snodes: the first sc.smem_nodes nodes staged in shared memory (may be null if 0).
-__device__ __forceinline__ HitRec closest_hit(const DevScene& sc, const float4* snodes, float3 o, float3 d) {
+template <bool STATS = false>
+__device__ __forceinline__ HitRec closest_hit(const DevScene& sc, const float4* snodes, float3 o, float3 d,
+                                              uint32_t* n_nodes = nullptr, uint32_t* n_tris = nullptr) {
   HitRec best{FLT_MAX, 0xFFFFFFFFu};
   uint32_t best_id = 0xFFFFFFFFu;
   // box tests use a direction with no zero component (finite reciprocals); triangle tests use d itself
@@ -128,6 +130,7 @@ __device__ __forceinline__ HitRec closest_hit(const DevScene& sc, const float4* 
   for (;;) {
     if (!(cur & kLeafBit)) {
       const float4* np = cur < sc.smem_nodes ? snodes + 16 * cur : sc.nodes + 16 * (size_t)cur;
+      if (STATS) ++*n_nodes;
       float tn[8];
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
@@ -166,6 +169,7 @@ __device__ __forceinline__ HitRec closest_hit(const DevScene& sc, const float4* 
     } else {
       const uint32_t first = cur & 0x07FFFFFFu, cnt = ((cur >> 27) & 0xFu) + 1u;
       for (uint32_t k = 0; k < cnt; ++k) test_tri(sc.tris, first + k, o, d, best, best_id);
+      if (STATS) *n_tris += cnt;
     }
     // pop the next entry that can still contain a closer (or tying) hit
     bool found = false;
@@ -358,8 +362,9 @@ __device__ void eval_analytic(const DevScene& sc, const XView& xv, EvalOut& out,
 }
 
 // Path evaluation.  GRAD: also the score, written through gv for all L vertex slots.
-template <bool GRAD>
-__device__ void eval_path(const DevScene& sc, const float4* snodes, const XView& xv, EvalOut& out, const GView& gv) {
+template <bool GRAD, bool STATS = false>
+__device__ void eval_path(const DevScene& sc, const float4* snodes, const XView& xv, EvalOut& out, const GView& gv,
+                          uint32_t* n_nodes = nullptr, uint32_t* n_tris = nullptr) {
   const uint32_t L = sc.L;
   // per-vertex record for the reverse pass (local memory; only touched when GRAD)
   float3 rec_d[GRAD ? kMaxPathLen : 1];
@@ -378,7 +383,7 @@ __device__ void eval_path(const DevScene& sc, const float4* snodes, const XView&
   float f0 = 0.f, f1 = 0.f, f2 = 0.f;
 
   for (uint32_t k = 1; k <= L; ++k) {
-    const HitRec h = closest_hit(sc, snodes, o, d);
+    const HitRec h = closest_hit<STATS>(sc, snodes, o, d, n_nodes, n_tris);
     ++out.nrays;
     if (h.li == 0xFFFFFFFFu) {
       sig = fnv(sig, 0u);
