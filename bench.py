@@ -21,8 +21,8 @@ import numpy as np  # noqa: E402
 METRIC = "chain mutations/s at 1024x576 (Diffusion Restore, transparent-machines scene)"
 UNIT = "mutations/s"
 # Algorithmic FLOPs of the path evaluation: one BVH8 node visit = 8 slab tests of
-# 6 FMA + 12 min/max = 192 FLOP; one Moeller-Trumbore test = 50 FLOP; shading one vertex = 150 FLOP.
-F_NODE, F_TRI, F_SHADE = 192.0, 50.0, 150.0
+# 6 FMA + 12 min/max = 192 FLOP; one Moeller-Trumbore test = 50 FLOP (k_trace does no shading).
+F_NODE, F_TRI = 192.0, 50.0
 # Algorithmic bytes per mutation of the state-streaming kernels (propose + decide + scan + scatter), d = 2L:
 # read x, score (2 * 4d) + write x, score (2 * 4d) + p, f/p_hat, pixel, flags read and written (2 * 21).
 def stream_bytes_per_mutation(d, grad):
@@ -198,7 +198,6 @@ def main():
     if world > 1:
         dist.barrier()
     st0 = chains.stats()
-    chains.profile_enable(True)
     per = [(ev(), ev()) for _ in range(args.steps)]
     torch.cuda.synchronize()
     t_wall0 = time.time()
@@ -215,11 +214,17 @@ def main():
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
-    prof = chains.profile_read()
-    chains.profile_enable(False)
     st1 = chains.stats()
     frame_ms = sorted(a.elapsed_time(b) for a, b in per)
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    # per-kernel device times: a second, untimed pass with an event pair around every launch
+    prof_frames = min(args.steps, 16)
+    chains.profile_enable(True)
+    for _ in range(prof_frames):
+        frame()
+    prof = chains.profile_read()
+    chains.profile_enable(False)
+    st2 = chains.stats()
     work = chains.work_stats()
 
     rays_local = st1["rays"] - st0["rays"]
@@ -265,16 +270,18 @@ def main():
     pk = peaks()
     nodes_per_ray = work["node_visits"] / max(work["rays"], 1)
     tris_per_ray = work["tri_tests"] / max(work["rays"], 1)
-    flop_per_ray = F_NODE * nodes_per_ray + F_TRI * tris_per_ray + F_SHADE
-    eval_ms = prof["eval"]["ms"] / max(prof["eval"]["launches"], 1)
-    rays_per_launch = rays_local / max(prof["eval"]["launches"], 1)
+    flop_per_ray = F_NODE * nodes_per_ray + F_TRI * tris_per_ray
+    trace_launches = max(prof["trace"]["launches"], 1)
+    trace_ms = prof["trace"]["ms"] / trace_launches
+    rays_per_launch = (st2["rays"] - st1["rays"]) / trace_launches
     alu_peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
-    achieved = flop_per_ray * rays_per_launch / (eval_ms * 1e-3) / 1e12
+    achieved = flop_per_ray * rays_per_launch / (trace_ms * 1e-3) / 1e12
     grad = args.method in ("mala", "mala_restore", "diffusion_restore")
-    stream_ms = sum(prof[k]["ms"] for k in ("propose", "decide", "scan", "scatter")) / args.steps
+    stream_ms = sum(prof[k]["ms"] for k in ("propose", "decide", "scan", "scatter")) / prof_frames
     stream_gbs = stream_bytes_per_mutation(desc.dim, grad) * n_local / (stream_ms * 1e-3) / 1e9
+    launches_per_frame = sum(v["launches"] for v in prof.values()) / prof_frames
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "r01_eval_traffic.json")
+    tp = os.path.join(ROOT, "profiles", "trace_traffic.json")
     if os.path.exists(tp):
         traffic = json.load(open(tp)).get("dram_bytes_per_launch")
     out = {
@@ -292,13 +299,15 @@ def main():
         "workload_stats": {"rays_per_mutation": rays_local / (n_local * args.steps), "nodes_per_ray": nodes_per_ray,
                            "tris_per_ray": tris_per_ray, "kill_fraction_last": st1["kills_last_step"] / n_local,
                            "tours": st1["tours"], "p_lambda": st1["p_lambda"], "nonfinite": st1["nonfinite"]},
-        "kernels_ms_per_frame": {k: v["ms"] / args.steps for k, v in prof.items()},
-        "gpu_launches": int(sum(v["launches"] for v in prof.values())),
+        "kernels_ms_per_frame": {k: v["ms"] / prof_frames for k, v in prof.items()},
+        "kernel_launches_per_frame": launches_per_frame,
+        "gpu_launches": int(round(launches_per_frame * args.steps)),
         "clocks": clocks,
-        "roofline": {"kernel": "k_eval<GRAD>" if grad else "k_eval", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+        "roofline": {"kernel": "k_trace", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                      "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": traffic,
                      "peak_source": f"148 SM x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
-                     "flop_per_ray": flop_per_ray, "rays_per_launch": rays_per_launch, "launch_ms": eval_ms},
+                     "flop_per_ray": flop_per_ray, "rays_per_launch": rays_per_launch, "launch_ms": trace_ms,
+                     "grays_per_s_in_kernel": rays_per_launch / (trace_ms * 1e-3) / 1e9},
         "roofline_streaming": {"kernels": "k_propose+k_decide+k_scan+k_scatter", "bound": "hbm", "achieved": stream_gbs,
                                "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": stream_gbs / pk["hbm_gbs"],
                                "bytes_per_mutation": stream_bytes_per_mutation(desc.dim, grad), "ms_per_frame": stream_ms,

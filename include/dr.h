@@ -159,8 +159,8 @@ dr_status dr_resolve_image_sharded(dr_chains* chains, const float* dev_accum_sum
  * the totals; while on, every kernel launch of dr_chains_init / dr_step / dr_resolve_image* is bracketed by two
  * events.  dr_profile_read synchronises the stream and returns, per kernel class, the summed device time in ms and
  * the number of launches (arrays of DR_PROF_COUNT entries). */
-enum { DR_PROF_PROPOSE = 0, DR_PROF_EVAL = 1, DR_PROF_DECIDE = 2, DR_PROF_SCAN = 3, DR_PROF_SCATTER = 4,
-       DR_PROF_RESOLVE = 5, DR_PROF_COUNT = 6 };
+enum { DR_PROF_PROPOSE = 0, DR_PROF_RAYGEN = 1, DR_PROF_TRACE = 2, DR_PROF_SHADE = 3, DR_PROF_GRAD = 4, DR_PROF_DECIDE = 5,
+       DR_PROF_SCAN = 6, DR_PROF_SCATTER = 7, DR_PROF_RESOLVE = 8, DR_PROF_COUNT = 9 };
 dr_status dr_profile_enable(dr_chains* chains, int32_t on, void* stream);
 dr_status dr_profile_read(dr_chains* chains, double* host_ms, uint64_t* host_launches, void* stream);
 /* Work of the last evaluation launch: host_out3 = {rays, BVH8 node visits, triangle tests} of the chains' last

@@ -26,7 +26,7 @@ EXPORTS = [
     "dr_trace_rays", "dr_eval_states", "dr_philox_blocks", "dr_rng_transforms", "dr_resolve_image_sharded",
     "dr_eval_work_stats", "dr_profile_enable", "dr_profile_read", "dr_chains_work_stats",
 ]
-PROF_NAMES = ["propose", "eval", "decide", "scan", "scatter", "resolve"]
+PROF_NAMES = ["propose", "raygen", "trace", "shade", "grad", "decide", "scan", "scatter", "resolve"]
 
 
 class dr_material(C.Structure):

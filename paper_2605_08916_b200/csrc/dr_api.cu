@@ -26,6 +26,8 @@ dr_status fail(dr_status s, const std::string& msg) { g_err = msg; return s; }
 
 size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
+constexpr size_t kMaxDynSmem = 227 * 1024;  // opt-in shared memory per block on sm_100
+
 bool finite3(const float* v) { return std::isfinite(v[0]) && std::isfinite(v[1]) && std::isfinite(v[2]); }
 
 void normalize(float* v) {
@@ -46,6 +48,8 @@ struct dr_scene {
   void* d_tris = nullptr;
   void* d_mats = nullptr;
   dr_scene_info info{};
+  int n_sm = 1;            // persistent k_trace grid: one block per SM
+  size_t trace_smem = 0;   // staged top-level nodes + per-thread traversal stacks
 };
 
 struct dr_chains {
@@ -64,18 +68,21 @@ struct dr_chains {
   std::vector<cudaEvent_t> ev;     // pool
   std::vector<int> ev_kind;        // kernel class of pair k (events 2k, 2k+1)
   size_t ev_used = 0;              // pairs in use
-  double prof_ms[DR_PROF_COUNT] = {0, 0, 0, 0, 0, 0};
-  uint64_t prof_launches[DR_PROF_COUNT] = {0, 0, 0, 0, 0, 0};
+  double prof_ms[DR_PROF_COUNT] = {};
+  uint64_t prof_launches[DR_PROF_COUNT] = {};
+  EvalWs ws{};
   ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
 };
 
 namespace {
 
 struct Layout {
-  size_t x, g, fp, pix, sig, killed, y, gy, fy, pixy, sigy, kind, accepted, weight, order, blockcnt, blockoff, partial, ctr, total;
+  size_t x, g, fp, pix, sig, killed, y, gy, fy, pixy, sigy, kind, accepted, weight, order, blockcnt, blockoff, partial, ctr;
+  size_t qa, qb, hits, rec, pinfo, gradlist, ctl;   // evaluation workspace (dr_eval.cuh EvalWs)
+  size_t total;
 };
 
-Layout make_layout(uint32_t N, uint32_t planes, bool grad) {
+Layout make_layout(uint32_t N, uint32_t planes, uint32_t Lseg, bool grad) {
   Layout L{};
   size_t o = 0;
   auto take = [&](size_t bytes) { const size_t at = o; o = align256(o + bytes); return at; };
@@ -99,6 +106,13 @@ Layout make_layout(uint32_t N, uint32_t planes, bool grad) {
   L.blockoff = take(4 * nb);
   L.partial = take(8 * nb);
   L.ctr = take(sizeof(Counters));
+  L.qa = take(3 * sizeof(float4) * (size_t)N);
+  L.qb = take(3 * sizeof(float4) * (size_t)N);
+  L.hits = take(sizeof(uint2) * (size_t)N);
+  L.rec = take(grad ? sizeof(float4) * (size_t)N * Lseg : 0);
+  L.pinfo = take(grad ? 4 * (size_t)N : 0);
+  L.gradlist = take(grad ? 4 * (size_t)N : 0);
+  L.ctl = take(4 * kCtlWords);
   L.total = o;
   return L;
 }
@@ -116,8 +130,6 @@ dr_status check_config(const dr_config* c) {
   return DR_OK;
 }
 
-size_t smem_bytes(const dr_scene* s) { return (size_t)s->dev.smem_nodes * sizeof(Node8); }
-
 constexpr size_t kMaxPairs = 8192;
 
 // Folds finished event pairs into the per-class totals (requires the stream to be idle).
@@ -134,7 +146,7 @@ void prof_drain(dr_chains* c) {
 
 struct ProfScope {
   dr_chains* c; cudaStream_t s; size_t k; bool on;
-  ProfScope(dr_chains* c_, int kind, cudaStream_t s_) : c(c_), s(s_), k(0), on(c_->profiling) {
+  ProfScope(dr_chains* c_, int kind, cudaStream_t s_) : c(c_), s(s_), k(0), on(c_ && c_->profiling) {
     if (!on) return;
     if (c->ev_used == kMaxPairs) { cudaStreamSynchronize(s); prof_drain(c); }
     k = c->ev_used++;
@@ -146,18 +158,55 @@ struct ProfScope {
   ~ProfScope() { if (on) cudaEventRecord(c->ev[2 * k + 1], s); }
 };
 
-// evaluation of all proposals (+ the kernels that must precede / follow it)
+// Rows a3-a6 for n states (dr_eval.cuh): raygen, then trace + shade per segment, then the reverse pass.
+// prof may be null (test hooks).  io.g must be zero on entry when grad is set.
+dr_status launch_eval(dr_chains* prof, const dr_scene* sc, const EvalWs& ws, const EvalIO& io, uint32_t n, bool grad, bool stats,
+                      cudaStream_t s) {
+  const DevScene& dev = sc->dev;
+  const uint32_t g = (n + kShadeBlock - 1) / kShadeBlock;
+  if (dev.analytic) {
+    ProfScope ps(prof, DR_PROF_SHADE, s);
+    if (grad) k_eval_analytic<true><<<g, kShadeBlock, 0, s>>>(dev, io, n);
+    else k_eval_analytic<false><<<g, kShadeBlock, 0, s>>>(dev, io, n);
+    CUDA_TRY(cudaGetLastError());
+    return DR_OK;
+  }
+  CUDA_TRY(cudaMemsetAsync(ws.ctl, 0, 4 * kCtlWords, s));
+  { ProfScope ps(prof, DR_PROF_RAYGEN, s); k_raygen<<<g, kShadeBlock, 0, s>>>(dev, ws, io, n); }
+  for (uint32_t k = 1; k <= dev.L; ++k) {
+    const float4* q = (k & 1u) ? ws.qa : ws.qb;
+    {
+      ProfScope ps(prof, DR_PROF_TRACE, s);
+      if (stats) k_trace<true><<<sc->n_sm, kTraceBlock, sc->trace_smem, s>>>(dev, q, ws.cap, ws.ctl + kCtlCnt + k, ws.ctl + kCtlHead + k, ws.hits, io.work);
+      else k_trace<false><<<sc->n_sm, kTraceBlock, sc->trace_smem, s>>>(dev, q, ws.cap, ws.ctl + kCtlCnt + k, ws.ctl + kCtlHead + k, ws.hits, io.work);
+    }
+    {
+      ProfScope ps(prof, DR_PROF_SHADE, s);
+      if (grad) k_shade<true><<<g, kShadeBlock, 0, s>>>(dev, ws, io, k);
+      else k_shade<false><<<g, kShadeBlock, 0, s>>>(dev, ws, io, k);
+    }
+  }
+  if (grad) { ProfScope ps(prof, DR_PROF_GRAD, s); k_grad<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io); }
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;
+}
+
+EvalIO chain_io(const dr_chains* c, bool use_order) {
+  EvalIO io{};
+  io.x = c->st.y; io.stride = c->cp.N; io.order = use_order ? c->st.order : nullptr;
+  io.g = c->st.gy; io.f = c->st.fy; io.pix = c->st.pixy; io.sig = c->st.sigy; io.nrays = nullptr;
+  io.rays_ctr = &c->st.ctr->rays; io.nonfinite_ctr = &c->st.ctr->nonfinite; io.work = nullptr;
+  return io;
+}
+
+// one iteration of every chain: propose, evaluate the proposals, (bootstrap,) decide, compact
 dr_status launch_iteration(dr_chains* c, uint32_t n, bool init, cudaStream_t s) {
   const ChainParams& cp = c->cp;
-  const uint32_t gb = c->nblocks, ge = (cp.N + kEvalBlock - 1) / kEvalBlock;
+  const uint32_t gb = c->nblocks;
   { ProfScope ps(c, DR_PROF_PROPOSE, s); k_propose<<<gb, kBlock, 0, s>>>(cp, c->st, n, init ? 1 : 0); }
-  const int use_order = (!init && cp.restore) ? 1 : 0;
-  const size_t sm = smem_bytes(c->scene);
-  {
-    ProfScope ps(c, DR_PROF_EVAL, s);
-    if (cp.grad) k_eval<true><<<ge, kEvalBlock, sm, s>>>(c->scene->dev, cp, c->st, use_order);
-    else k_eval<false><<<ge, kEvalBlock, sm, s>>>(c->scene->dev, cp, c->st, use_order);
-  }
+  // evaluation order: alive chains first, then the regeneration queue (a9), once the queue exists
+  const dr_status es = launch_eval(c, c->scene, c->ws, chain_io(c, !init && cp.restore), cp.N, cp.grad != 0, false, s);
+  if (es != DR_OK) return es;
   if (init) {
     k_psum_partial<<<gb, kBlock, 0, s>>>(cp, c->st);
     k_bootstrap<<<1, kBlock, 0, s>>>(cp, c->st, gb);
@@ -170,6 +219,36 @@ dr_status launch_iteration(dr_chains* c, uint32_t n, bool init, cudaStream_t s) 
   CUDA_TRY(cudaGetLastError());
   return DR_OK;
 }
+
+// Device scratch of the test hooks (freed on scope exit).
+struct DevBuf {
+  void* p = nullptr;
+  cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 16); }
+  ~DevBuf() { cudaFree(p); }
+  template <class T> T* as() const { return (T*)p; }
+};
+
+// Workspace + plane buffers for evaluating n states outside a chain ensemble.
+struct HookEval {
+  DevBuf ws_mem, xpl, gpl, f4;
+  EvalWs ws{};
+  cudaError_t setup(const dr_scene* sc, uint32_t n, bool grad) {
+    const size_t N = n, L = sc->dev.L;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { const size_t at = o; o = align256(o + bytes); return at; };
+    const size_t qa = take(48 * N), qb = take(48 * N), hits = take(8 * N), rec = take(grad ? 16 * N * L : 0), pinfo = take(grad ? 4 * N : 0),
+                 gl = take(grad ? 4 * N : 0), ctl = take(4 * kCtlWords);
+    cudaError_t e = ws_mem.alloc(o);
+    if (e == cudaSuccess) e = xpl.alloc(16 * N * sc->dev.planes);
+    if (e == cudaSuccess) e = gpl.alloc(grad ? 16 * N * sc->dev.planes : 0);
+    if (e == cudaSuccess) e = f4.alloc(16 * N);
+    if (e != cudaSuccess) return e;
+    char* b = ws_mem.as<char>();
+    ws.qa = (float4*)(b + qa); ws.qb = (float4*)(b + qb); ws.hits = (uint2*)(b + hits); ws.rec = (float4*)(b + rec);
+    ws.pinfo = (uint32_t*)(b + pinfo); ws.gradlist = (uint32_t*)(b + gl); ws.ctl = (uint32_t*)(b + ctl); ws.cap = n;
+    return cudaSuccess;
+  }
+};
 
 }  // namespace
 
@@ -212,24 +291,39 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   }
   BuiltBvh bvh;
   build_bvh8(d->host_vertices, d->nv, d->host_indices, d->nt, d->host_tri_material, bvh);
+  if (bvh.depth > (uint32_t)kMaxBvhDepth) return fail(DR_ERR_UNSUPPORTED, "BVH8 deeper than the traversal stack allows");
 
   dr_scene* s = new dr_scene();
   DevScene& dev = s->dev;
-  const size_t nb = bvh.nodes.size() * sizeof(Node8), tb = bvh.tris.size() * sizeof(TriPacked), mb = mats.size() * sizeof(MatPacked);
+  const size_t nb = bvh.nodes.size() * sizeof(NodeC), tb = bvh.tris.size() * sizeof(TriPacked), mb = mats.size() * sizeof(MatPacked);
   cudaError_t e = cudaMalloc(&s->d_nodes, nb);
   if (e == cudaSuccess) e = cudaMalloc(&s->d_tris, tb);
   if (e == cudaSuccess) e = cudaMalloc(&s->d_mats, mb);
   if (e == cudaSuccess) e = cudaMemcpy(s->d_nodes, bvh.nodes.data(), nb, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(s->d_tris, bvh.tris.data(), tb, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(s->d_mats, mats.data(), mb, cudaMemcpyHostToDevice);
+  int device = 0;
+  if (e == cudaSuccess) e = cudaGetDevice(&device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&s->n_sm, cudaDevAttrMultiProcessorCount, device);
   if (e != cudaSuccess) {
     cudaFree(s->d_nodes); cudaFree(s->d_tris); cudaFree(s->d_mats);
     delete s;
     return fail(e == cudaErrorMemoryAllocation ? DR_ERR_OOM : DR_ERR_CUDA, std::string("scene upload: ") + cudaGetErrorString(e));
   }
-  dev.nodes = (const float4*)s->d_nodes; dev.tris = (const float4*)s->d_tris; dev.mats = (const float4*)s->d_mats;
+  dev.nodes = (const uint4*)s->d_nodes; dev.tris = (const float4*)s->d_tris; dev.mats = (const float4*)s->d_mats;
   dev.n_nodes = (uint32_t)bvh.nodes.size();
-  dev.smem_nodes = dev.n_nodes < (uint32_t)kSmemNodes ? dev.n_nodes : (uint32_t)kSmemNodes;
+  dev.smem_nodes = dev.n_nodes < (uint32_t)kMaxSmemNodes ? dev.n_nodes : (uint32_t)kMaxSmemNodes;
+  dev.stack_cap = bvh.depth + 1;  // node groups: at most one per level
+  const size_t stack_bytes = (size_t)(dev.stack_cap + kTriStack) * sizeof(uint2) * kTraceBlock;
+  if (stack_bytes + (size_t)dev.smem_nodes * sizeof(NodeC) > kMaxDynSmem)
+    dev.smem_nodes = (uint32_t)((kMaxDynSmem - stack_bytes) / sizeof(NodeC));
+  s->trace_smem = (size_t)dev.smem_nodes * sizeof(NodeC) + stack_bytes;
+  e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e != cudaSuccess) {
+    dr_scene_destroy(s);
+    return fail(DR_ERR_CUDA, std::string("k_trace shared memory: ") + cudaGetErrorString(e));
+  }
   dev.n_tris = d->nt; dev.n_mats = d->nm;
   for (int c = 0; c < 3; ++c) { dev.env[c] = d->env_radiance[c]; dev.cam_pos[c] = d->cam_pos[c]; }
   // pinhole basis: w = normalize(look - pos), r = normalize(w x up), v = r x w
@@ -293,7 +387,7 @@ dr_status dr_scene_get_info(const dr_scene* s, dr_scene_info* o) {
 size_t dr_chains_state_bytes(const dr_scene* s, const dr_config* c) {
   if (!s || check_config(c) != DR_OK) return 0;
   const bool grad = c->method == DR_MALA || c->method == DR_MALA_RESTORE || c->method == DR_DIFFUSION_RESTORE;
-  return make_layout(c->n_chains, s->dev.planes, grad).total;
+  return make_layout(c->n_chains, s->dev.planes, s->dev.L, grad).total;
 }
 
 dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_state, size_t bytes, float* dev_accum, dr_chains** out) {
@@ -303,7 +397,7 @@ dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_stat
   if (cs != DR_OK) return cs;
   if (((uintptr_t)dev_state & 255u) || ((uintptr_t)dev_accum & 15u)) return fail(DR_ERR_INVALID_ARG, "dev_state must be 256-byte and dev_accum 16-byte aligned");
   const bool grad = c->method == DR_MALA || c->method == DR_MALA_RESTORE || c->method == DR_DIFFUSION_RESTORE;
-  const Layout L = make_layout(c->n_chains, s->dev.planes, grad);
+  const Layout L = make_layout(c->n_chains, s->dev.planes, s->dev.L, grad);
   if (bytes < L.total) return fail(DR_ERR_INVALID_ARG, "state buffer smaller than dr_chains_state_bytes");
   dr_chains* h = new dr_chains();
   h->scene = s; h->cfg = *c;
@@ -325,11 +419,9 @@ dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_stat
   h->npix = s->dev.W * s->dev.H;
   h->nblocks = (cp.N + kBlock - 1) / kBlock;
   h->state_bytes = L.total; h->state_base = dev_state;
-  const size_t sm = smem_bytes(s);
-  if (sm > 48 * 1024) {
-    CUDA_TRY(cudaFuncSetAttribute(k_eval<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    CUDA_TRY(cudaFuncSetAttribute(k_eval<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-  }
+  EvalWs& ws = h->ws;
+  ws.qa = (float4*)(b + L.qa); ws.qb = (float4*)(b + L.qb); ws.hits = (uint2*)(b + L.hits); ws.rec = (float4*)(b + L.rec);
+  ws.pinfo = (uint32_t*)(b + L.pinfo); ws.gradlist = (uint32_t*)(b + L.gradlist); ws.ctl = (uint32_t*)(b + L.ctl); ws.cap = cp.N;
   *out = h;
   return DR_OK;
 }
@@ -408,18 +500,19 @@ dr_status dr_profile_read(dr_chains* c, double* host_ms, uint64_t* host_launches
 
 dr_status dr_chains_work_stats(dr_chains* c, uint64_t* host_out3, void* stream) {
   if (!c || !host_out3) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (!c->initialised) return fail(DR_ERR_INVALID_ARG, "dr_chains_init has not been called");
   cudaStream_t s = (cudaStream_t)stream;
-  unsigned long long* d = nullptr;
-  CUDA_TRY(cudaMalloc(&d, 24));
-  cudaError_t e = cudaMemsetAsync(d, 0, 24, s);
-  if (e == cudaSuccess) {
-    k_chain_stats<<<(c->cp.N + kEvalBlock - 1) / kEvalBlock, kEvalBlock, smem_bytes(c->scene), s>>>(c->scene->dev, c->cp, c->st, d);
-    e = cudaMemcpyAsync(host_out3, d, 24, cudaMemcpyDeviceToHost, s);
-  }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  if (e == cudaSuccess) e = cudaGetLastError();
-  cudaFree(d);
-  if (e != cudaSuccess) return fail(DR_ERR_CUDA, std::string("work stats: ") + cudaGetErrorString(e));
+  DevBuf d;
+  CUDA_TRY(d.alloc(24));
+  CUDA_TRY(cudaMemsetAsync(d.p, 0, 24, s));
+  // re-evaluates the last proposals (same values are written again) with the counting variant of k_trace
+  EvalIO io = chain_io(c, false);
+  io.rays_ctr = d.as<unsigned long long>(); io.nonfinite_ctr = nullptr; io.work = d.as<unsigned long long>() + 1;
+  if (c->cp.grad) CUDA_TRY(cudaMemsetAsync(c->st.gy, 0, sizeof(float4) * (size_t)c->cp.planes * c->cp.N, s));
+  const dr_status r = launch_eval(nullptr, c->scene, c->ws, io, c->cp.N, c->cp.grad != 0, true, s);
+  if (r != DR_OK) return r;
+  CUDA_TRY(cudaMemcpyAsync(host_out3, d.p, 24, cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(cudaStreamSynchronize(s));
   return DR_OK;
 }
 
@@ -530,33 +623,63 @@ dr_status dr_trace_rays(const dr_scene* sc, const float* o, const float* d, uint
   if (sc->dev.analytic) return fail(DR_ERR_UNSUPPORTED, "analytic scene has no geometry");
   if (!n) return DR_OK;  // empty input: nothing to do, pointers may be null
   if (!o || !d || !t || !prim) return fail(DR_ERR_INVALID_ARG, "null argument");
-  const size_t sm = smem_bytes(sc);
-  k_trace<<<(n + kEvalBlock - 1) / kEvalBlock, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, o, d, n, t, prim);
+  cudaStream_t s = (cudaStream_t)stream;
+  DevBuf q, hits, ctl;
+  CUDA_TRY(q.alloc(32 * (size_t)n));
+  CUDA_TRY(hits.alloc(8 * (size_t)n));
+  CUDA_TRY(ctl.alloc(8));
+  CUDA_TRY(cudaMemsetAsync(ctl.p, 0, 8, s));
+  const uint32_t g = (n + 255) / 256;
+  k_pack_rays<<<g, 256, 0, s>>>(o, d, n, q.as<float4>(), n, ctl.as<uint32_t>());
+  k_trace<false><<<sc->n_sm, kTraceBlock, sc->trace_smem, s>>>(sc->dev, q.as<float4>(), n, ctl.as<uint32_t>(), ctl.as<uint32_t>() + 1,
+                                                               hits.as<uint2>(), nullptr);
+  k_unpack_hits<<<g, 256, 0, s>>>(sc->dev, hits.as<uint2>(), n, t, prim);
   CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaStreamSynchronize(s));  // the scratch buffers are freed on return
   return DR_OK;
 }
+
+namespace {
+// Evaluates n row-major states through the wavefront path.  Any output may be null.  work3: {rays, nodes, tris} counters.
+dr_status eval_rows(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score, uint32_t* nrays,
+                    uint32_t* sig, unsigned long long* work3, cudaStream_t s) {
+  const bool grad = score != nullptr;
+  const uint32_t d = sc->dev.d, planes = sc->dev.planes, g = (n + 255) / 256;
+  HookEval he;
+  DevBuf tpix, tsig;
+  CUDA_TRY(he.setup(sc, n, grad));
+  CUDA_TRY(tpix.alloc(4 * (size_t)n));
+  CUDA_TRY(tsig.alloc(4 * (size_t)n));
+  k_rows_to_planes<<<g, 256, 0, s>>>(x, he.xpl.as<float4>(), n, d, planes);
+  if (grad) CUDA_TRY(cudaMemsetAsync(he.gpl.p, 0, 16 * (size_t)n * planes, s));
+  EvalIO io{};
+  io.x = he.xpl.as<float4>(); io.stride = n; io.order = nullptr; io.g = he.gpl.as<float4>(); io.f = he.f4.as<float4>();
+  io.pix = pix ? pix : tpix.as<uint32_t>(); io.sig = sig ? sig : tsig.as<uint32_t>(); io.nrays = nrays;
+  io.rays_ctr = work3; io.nonfinite_ctr = nullptr; io.work = work3 ? work3 + 1 : nullptr;
+  const dr_status r = launch_eval(nullptr, sc, he.ws, io, n, grad, work3 != nullptr, s);
+  if (r != DR_OK) return r;
+  if (f || p) k_fp_split<<<g, 256, 0, s>>>(he.f4.as<float4>(), p, f, n);
+  if (grad) k_planes_to_rows<<<g, 256, 0, s>>>(he.gpl.as<float4>(), score, n, d, planes);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaStreamSynchronize(s));  // the scratch buffers are freed on return
+  return DR_OK;
+}
+}  // namespace
 
 dr_status dr_eval_states(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score,
                          uint32_t* nrays, uint32_t* sig, void* stream) {
   if (!sc) return fail(DR_ERR_INVALID_ARG, "null scene");
   if (!n) return DR_OK;  // empty input
   if (!x || !f || !p || !pix || !nrays || !sig) return fail(DR_ERR_INVALID_ARG, "null argument");
-  const size_t sm = smem_bytes(sc);
-  const uint32_t g = (n + kEvalBlock - 1) / kEvalBlock;
-  if (score) k_eval_states<true><<<g, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, x, n, f, p, pix, score, nrays, sig);
-  else k_eval_states<false><<<g, kEvalBlock, sm, (cudaStream_t)stream>>>(sc->dev, x, n, f, p, pix, nullptr, nrays, sig);
-  CUDA_TRY(cudaGetLastError());
-  return DR_OK;
+  return eval_rows(sc, x, n, f, p, pix, score, nrays, sig, nullptr, (cudaStream_t)stream);
 }
 
 dr_status dr_eval_work_stats(const dr_scene* sc, const float* x, uint32_t n, uint64_t* dev_out3, void* stream) {
   if (!sc) return fail(DR_ERR_INVALID_ARG, "null scene");
   if (!n) return DR_OK;
   if (!x || !dev_out3) return fail(DR_ERR_INVALID_ARG, "null argument");
-  k_eval_stats<<<(n + kEvalBlock - 1) / kEvalBlock, kEvalBlock, smem_bytes(sc), (cudaStream_t)stream>>>(
-      sc->dev, x, n, (unsigned long long*)dev_out3);
-  CUDA_TRY(cudaGetLastError());
-  return DR_OK;
+  if (sc->dev.analytic) return DR_OK;
+  return eval_rows(sc, x, n, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, (unsigned long long*)dev_out3, (cudaStream_t)stream);
 }
 
 dr_status dr_philox_blocks(uint64_t seed, const uint32_t* ctr, uint32_t n, uint32_t* out, void* stream) {

@@ -1,7 +1,9 @@
-// Host-side acceleration-structure build: binned-SAH BVH2, collapsed to a BVH8 and emitted breadth-first
-// so that the top levels are contiguous (they are staged in shared memory by the traversal kernel).
+// Host-side acceleration-structure build: binned-SAH BVH2, collapsed to a BVH8, children placed in octant
+// slots, child boxes quantised to 8 bits per plane (80-byte nodes, dr_types.h), emitted breadth-first so that
+// the top levels are contiguous (the traversal kernel stages them in shared memory).
 // The paper uses a hardware ray-tracing pipeline; B200 has no RT cores, so the closest-hit
-// query of row a4 runs in software over this structure.
+// query of row a4 runs in software over this structure.  The compressed wide node with octant-ordered
+// traversal follows the published idea of Ylitie, Karras and Laine (HPG 2017), restated here from scratch.
 #include <algorithm>
 #include <cfloat>
 #include <cmath>
@@ -29,10 +31,7 @@ struct Node2 {
   uint32_t first = 0, count = 0;  // leaf range into `order`
 };
 
-// Empty child slots hold a far-away point box: the min/max slab test can never report a hit for it.
-constexpr float kFar = 1e30f;
-constexpr int kBins = 16;
-constexpr uint32_t kLeafMax = 4;
+constexpr int kBins = 32;
 
 struct Builder {
   const std::vector<Box>& tb;
@@ -57,7 +56,7 @@ struct Builder {
     nodes[me].box = box;
     nodes[me].first = first;
     nodes[me].count = count;
-    if (count <= kLeafMax) return me;
+    if (count <= (uint32_t)kMaxLeafTris) return me;
     // binned SAH over the three axes
     float best_cost = FLT_MAX;
     int best_axis = -1, best_bin = -1;
@@ -107,6 +106,34 @@ struct Builder {
   }
 };
 
+// Places up to eight children in the octant slots: child c goes to the free slot s that maximises
+// dot(centre(c) - centre(node), corner(s)), greedily over all (child, slot) pairs.
+void assign_slots(const std::vector<Node2>& n2, const uint32_t* kids, int nk, int* slot_of) {
+  Box nb;
+  for (int i = 0; i < nk; ++i) nb.grow(n2[kids[i]].box);
+  float score[8][8];
+  for (int i = 0; i < nk; ++i) {
+    const Box& b = n2[kids[i]].box;
+    float off[3];
+    for (int a = 0; a < 3; ++a) off[a] = 0.5f * (b.lo[a] + b.hi[a]) - 0.5f * (nb.lo[a] + nb.hi[a]);
+    for (int s = 0; s < 8; ++s)
+      score[i][s] = ((s & 4) ? off[0] : -off[0]) + ((s & 2) ? off[1] : -off[1]) + ((s & 1) ? off[2] : -off[2]);
+  }
+  bool child_done[8] = {false}, slot_used[8] = {false};
+  for (int round = 0; round < nk; ++round) {
+    int bi = -1, bs = -1;
+    float best = -FLT_MAX;
+    for (int i = 0; i < nk; ++i) {
+      if (child_done[i]) continue;
+      for (int s = 0; s < 8; ++s)
+        if (!slot_used[s] && score[i][s] > best) { best = score[i][s]; bi = i; bs = s; }
+    }
+    child_done[bi] = true;
+    slot_used[bs] = true;
+    slot_of[bi] = bs;
+  }
+}
+
 }  // namespace
 
 void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t nt, const uint32_t* tri_mat, BuiltBvh& out) {
@@ -121,40 +148,41 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
   }
   const float dx = scene.hi[0] - scene.lo[0], dy = scene.hi[1] - scene.lo[1], dz = scene.hi[2] - scene.lo[2];
   out.diag = nt ? std::sqrt(dx * dx + dy * dy + dz * dz) : 0.f;
-  // Child boxes are inflated so that fp32 slab tests can never cull a triangle the exact test accepts:
-  // slab rounding moves an entry/exit point by < 2e-7 * diag, the inflation is 20 times that.
+  // Child boxes are inflated before quantisation so that fp32 slab tests can never cull a triangle the exact
+  // test accepts: slab rounding moves an entry/exit point by < 2e-7 * diag, the inflation is 20 times that.
+  // Quantisation then only rounds outwards.
   const float pad = 4e-6f * out.diag;
   out.nodes.clear();
   out.tris.clear();
   out.depth = 0;
   out.sah_cost = 0.f;
   if (!nt) {
-    Node8 root;
+    NodeC root;
     std::memset(&root, 0, sizeof(root));
-    for (int i = 0; i < 8; ++i) {
-      root.child[i] = kEmptyChild;
-      for (int a = 0; a < 3; ++a) { root.lo[a][i] = kFar; root.hi[a][i] = kFar; }
+    for (int a = 0; a < 3; ++a) {
+      root.e[a] = 127;
+      for (int s = 0; s < 8; ++s) { root.qlo[a][s] = 255; root.qhi[a][s] = 0; }
     }
     out.nodes.push_back(root);
+    out.depth = 1;
     return;
   }
   Builder b(tb, cen);
   b.build(0, nt);
   const std::vector<Node2>& n2 = b.nodes;
 
-  // leaf-order triangle array
-  out.tris.resize(nt);
-  for (uint32_t k = 0; k < nt; ++k) {
-    const uint32_t id = b.order[k];
+  auto emit_tri = [&](uint32_t id) {
     const float* a = &verts[3 * idx[3 * id]];
     const float* bb = &verts[3 * idx[3 * id + 1]];
     const float* c = &verts[3 * idx[3 * id + 2]];
-    TriPacked& tp = out.tris[k];
+    TriPacked tp;
     for (int x = 0; x < 3; ++x) { tp.v0[x] = a[x]; tp.e1[x] = bb[x] - a[x]; tp.e2[x] = c[x] - a[x]; }
     tp.id = id; tp.mat = tri_mat[id]; tp.pad = 0;
-  }
+    out.tris.push_back(tp);
+  };
+  out.tris.reserve(nt);
 
-  // collapse to BVH8, breadth-first
+  // collapse to BVH8, breadth-first; a node's index is its position in the queue order
   struct Item { uint32_t n2; uint32_t depth; };
   std::queue<Item> q;
   q.push({0, 1});
@@ -167,7 +195,7 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
     out.depth = std::max(out.depth, it.depth);
     uint32_t kids[8];
     int nk = 0;
-    if (n2[it.n2].count) kids[nk++] = it.n2;  // root is itself a leaf
+    if (n2[it.n2].count) kids[nk++] = it.n2;  // the root is itself a leaf
     else { kids[nk++] = n2[it.n2].left; kids[nk++] = n2[it.n2].right; }
     for (;;) {  // open the internal child with the largest area until 8 children
       if (nk == 8) break;
@@ -180,22 +208,62 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
       kids[pick] = n2[p].left;
       kids[nk++] = n2[p].right;
     }
-    Node8 node;
+    int slot_of[8];
+    assign_slots(n2, kids, nk, slot_of);
+    int kid_in_slot[8];
+    for (int s = 0; s < 8; ++s) kid_in_slot[s] = -1;
+    for (int i = 0; i < nk; ++i) kid_in_slot[slot_of[i]] = i;
+
+    NodeC node;
     std::memset(&node, 0, sizeof(node));
-    for (int i = 0; i < 8; ++i) {
-      if (i >= nk) {
-        node.child[i] = kEmptyChild;
-        for (int a = 0; a < 3; ++a) { node.lo[a][i] = kFar; node.hi[a][i] = kFar; }
-        continue;
+    node.child_base = next_index;
+    node.tri_base = (uint32_t)out.tris.size();
+    // padded child boxes and the node grid
+    Box cb[8], nb;
+    for (int s = 0; s < 8; ++s) {
+      if (kid_in_slot[s] < 0) continue;
+      const Node2& c = n2[kids[kid_in_slot[s]]];
+      for (int a = 0; a < 3; ++a) { cb[s].lo[a] = c.box.lo[a] - pad; cb[s].hi[a] = c.box.hi[a] + pad; }
+      nb.grow(cb[s]);
+    }
+    for (int a = 0; a < 3; ++a) {
+      node.p[a] = nb.lo[a];
+      const double p = (double)nb.lo[a], ext = (double)nb.hi[a] - p;
+      int e = ext > 0.0 ? (int)std::ceil(std::log2(ext / 255.0)) : -120;
+      e = std::max(e, -120);
+      for (;;) {
+        const double cell = std::ldexp(1.0, e);
+        bool ok = true;
+        for (int s = 0; s < 8 && ok; ++s) {
+          if (kid_in_slot[s] < 0) { node.qlo[a][s] = 255; node.qhi[a][s] = 0; continue; }  // inverted: never hit
+          // outward rounding with 0.01 cell of slack for the kernel's plane arithmetic (dr_traverse.cuh node_hits)
+          double ql = std::floor(((double)cb[s].lo[a] - p) / cell - 0.01);
+          while (ql > 0.0 && p + (ql + 0.01) * cell > (double)cb[s].lo[a]) ql -= 1.0;
+          double qh = std::ceil(((double)cb[s].hi[a] - p) / cell + 0.01);
+          while (p + (qh - 0.01) * cell < (double)cb[s].hi[a]) qh += 1.0;
+          if (ql < 0.0) ql = 0.0;
+          if (qh > 255.0) { ok = false; break; }
+          node.qlo[a][s] = (uint8_t)ql;
+          node.qhi[a][s] = (uint8_t)qh;
+        }
+        if (ok) break;
+        ++e;
       }
-      const Node2& c = n2[kids[i]];
-      for (int a = 0; a < 3; ++a) { node.lo[a][i] = c.box.lo[a] - pad; node.hi[a][i] = c.box.hi[a] + pad; }
+      node.e[a] = (uint8_t)(e + 127);
+    }
+    for (int s = 0; s < 8; ++s) {
+      if (kid_in_slot[s] < 0) continue;
+      const Node2& c = n2[kids[kid_in_slot[s]]];
       if (c.count) {
-        node.child[i] = kLeafBit | ((c.count - 1) << 27) | c.first;
+        const uint32_t off = (uint32_t)out.tris.size() - node.tri_base;
+        node.meta[s] = (uint8_t)((((1u << c.count) - 1u) << 5) | off);
+        for (uint32_t k = 0; k < c.count; ++k) emit_tri(b.order[c.first + k]);
         sah += (double)c.box.area() / root_area * c.count;
       } else {
-        node.child[i] = next_index++;
-        q.push({kids[i], it.depth + 1});
+        node.meta[s] = (uint8_t)((1u << 5) | (24u + (uint32_t)s));
+        node.imask |= (uint8_t)(1u << s);
+        ++next_index;
+        q.push({kids[kid_in_slot[s]], it.depth + 1});
         sah += (double)c.box.area() / root_area;
       }
     }

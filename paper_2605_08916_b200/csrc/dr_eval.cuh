@@ -1,0 +1,431 @@
+// Wavefront evaluation of the target for a batch of PSS states (rows a3-a6): x -> (f, p, pixel, score).
+//   k_raygen            a3: camera ray of every state -> ray queue
+//   per segment k = 1..L:
+//     k_trace           a4: persistent closest-hit kernel; a warp refills its idle lanes from the ray queue
+//     k_shade           a3/a5: emission / termination, direction sampling at vertex k, throughput; surviving paths
+//                       are compacted into the next queue (ballot + block-level prefix sum, one atomic per block)
+//   k_grad              a6: reverse pass over the recorded vertices, only for the states that need it
+// One thread = one ray / path vertex; nothing here is a dense contraction (no tensor cores).  The paper runs one
+// shader thread per chain through a hardware ray-tracing pipeline; splitting the path into
+// per-segment waves is what keeps 32-wide warps busy without RT cores (profiles/r01a: the one-thread-one-path
+// kernel ran with 4.5 of 32 lanes active).
+#pragma once
+#include "dr_path.cuh"
+#include "dr_traverse.cuh"
+
+namespace dr {
+
+constexpr int kTraceBlock = 640;   // one persistent block per SM
+constexpr int kTriStack = 12;      // postponed triangle groups per ray
+constexpr int kTrisPerStep = 2;    // triangle tests per lockstep step
+constexpr int kShadeBlock = 256;
+constexpr int kGradBlock = 128;
+constexpr uint32_t kFetchChunk = 64;   // rays a warp takes from the queue per atomic
+constexpr int kRefillBelow = 30;       // a warp goes back to the queue when fewer lanes than this hold a ray
+constexpr uint32_t kSigInit = 2166136261u;
+constexpr uint32_t kMiss = 0xFFFFFFFFu;
+
+// control words of one evaluation (zeroed before k_raygen)
+constexpr int kCtlCnt = 0;     // cnt[k], k = 1..L: rays of segment k
+constexpr int kCtlHead = 20;   // head[k]: fetch counter of k_trace for segment k
+constexpr int kCtlGrad = 40;   // states on the reverse-pass list
+constexpr int kCtlWords = 64;
+
+// Workspace for up to `cap` states.  A ray-queue entry is three float4 (planes of `cap` entries):
+//   Q0 = (o.xyz, bits(state)), Q1 = (d.xyz, bits(path signature)), Q2 = (T.rgb, bits(refract mask | has_ggx << 16)).
+struct EvalWs {
+  float4* qa;          // 3 * cap
+  float4* qb;          // 3 * cap
+  uint2* hits;         // cap: (bits(t), triangle in leaf order or kMiss)
+  float4* rec;         // L * cap (score only): incoming direction and triangle of vertex k of state s at [k * cap + s]
+  uint32_t* pinfo;     // cap (score only): refract mask | rays << 16 of the finished path
+  uint32_t* gradlist;  // cap (score only)
+  uint32_t* ctl;       // kCtlWords
+  uint32_t cap;
+};
+
+// Inputs and outputs of one evaluation, all indexed by state s (planes: [plane * stride + s]).
+struct EvalIO {
+  const float4* x;       // PSS coordinates, d/4 planes
+  size_t stride;
+  const uint32_t* order; // optional: queue slot t evaluates state order[t]
+  float4* g;             // score planes (score only); must be zero on entry
+  float4* f;             // (f.rgb, p)
+  uint32_t* pix;
+  uint32_t* sig;
+  uint32_t* nrays;       // optional
+  unsigned long long* rays_ctr;       // optional: += closest-hit queries
+  unsigned long long* nonfinite_ctr;  // optional: += states with non-finite f or score (Q18)
+  unsigned long long* work;           // optional (k_trace<true>): work[0] += node visits, work[1] += triangle tests
+};
+
+__device__ __forceinline__ float2 x_pair(const EvalIO& io, uint32_t s, uint32_t k) {  // coordinates (2k, 2k+1)
+  const float4 q = io.x[(size_t)(k >> 1) * io.stride + s];
+  return (k & 1u) ? make_float2(q.z, q.w) : make_float2(q.x, q.y);
+}
+__device__ __forceinline__ void g_pair(const EvalIO& io, uint32_t s, uint32_t k, float a, float b) {
+  reinterpret_cast<float2*>(&io.g[(size_t)(k >> 1) * io.stride + s])[k & 1u] = make_float2(a, b);
+}
+
+// ---- a3: camera rays -------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kShadeBlock) k_raygen(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
+  const uint32_t t = blockIdx.x * kShadeBlock + threadIdx.x;
+  if (t == 0) ws.ctl[kCtlCnt + 1] = n;
+  if (t >= n) return;
+  const uint32_t s = io.order ? io.order[t] : t;
+  const float4 x = io.x[s];
+  io.pix[s] = pixel_of(x.x, x.y, sc.W, sc.H);
+  const V3<float> d = camera_dir<float>(sc, x.x, x.y);
+  ws.qa[t] = make_float4(sc.cam_pos[0], sc.cam_pos[1], sc.cam_pos[2], __uint_as_float(s));
+  ws.qa[(size_t)ws.cap + t] = make_float4(d.x, d.y, d.z, __uint_as_float(kSigInit));
+  ws.qa[2 * (size_t)ws.cap + t] = make_float4(1.f, 1.f, 1.f, __uint_as_float(0u));
+}
+
+// ---- a4: closest hit, persistent ---------------------------------------------------------------------------------
+// Per-thread stacks in shared memory, entry e of thread t at base[e * kTraceBlock] (bank = lane: conflict-free).
+// Node groups grow up from entry 0; postponed triangle groups live in their own kTriStack entries above them.
+struct SmemStack {
+  uint2* base;
+  __device__ __forceinline__ void push(int sp, uint2 v) { base[sp * kTraceBlock] = v; }
+  __device__ __forceinline__ uint2 pop(int sp) const { return base[sp * kTraceBlock]; }
+};
+
+__device__ __forceinline__ void tri_one(const DevScene& sc, TravRay& r, TravState& s) {
+  const uint32_t li = s.tx + low_bit(s.ty);
+  s.ty &= s.ty - 1u;
+  tri_test(__ldg(&sc.tris[3 * li]), __ldg(&sc.tris[3 * li + 1]), __ldg(&sc.tris[3 * li + 2]), li, r);
+}
+
+// q: planes Q0, Q1 of the queue (o, d).  Every warp takes kFetchChunk rays at a time from *head and keeps its lanes
+// supplied from that private range.  The traversal runs in lockstep steps: every lane that has an internal child
+// to visit does one node test, then every lane with pending triangles tests up to kTrisPerStep of them, so lanes
+// in different phases of different rays still share instructions (DESIGN.md section 6 gives the warp-level
+// simulation this schedule was chosen from).
+template <bool STATS>
+__global__ void __launch_bounds__(kTraceBlock, 1)
+k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t* __restrict__ cnt, uint32_t* head,
+        uint2* __restrict__ hits, unsigned long long* work) {
+  extern __shared__ uint4 smem[];
+  const uint32_t n = *cnt;
+  if (n == 0) return;
+  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 5u; k += kTraceBlock) smem[k] = sc.nodes[k];
+  __syncthreads();
+  SmemStack st{reinterpret_cast<uint2*>(smem + 5u * sc.smem_nodes) + threadIdx.x};
+  SmemStack tst{st.base + (size_t)sc.stack_cap * kTraceBlock};
+  const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
+  constexpr unsigned kFull = 0xFFFFFFFFu;
+  uint32_t wnext = 0, wend = 0;  // this warp's private range of the queue
+  bool drained = false, active = false;
+  TravRay r;
+  TravState s;
+  int tsp = 0;  // postponed triangle groups
+  uint32_t ridx = 0, nn = 0, nt = 0;
+  trav_setup(r, 0.f, 0.f, 0.f, 1.f, 1.f, 1.f);
+  trav_begin(s);
+  for (;;) {
+    // ---- hand rays to the idle lanes
+    unsigned want = __ballot_sync(kFull, !active);
+    while (want && !drained) {
+      if (wnext == wend) {
+        uint32_t b = 0;
+        if (lane == 0) b = atomicAdd(head, kFetchChunk);
+        b = __shfl_sync(kFull, b, 0);
+        if (b >= n) { drained = true; break; }
+        wnext = b;
+        wend = min(b + kFetchChunk, n);
+      }
+      const uint32_t rank = __popc(want & lt);
+      const bool mine = ((want >> lane) & 1u) && rank < wend - wnext;
+      if (mine) {
+        ridx = wnext + rank;
+        const float4 o = q[ridx], d = q[(size_t)cap + ridx];
+        trav_setup(r, o.x, o.y, o.z, d.x, d.y, d.z);
+        trav_begin(s);
+        tsp = 0;
+        active = true;
+      }
+      const unsigned got = __ballot_sync(kFull, mine);
+      wnext += __popc(got);
+      want &= ~got;
+    }
+    unsigned act = __ballot_sync(kFull, active);
+    if (!act) break;
+    // ---- lockstep traversal
+    do {
+      if (active && (s.gy & 0xFF000000u)) {  // visit the next internal child
+        const uint32_t node = trav_next_node(s, st, r);
+        const uint4* np = node < sc.smem_nodes ? smem + 5u * node : sc.nodes + 5u * (size_t)node;
+        const uint4 w0 = np[0], w1 = np[1], w2 = np[2], w3 = np[3], w4 = np[4];
+        if (STATS) ++nn;
+        const uint32_t h = node_hits(w0, w1, w2, w3, w4, r);
+        const uint32_t nty = h & 0x00FFFFFFu;
+        if (nty) {
+          if (s.ty) {  // triangles still pending from an earlier node: postpone them (or test them now if full)
+            if (tsp < kTriStack) tst.push(tsp++, make_uint2(s.tx, s.ty));
+            else while (s.ty) { if (STATS) ++nt; tri_one(sc, r, s); }
+          }
+          s.tx = w1.y;
+          s.ty = nty;
+        }
+        s.gx = w1.x;
+        s.gy = (h & 0xFF000000u) | (w0.w >> 24);
+      }
+#pragma unroll
+      for (int it = 0; it < kTrisPerStep; ++it) {
+        if (active) {
+          if (!s.ty && tsp > 0) { const uint2 e = tst.pop(--tsp); s.tx = e.x; s.ty = e.y; }
+          if (s.ty) { if (STATS) ++nt; tri_one(sc, r, s); }
+        }
+      }
+      if (active && !(s.gy & 0xFF000000u)) {  // node group exhausted: next one from the stack, or done
+        if (s.sp > 0) {
+          const uint2 e = st.pop(--s.sp);
+          s.gx = e.x; s.gy = e.y;
+        } else if (!s.ty && tsp == 0) {
+          hits[ridx] = make_uint2(__float_as_uint(r.t), r.li);
+          active = false;
+        }
+      }
+      act = __ballot_sync(kFull, active);
+    } while (drained ? act != 0u : __popc(act) >= kRefillBelow);
+  }
+  if (STATS) {
+    nn = __reduce_add_sync(kFull, nn);
+    nt = __reduce_add_sync(kFull, nt);
+    if (lane == 0) { atomicAdd(&work[0], (unsigned long long)nn); atomicAdd(&work[1], (unsigned long long)nt); }
+  }
+}
+
+// ---- a3 / a5: shade vertex k of every ray of segment k -------------------------------------------------------------
+template <bool GRAD>
+__global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, EvalIO io, uint32_t k) {
+  __shared__ uint32_t s_warp[kShadeBlock / 32];
+  __shared__ uint32_t s_base;
+  const uint32_t n = ws.ctl[kCtlCnt + k];
+  if (blockIdx.x * kShadeBlock >= n) return;  // whole block past the end of the queue
+  const uint32_t j = blockIdx.x * kShadeBlock + threadIdx.x;
+  const float4* qin = (k & 1u) ? ws.qa : ws.qb;
+  float4* qout = (k & 1u) ? ws.qb : ws.qa;
+  const size_t cap = ws.cap;
+  bool cont = false, want_grad = false;
+  float4 n0, n1, n2;
+  uint32_t bad = 0, s = 0;
+  if (j < n) {
+    const float4 Q0 = qin[j], Q1 = qin[cap + j], Q2 = qin[2 * cap + j];
+    const uint2 h = ws.hits[j];
+    s = __float_as_uint(Q0.w);
+    uint32_t sig = __float_as_uint(Q1.w), info = __float_as_uint(Q2.w);
+    const float3 o = xyz(Q0), d = xyz(Q1);
+    float T0 = Q2.x, T1 = Q2.y, T2 = Q2.z;
+    float f0 = 0.f, f1 = 0.f, f2 = 0.f;
+    bool done = true;
+    if (h.y == kMiss) {
+      sig = fnv(sig, 0u);
+      f0 = T0 * sc.env[0]; f1 = T1 * sc.env[1]; f2 = T2 * sc.env[2];
+    } else {
+      const uint32_t li = h.y;
+      const float4 q0 = __ldg(&sc.tris[3 * li]), q1 = __ldg(&sc.tris[3 * li + 1]), q2 = __ldg(&sc.tris[3 * li + 2]);
+      sig = fnv(sig, __float_as_uint(q0.w) + 1u);
+      const uint32_t mi = __float_as_uint(q1.w);
+      const float4 m0 = __ldg(&sc.mats[3 * mi]), m1 = __ldg(&sc.mats[3 * mi + 1]);
+      const uint32_t kind = __float_as_uint(m0.x);
+      Frame fr;
+      float dn;
+      tri_frame(xyz(q1), xyz(q2), d, fr, dn);
+      if (kind == 3u) {  // emitter: front face emits, path stops
+        if (dn < 0.f) {
+          sig = fnv(sig, 4u);
+          const float4 m2 = __ldg(&sc.mats[3 * mi + 2]);
+          f0 = T0 * m1.z; f1 = T1 * m1.w; f2 = T2 * m2.x;
+        } else {
+          sig = fnv(sig, 5u);
+        }
+      } else if (k < sc.L) {
+        const float3 hit = o + d * __uint_as_float(h.x);
+        const float2 u = x_pair(io, s, k);
+        if (GRAD) ws.rec[(size_t)k * cap + s] = make_float4(d.x, d.y, d.z, __uint_as_float(li));
+        V3<float> din{d.x, d.y, d.z}, dnew;
+        float off = 1.f;
+        if (kind == 0u) {
+          sig = fnv(sig, 0u);
+          dnew = lambert_dir<float>(fr, u.x, u.y);
+          T0 *= m0.y; T1 *= m0.z; T2 *= m0.w;
+        } else if (kind == 1u) {
+          const float eta = dn < 0.f ? m1.x : 1.0f / m1.x;
+          const float F = fresnel_dielectric(-dot3(d, fr.nf), eta);
+          const bool reflect = u.x < F;
+          sig = fnv(sig, reflect ? 1u : 2u);
+          if (!reflect) { off = -1.f; info |= 1u << k; }
+          dnew = dielectric_dir<float>(fr, eta, reflect, din);
+        } else {
+          sig = fnv(sig, 3u);
+          info |= 1u << 16;
+          float c5, G1;
+          if (!ggx_dir<float>(fr, m1.y, din, u.x, u.y, dnew, c5, G1)) {
+            T0 = T1 = T2 = 0.f;
+          } else {
+            T0 *= (m0.y + (1.0f - m0.y) * c5) * G1;
+            T1 *= (m0.z + (1.0f - m0.z) * c5) * G1;
+            T2 *= (m0.w + (1.0f - m0.w) * c5) * G1;
+          }
+        }
+        if (!(T0 == 0.f && T1 == 0.f && T2 == 0.f)) {
+          done = false;
+          const float3 on = hit + fr.nf * (sc.eps_ray * off);
+          n0 = make_float4(on.x, on.y, on.z, Q0.w);
+          n1 = make_float4(dnew.x, dnew.y, dnew.z, __uint_as_float(sig));
+          n2 = make_float4(T0, T1, T2, __uint_as_float(info));
+        }
+      }
+    }
+    cont = !done;
+    if (done) {
+      float p = f0 * 0.2126f + f1 * 0.7152f + f2 * 0.0722f;
+      if (!(isfinite(f0) && isfinite(f1) && isfinite(f2) && isfinite(p))) { f0 = f1 = f2 = p = 0.f; bad = 1; }
+      io.f[s] = make_float4(f0, f1, f2, p);
+      io.sig[s] = sig;
+      if (io.nrays) io.nrays[s] = k;
+      if (GRAD) {
+        ws.pinfo[s] = (info & 0xFFFFu) | (k << 16);
+        // only GGX weights depend on x: no GGX vertex or p == 0  =>  score == 0 exactly
+        want_grad = (info >> 16) && p > 0.f;
+      }
+    }
+  }
+  const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
+  if (GRAD) {  // reverse-pass list: one atomic per warp
+    const unsigned gm = __ballot_sync(0xFFFFFFFFu, want_grad);
+    if (gm) {
+      uint32_t base = 0;
+      if (lane == 0) base = atomicAdd(&ws.ctl[kCtlGrad], (uint32_t)__popc(gm));
+      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      if (want_grad) ws.gradlist[base + __popc(gm & ((1u << lane) - 1u))] = s;
+    }
+  }
+  // compaction of the surviving paths into the next queue: warp ballot, block prefix, one atomic per block
+  const unsigned b = __ballot_sync(0xFFFFFFFFu, cont);
+  if (lane == 0) s_warp[wid] = __popc(b);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t tot = 0;
+    for (int w = 0; w < kShadeBlock / 32; ++w) { const uint32_t c = s_warp[w]; s_warp[w] = tot; tot += c; }
+    s_base = tot ? atomicAdd(&ws.ctl[kCtlCnt + k + 1], tot) : 0u;
+    if (j == 0 && io.rays_ctr) atomicAdd(io.rays_ctr, (unsigned long long)n);
+  }
+  __syncthreads();
+  if (cont) {
+    const size_t at = s_base + s_warp[wid] + __popc(b & ((1u << lane) - 1u));
+    qout[at] = n0; qout[cap + at] = n1; qout[2 * cap + at] = n2;
+  }
+  if (io.nonfinite_ctr) {
+    bad = __reduce_add_sync(0xFFFFFFFFu, bad);
+    if (lane == 0 && bad) atomicAdd(io.nonfinite_ctr, (unsigned long long)bad);
+  }
+}
+
+// ---- a6: score by reverse accumulation -------------------------------------------------------------------------------
+// With every discrete outcome frozen, grad p flows back from each GGX vertex through the chain of preceding specular
+// vertices to the first diffuse vertex or the camera ("Score").  One thread = one listed state.
+__global__ void __launch_bounds__(kGradBlock) k_grad(DevScene sc, EvalWs ws, EvalIO io) {
+  const uint32_t idx = blockIdx.x * kGradBlock + threadIdx.x;
+  if (idx >= ws.ctl[kCtlGrad]) return;
+  const uint32_t s = ws.gradlist[idx];
+  const size_t cap = ws.cap;
+  const float4 fp = io.f[s];
+  const uint32_t info = ws.pinfo[s];
+  const uint32_t refract_mask = info & 0xFFFFu, nvert = (info >> 16) - 1u;  // vertices 1..nvert sampled a direction
+  const float inv_phat = 1.0f / (fp.w + kEps);
+  const float A0 = 0.2126f * fp.x, A1 = 0.7152f * fp.y, A2 = 0.0722f * fp.z;  // d p / d ln(w_c) per channel
+  float db0 = 0.f, db1 = 0.f, db2 = 0.f;  // adjoint of the outgoing direction of the current vertex
+  bool bad = false;
+  for (uint32_t k = nvert; k >= 1; --k) {
+    float ga = 0.f, gb = 0.f;
+    const float4 rc = ws.rec[(size_t)k * cap + s];
+    const uint32_t li = __float_as_uint(rc.w);
+    const float3 din = xyz(rc);
+    const float4 q1 = __ldg(&sc.tris[3 * li + 1]), q2 = __ldg(&sc.tris[3 * li + 2]);
+    const uint32_t mi = __float_as_uint(q1.w);
+    const float4 m0 = __ldg(&sc.mats[3 * mi]), m1 = __ldg(&sc.mats[3 * mi + 1]);
+    const uint32_t kind = __float_as_uint(m0.x);
+    Frame fr;
+    float dn;
+    tri_frame(xyz(q1), xyz(q2), din, fr, dn);
+    const float2 u = x_pair(io, s, k);
+    const bool live = db0 != 0.f || db1 != 0.f || db2 != 0.f;
+    if (kind == 0u) {
+      if (live) {
+        const V3<Du<2>> w = lambert_dir<Du<2>>(fr, du_var<2>(u.x, 0), du_var<2>(u.y, 1));
+        ga = db0 * w.x.d[0] + db1 * w.y.d[0] + db2 * w.z.d[0];
+        gb = db0 * w.x.d[1] + db1 * w.y.d[1] + db2 * w.z.d[1];
+      }
+      db0 = db1 = db2 = 0.f;  // a diffuse vertex forgets the incoming direction
+    } else if (kind == 1u) {
+      if (live) {
+        const float eta = dn < 0.f ? m1.x : 1.0f / m1.x;
+        V3<Du<3>> di{du_var<3>(din.x, 0), du_var<3>(din.y, 1), du_var<3>(din.z, 2)};
+        const V3<Du<3>> w = dielectric_dir<Du<3>>(fr, eta, !((refract_mask >> k) & 1u), di);
+        const float n0 = db0 * w.x.d[0] + db1 * w.y.d[0] + db2 * w.z.d[0];
+        const float n1 = db0 * w.x.d[1] + db1 * w.y.d[1] + db2 * w.z.d[1];
+        const float n2 = db0 * w.x.d[2] + db1 * w.y.d[2] + db2 * w.z.d[2];
+        db0 = n0; db1 = n1; db2 = n2;
+      }
+    } else if (kind == 2u) {
+      V3<Du<5>> di{du_var<5>(din.x, 2), du_var<5>(din.y, 3), du_var<5>(din.z, 4)};
+      V3<Du<5>> w;
+      Du<5> c5, G1;
+      if (ggx_dir<Du<5>>(fr, m1.y, di, du_var<5>(u.x, 0), du_var<5>(u.y, 1), w, c5, G1)) {
+        // S = sum_c (A_c / w_c) w_c(x) with w_c = (F0_c + (1 - F0_c) c5) G1
+        const float w0 = (m0.y + (1.0f - m0.y) * c5.v) * G1.v, w1 = (m0.z + (1.0f - m0.z) * c5.v) * G1.v,
+                    w2 = (m0.w + (1.0f - m0.w) * c5.v) * G1.v;
+        const float B0 = w0 > 0.f ? A0 / w0 : 0.f, B1 = w1 > 0.f ? A1 / w1 : 0.f, B2 = w2 > 0.f ? A2 / w2 : 0.f;
+        const float a0 = B0 * m0.y + B1 * m0.z + B2 * m0.w;
+        const float a1 = B0 * (1.0f - m0.y) + B1 * (1.0f - m0.z) + B2 * (1.0f - m0.w);
+        const Du<5> S = G1 * (c5 * a1 + a0);
+        float nj[5];
+#pragma unroll
+        for (int j = 0; j < 5; ++j) nj[j] = db0 * w.x.d[j] + db1 * w.y.d[j] + db2 * w.z.d[j] + S.d[j];
+        ga = nj[0]; gb = nj[1];
+        db0 = nj[2]; db1 = nj[3]; db2 = nj[4];
+      }
+    }
+    ga *= inv_phat; gb *= inv_phat;
+    bad = bad || !(isfinite(ga) && isfinite(gb));
+    g_pair(io, s, k, ga, gb);
+  }
+  {
+    float ga = 0.f, gb = 0.f;
+    if (db0 != 0.f || db1 != 0.f || db2 != 0.f) {
+      const float4 x = io.x[s];
+      const V3<Du<2>> w = camera_dir<Du<2>>(sc, du_var<2>(x.x, 0), du_var<2>(x.y, 1));
+      ga = (db0 * w.x.d[0] + db1 * w.y.d[0] + db2 * w.z.d[0]) * inv_phat;
+      gb = (db0 * w.x.d[1] + db1 * w.y.d[1] + db2 * w.z.d[1]) * inv_phat;
+    }
+    bad = bad || !(isfinite(ga) && isfinite(gb));
+    g_pair(io, s, 0, ga, gb);
+  }
+  if (bad) {  // Q18: a non-finite score makes the state a zero-contribution state
+    io.f[s] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (uint32_t k = 0; k <= nvert; ++k) g_pair(io, s, k, 0.f, 0.f);
+    if (io.nonfinite_ctr) atomicAdd(io.nonfinite_ctr, 1ull);
+  }
+}
+
+// ---- the 2-D analytic target (no rays) -----------------------------------------------------------------------------------
+template <bool GRAD>
+__global__ void __launch_bounds__(kShadeBlock) k_eval_analytic(DevScene sc, EvalIO io, uint32_t n) {
+  const uint32_t t = blockIdx.x * kShadeBlock + threadIdx.x;
+  if (t >= n) return;
+  const uint32_t s = io.order ? io.order[t] : t;
+  const float4 x = io.x[s];
+  float p, g0, g1;
+  eval_analytic(sc, x.x, x.y, p, g0, g1);
+  const bool bad = !isfinite(p) || (GRAD && !(isfinite(g0) && isfinite(g1)));
+  if (bad) { p = 0.f; g0 = g1 = 0.f; if (io.nonfinite_ctr) atomicAdd(io.nonfinite_ctr, 1ull); }
+  io.f[s] = make_float4(p, p, p, p);
+  io.pix[s] = pixel_of(x.x, x.y, sc.W, sc.H);
+  io.sig[s] = 0u;
+  if (io.nrays) io.nrays[s] = 0u;
+  if (GRAD) g_pair(io, s, 0, g0, g1);
+}
+
+}  // namespace dr

@@ -1,15 +1,15 @@
-// Chain kernels: propose (a1, a2, a10), eval (a3-a6), decide (a7, a8, a11 + block kill counts),
-// scan / scatter (a9), bootstrap (a0), resolve (a12).  One thread = one chain; chain state is
-// structure-of-arrays: x and score as d/4 planes of float4[N], so every load/store below is a coalesced
-// 128-bit access (the paper's array-of-structs stateBuffer is prior art, not the layout used here).
+// Chain kernels: propose (a1, a2, a10), decide (a7, a8, a11 + block kill counts), scan / scatter (a9),
+// bootstrap (a0), resolve (a12); the target evaluation between propose and decide (a3-a6) is dr_eval.cuh.
+// One thread = one chain; chain state is structure-of-arrays: x and score as d/4 planes of
+// float4[N], so every load/store below is a coalesced 128-bit access (the paper's array-of-structs stateBuffer
+// is prior art, not the layout used here).
 #pragma once
-#include "dr_path.cuh"
+#include "dr_eval.cuh"
 #include "dr_rng.cuh"
 
 namespace dr {
 
 constexpr int kBlock = 256;      // streaming kernels
-constexpr int kEvalBlock = 128;  // path evaluation (register heavy)
 
 struct Counters {
   unsigned long long tours, mutations, rays, mh_accepts, nonfinite;
@@ -106,36 +106,7 @@ __global__ void __launch_bounds__(kBlock) k_propose(ChainParams cp, ChainState s
       }
     }
     st.y[at] = mask_dims(y, j, cp.d);
-  }
-}
-
-// a3-a6: evaluate the proposal of every chain, in the order given by st.order (alive chains first, then the
-// regeneration queue, so that a warp holds either local moves or fresh samples).
-template <bool GRAD>
-__global__ void __launch_bounds__(kEvalBlock) k_eval(DevScene sc, ChainParams cp, ChainState st, int use_order) {
-  extern __shared__ float4 snodes[];
-  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 16u; k += kEvalBlock) snodes[k] = sc.nodes[k];
-  __syncthreads();
-  const uint32_t t = blockIdx.x * kEvalBlock + threadIdx.x;
-  uint32_t nrays = 0, bad = 0;
-  if (t < cp.N) {
-    const uint32_t i = use_order ? st.order[t] : t;
-    XView xv{st.y, nullptr, cp.N, i};
-    GView gv{st.gy, nullptr, cp.N, i};
-    EvalOut e;
-    if (sc.analytic) eval_analytic<GRAD>(sc, xv, e, gv);
-    else eval_path<GRAD>(sc, snodes, xv, e, gv);
-    st.fy[i] = make_float4(e.f[0], e.f[1], e.f[2], e.p);
-    st.pixy[i] = e.pix;
-    st.sigy[i] = e.sig;
-    nrays = e.nrays;
-    bad = e.nonfinite ? 1u : 0u;
-  }
-  nrays = __reduce_add_sync(0xFFFFFFFFu, nrays);
-  bad = __reduce_add_sync(0xFFFFFFFFu, bad);
-  if ((threadIdx.x & 31) == 0) {
-    if (nrays) atomicAdd(&st.ctr->rays, (unsigned long long)nrays);
-    if (bad) atomicAdd(&st.ctr->nonfinite, (unsigned long long)bad);
+    if (cp.grad) st.gy[at] = make_float4(0.f, 0.f, 0.f, 0.f);  // the evaluation writes only non-zero scores
   }
 }
 
@@ -339,75 +310,20 @@ __global__ void __launch_bounds__(kBlock) k_resolve(ChainParams cp, const Counte
 }
 
 // ---- test hooks -------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kEvalBlock) k_trace(DevScene sc, const float* o, const float* d, uint32_t n, float* t,
-                                                      uint32_t* prim) {
-  extern __shared__ float4 snodes[];
-  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 16u; k += kEvalBlock) snodes[k] = sc.nodes[k];
-  __syncthreads();
-  const uint32_t i = blockIdx.x * kEvalBlock + threadIdx.x;
+// dr_trace_rays: user rays -> queue planes (o, d), and hits -> (t, original triangle id).
+__global__ void k_pack_rays(const float* o, const float* d, uint32_t n, float4* q, uint32_t cap, uint32_t* cnt) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) *cnt = n;
   if (i >= n) return;
-  const HitRec h = closest_hit(sc, snodes, make_float3(o[3 * i], o[3 * i + 1], o[3 * i + 2]),
-                               make_float3(d[3 * i], d[3 * i + 1], d[3 * i + 2]));
-  if (h.li == 0xFFFFFFFFu) { t[i] = -1.f; prim[i] = 0xFFFFFFFFu; }
-  else { t[i] = h.t; prim[i] = __float_as_uint(sc.tris[3 * h.li].w); }
+  q[i] = make_float4(o[3 * i], o[3 * i + 1], o[3 * i + 2], 0.f);
+  q[(size_t)cap + i] = make_float4(d[3 * i], d[3 * i + 1], d[3 * i + 2], 0.f);
 }
-
-template <bool GRAD>
-__global__ void __launch_bounds__(kEvalBlock) k_eval_states(DevScene sc, const float* x, uint32_t n, float* f, float* p,
-                                                            uint32_t* pix, float* score, uint32_t* nrays, uint32_t* sig) {
-  extern __shared__ float4 snodes[];
-  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 16u; k += kEvalBlock) snodes[k] = sc.nodes[k];
-  __syncthreads();
-  const uint32_t i = blockIdx.x * kEvalBlock + threadIdx.x;
+__global__ void k_unpack_hits(DevScene sc, const uint2* hits, uint32_t n, float* t, uint32_t* prim) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  XView xv{nullptr, x + (size_t)i * sc.d, 0, 0};
-  GView gv{nullptr, GRAD ? score + (size_t)i * sc.d : nullptr, 0, 0};
-  EvalOut e;
-  if (sc.analytic) eval_analytic<GRAD>(sc, xv, e, gv);
-  else eval_path<GRAD>(sc, snodes, xv, e, gv);
-  f[3 * i] = e.f[0]; f[3 * i + 1] = e.f[1]; f[3 * i + 2] = e.f[2];
-  p[i] = e.p; pix[i] = e.pix; nrays[i] = e.nrays; sig[i] = e.sig;
-}
-
-// Work statistics of the evaluation of n states: totals of rays, BVH8 node visits and triangle tests
-// (the algorithmic work the roofline of bench.py is computed from).  out[0..2] += totals.
-__global__ void __launch_bounds__(kEvalBlock) k_eval_stats(DevScene sc, const float* x, uint32_t n, unsigned long long* out) {
-  extern __shared__ float4 snodes[];
-  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 16u; k += kEvalBlock) snodes[k] = sc.nodes[k];
-  __syncthreads();
-  const uint32_t i = blockIdx.x * kEvalBlock + threadIdx.x;
-  uint32_t nr = 0, nn = 0, nt = 0;
-  if (i < n && !sc.analytic) {
-    XView xv{nullptr, x + (size_t)i * sc.d, 0, 0};
-    GView gv{nullptr, nullptr, 0, 0};
-    EvalOut e;
-    eval_path<false, true>(sc, snodes, xv, e, gv, &nn, &nt);
-    nr = e.nrays;
-  }
-  nr = __reduce_add_sync(0xFFFFFFFFu, nr); nn = __reduce_add_sync(0xFFFFFFFFu, nn); nt = __reduce_add_sync(0xFFFFFFFFu, nt);
-  if ((threadIdx.x & 31) == 0) {
-    atomicAdd(&out[0], (unsigned long long)nr); atomicAdd(&out[1], (unsigned long long)nn); atomicAdd(&out[2], (unsigned long long)nt);
-  }
-}
-
-// Same statistics for the chains' last proposals (the states the last k_eval launch evaluated).
-__global__ void __launch_bounds__(kEvalBlock) k_chain_stats(DevScene sc, ChainParams cp, ChainState st, unsigned long long* out) {
-  extern __shared__ float4 snodes[];
-  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 16u; k += kEvalBlock) snodes[k] = sc.nodes[k];
-  __syncthreads();
-  const uint32_t i = blockIdx.x * kEvalBlock + threadIdx.x;
-  uint32_t nr = 0, nn = 0, nt = 0;
-  if (i < cp.N && !sc.analytic) {
-    XView xv{st.y, nullptr, cp.N, i};
-    GView gv{nullptr, nullptr, 0, 0};
-    EvalOut e;
-    eval_path<false, true>(sc, snodes, xv, e, gv, &nn, &nt);
-    nr = e.nrays;
-  }
-  nr = __reduce_add_sync(0xFFFFFFFFu, nr); nn = __reduce_add_sync(0xFFFFFFFFu, nn); nt = __reduce_add_sync(0xFFFFFFFFu, nt);
-  if ((threadIdx.x & 31) == 0) {
-    atomicAdd(&out[0], (unsigned long long)nr); atomicAdd(&out[1], (unsigned long long)nn); atomicAdd(&out[2], (unsigned long long)nt);
-  }
+  const uint2 h = hits[i];
+  if (h.y == kMiss) { t[i] = -1.f; prim[i] = 0xFFFFFFFFu; }
+  else { t[i] = __uint_as_float(h.x); prim[i] = __float_as_uint(sc.tris[3 * h.y].w); }
 }
 
 __global__ void k_philox_blocks(uint64_t seed, const uint32_t* ctr, uint32_t n, uint32_t* out) {

@@ -8,20 +8,34 @@ namespace dr {
 
 constexpr int kMaxPathLen = 16;        // L <= 16, d = 2L <= 32 (BASELINE.json configs[3])
 constexpr int kMaxPlanes = 8;          // d / 4 float4 planes
-constexpr uint32_t kLeafBit = 0x80000000u;
-constexpr uint32_t kEmptyChild = 0xFFFFFFFFu;
-constexpr int kSmemNodes = 73;         // root + 8 + 64: the top three BVH8 levels staged in shared memory
 constexpr int kMaxMix = 16;
+constexpr int kMaxLeafTris = 3;        // triangles per leaf (unary count in the child's meta byte)
+constexpr int kMaxSmemNodes = 585;     // 1 + 8 + 64 + 512: the top four BVH8 levels, staged in shared memory
+constexpr int kMaxBvhDepth = 30;       // traversal stack entries per ray = depth + 1 (shared memory)
 
-// BVH8 node, 256 bytes, child boxes as structure-of-arrays so a lane reads them as float4 pairs.
-// child[i]: kEmptyChild, or internal node index, or kLeafBit | (count-1) << 27 | first triangle (leaf order).
-struct alignas(256) Node8 {
-  float lo[3][8];
-  float hi[3][8];
-  uint32_t child[8];
-  uint32_t pad[8];
+// BVH8 node, 80 bytes = five 16-byte words.  Child boxes are quantised to 8 bits per plane on a per-node
+// grid (origin p, per-axis power-of-two cell 2^(e-127)), rounded outwards, so a node costs five 128-bit loads.
+//   w0 = (p.x, p.y, p.z, e_x | e_y << 8 | e_z << 16 | imask << 24)      imask: bit s = slot s is an internal node
+//   w1 = (child_base, tri_base, meta[0..3], meta[4..7])
+//   w2 = (qlo_x[0..3], qlo_x[4..7], qlo_y[0..3], qlo_y[4..7])
+//   w3 = (qlo_z[0..3], qlo_z[4..7], qhi_x[0..3], qhi_x[4..7])
+//   w4 = (qhi_y[0..3], qhi_y[4..7], qhi_z[0..3], qhi_z[4..7])
+// meta[s]: 0 = empty slot; internal child: 0b001_11sss (one work bit at position 24 + s);
+//          leaf with n <= 3 triangles at tri_base + off (off <= 23): ((1 << n) - 1) << 5 | off.
+// Internal children of a node are stored contiguously from child_base in slot order: the child in slot s is
+// node child_base + popcount(imask & ((1 << s) - 1)).  Slots are assigned so that children lie towards corner
+// (s&4 ? +x : -x, s&2 ? +y : -y, s&1 ? +z : -z) of the node: visiting slots in the order of descending
+// (s ^ octinv), octinv = (d.x >= 0 ? 4 : 0) | (d.y >= 0 ? 2 : 0) | (d.z >= 0 ? 1 : 0), is roughly front to back.
+struct alignas(16) NodeC {
+  float p[3];
+  uint8_t e[3];
+  uint8_t imask;
+  uint32_t child_base, tri_base;
+  uint8_t meta[8];
+  uint8_t qlo[3][8];
+  uint8_t qhi[3][8];
 };
-static_assert(sizeof(Node8) == 256, "Node8 must be 256 bytes");
+static_assert(sizeof(NodeC) == 80, "NodeC must be 80 bytes");
 
 // Triangle in leaf order, 48 bytes: three float4.
 //   q0 = (v0.xyz, bits(original triangle id)), q1 = (e1.xyz, bits(material id)), q2 = (e2.xyz, 0)
@@ -41,14 +55,14 @@ struct MatPacked {
 static_assert(sizeof(MatPacked) == 48, "MatPacked must be 48 bytes");
 
 struct BuiltBvh {
-  std::vector<Node8> nodes;         // breadth-first order: node 0 = root, top levels first
-  std::vector<TriPacked> tris;      // leaf order
-  uint32_t depth = 0;
+  std::vector<NodeC> nodes;         // breadth-first order: node 0 = root, top levels first
+  std::vector<TriPacked> tris;      // leaf order (the leaves of one node are contiguous)
+  uint32_t depth = 0;               // levels of BVH8 nodes
   float sah_cost = 0.f;
   float diag = 0.f;
 };
 
-// Binned-SAH BVH2 -> BVH8 collapse (host).  verts: 3*nv floats, idx: 3*nt, tri_mat: nt.
+// Binned-SAH BVH2 -> BVH8 collapse -> slot assignment -> quantisation (host).  verts: 3*nv floats, idx: 3*nt, tri_mat: nt.
 void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t nt, const uint32_t* tri_mat, BuiltBvh& out);
 
 }  // namespace dr
