@@ -24,6 +24,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                "-Xcompiler", "-fPIC", "-o", LIB]
         if verbose:
             cmd += ["-Xptxas", "-v"]
+        cmd += os.environ.get("DR_NVCC_FLAGS", "").split()   # e.g. -DDR_TRACE_BLOCK=640 for a tuning sweep
         cmd += [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.run(cmd, check=True, cwd=CSRC)
     return LIB

@@ -15,13 +15,25 @@
 
 namespace dr {
 
-constexpr int kTraceBlock = 640;   // one persistent block per SM
-constexpr int kTriStack = 12;      // postponed triangle groups per ray
-constexpr int kTrisPerStep = 2;    // triangle tests per lockstep step
+#ifndef DR_TRACE_BLOCK
+#define DR_TRACE_BLOCK 640
+#endif
+#ifndef DR_TRI_STACK
+#define DR_TRI_STACK 12
+#endif
+#ifndef DR_TRIS_PER_STEP
+#define DR_TRIS_PER_STEP 2
+#endif
+#ifndef DR_REFILL_BELOW
+#define DR_REFILL_BELOW 30
+#endif
+constexpr int kTraceBlock = DR_TRACE_BLOCK;   // one persistent block per SM
+constexpr int kTriStack = DR_TRI_STACK;      // postponed triangle groups per ray
+constexpr int kTrisPerStep = DR_TRIS_PER_STEP;    // triangle tests per lockstep step
 constexpr int kShadeBlock = 256;
 constexpr int kGradBlock = 128;
 constexpr uint32_t kFetchChunk = 64;   // rays a warp takes from the queue per atomic
-constexpr int kRefillBelow = 30;       // a warp goes back to the queue when fewer lanes than this hold a ray
+constexpr int kRefillBelow = DR_REFILL_BELOW;       // a warp goes back to the queue when fewer lanes than this hold a ray
 constexpr uint32_t kSigInit = 2166136261u;
 constexpr uint32_t kMiss = 0xFFFFFFFFu;
 
@@ -96,11 +108,31 @@ __device__ __forceinline__ void tri_one(const DevScene& sc, TravRay& r, TravStat
   tri_test(__ldg(&sc.tris[3 * li]), __ldg(&sc.tris[3 * li + 1]), __ldg(&sc.tris[3 * li + 2]), li, r);
 }
 
+// One prefetched triangle of a lane: its three words are requested one step before they are tested.
+struct TriSlot {
+  float4 q0, q1, q2;
+  uint32_t li;  // leaf-order index, kMiss = empty
+};
+
+__device__ __forceinline__ void tri_fetch(const DevScene& sc, TravState& s, SmemStack& tst, int& tsp, TriSlot& t) {
+  if (!s.ty && tsp > 0) { const uint2 e = tst.pop(--tsp); s.tx = e.x; s.ty = e.y; }
+  if (s.ty) {
+    t.li = s.tx + low_bit(s.ty);
+    s.ty &= s.ty - 1u;
+    const float4* p = sc.tris + 3 * (size_t)t.li;
+    t.q0 = __ldg(p); t.q1 = __ldg(p + 1); t.q2 = __ldg(p + 2);
+  }
+}
+
 // q: planes Q0, Q1 of the queue (o, d).  Every warp takes kFetchChunk rays at a time from *head and keeps its lanes
-// supplied from that private range.  The traversal runs in lockstep steps: every lane that has an internal child
-// to visit does one node test, then every lane with pending triangles tests up to kTrisPerStep of them, so lanes
-// in different phases of different rays still share instructions (DESIGN.md section 6 gives the warp-level
-// simulation this schedule was chosen from).
+// supplied from that private range.  The traversal runs in lockstep steps, software-pipelined one step deep so that
+// every load has a phase of arithmetic between its issue and its first use (profiles/r01b: the un-pipelined loop
+// spent 35 % of its warp-cycles waiting for the node and triangle words, one L2 round trip after the other):
+//   A  node test of the node whose five words were requested in step k-1           (new children, new triangles)
+//   N  choose the next node (nearest octant first), request its words               -> in flight during T
+//   T  test the (up to kTrisPerStep) triangles whose words were requested in step k-1
+//   F  choose the next triangles, request their words                               -> in flight during A of step k+1
+// Lanes in different phases of different rays share the instructions of all four parts.
 template <bool STATS>
 __global__ void __launch_bounds__(kTraceBlock, 1)
 k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t* __restrict__ cnt, uint32_t* head,
@@ -115,13 +147,18 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr unsigned kFull = 0xFFFFFFFFu;
   uint32_t wnext = 0, wend = 0;  // this warp's private range of the queue
-  bool drained = false, active = false;
+  bool drained = false, active = false, has_node = false;
   TravRay r;
   TravState s;
+  uint4 w0, w1, w2, w3, w4;      // words of the node to test next (valid if has_node)
+  TriSlot tri[kTrisPerStep];
   int tsp = 0;  // postponed triangle groups
   uint32_t ridx = 0, nn = 0, nt = 0;
   trav_setup(r, 0.f, 0.f, 0.f, 1.f, 1.f, 1.f);
   trav_begin(s);
+  w0 = w1 = w2 = w3 = w4 = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+  for (int it = 0; it < kTrisPerStep; ++it) { tri[it].li = kMiss; tri[it].q0 = tri[it].q1 = tri[it].q2 = make_float4(0.f, 0.f, 0.f, 0.f); }
   for (;;) {
     // ---- hand rays to the idle lanes
     unsigned want = __ballot_sync(kFull, !active);
@@ -140,7 +177,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
         ridx = wnext + rank;
         const float4 o = q[ridx], d = q[(size_t)cap + ridx];
         trav_setup(r, o.x, o.y, o.z, d.x, d.y, d.z);
-        trav_begin(s);
+        trav_begin(s);   // one work bit: the root, requested by part N of the first step
         tsp = 0;
         active = true;
       }
@@ -152,10 +189,8 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
     if (!act) break;
     // ---- lockstep traversal
     do {
-      if (active && (s.gy & 0xFF000000u)) {  // visit the next internal child
-        const uint32_t node = trav_next_node(s, st, r);
-        const uint4* np = node < sc.smem_nodes ? smem + 5u * node : sc.nodes + 5u * (size_t)node;
-        const uint4 w0 = np[0], w1 = np[1], w2 = np[2], w3 = np[3], w4 = np[4];
+      // A: node test
+      if (has_node) {
         if (STATS) ++nn;
         const uint32_t h = node_hits(w0, w1, w2, w3, w4, r);
         const uint32_t nty = h & 0x00FFFFFFu;
@@ -169,19 +204,42 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
         }
         s.gx = w1.x;
         s.gy = (h & 0xFF000000u) | (w0.w >> 24);
+        has_node = false;
       }
-#pragma unroll
-      for (int it = 0; it < kTrisPerStep; ++it) {
-        if (active) {
-          if (!s.ty && tsp > 0) { const uint2 e = tst.pop(--tsp); s.tx = e.x; s.ty = e.y; }
-          if (s.ty) { if (STATS) ++nt; tri_one(sc, r, s); }
+      // N: next node
+      if (active) {
+        if (!(s.gy & 0xFF000000u) && s.sp > 0) { const uint2 e = st.pop(--s.sp); s.gx = e.x; s.gy = e.y; }
+        if (s.gy & 0xFF000000u) {
+          const uint32_t node = trav_next_node(s, st, r);
+          const uint4* np = node < sc.smem_nodes ? smem + 5u * node : sc.nodes + 5u * (size_t)node;
+          w0 = np[0]; w1 = np[1]; w2 = np[2]; w3 = np[3]; w4 = np[4];
+          has_node = true;
         }
       }
-      if (active && !(s.gy & 0xFF000000u)) {  // node group exhausted: next one from the stack, or done
-        if (s.sp > 0) {
-          const uint2 e = st.pop(--s.sp);
-          s.gx = e.x; s.gy = e.y;
-        } else if (!s.ty && tsp == 0) {
+      // T: triangle tests
+#pragma unroll
+      for (int it = 0; it < kTrisPerStep; ++it) {
+        if (tri[it].li != kMiss) {
+          if (STATS) ++nt;
+          tri_test(tri[it].q0, tri[it].q1, tri[it].q2, tri[it].li, r);
+          tri[it].li = kMiss;
+        }
+        {
+          // The fourth words of q1 / q2 are not read by the test; keeping them "live" up to here stops the register
+          // allocator from reusing them while the 128-bit loads are in flight (a write-after-write wait on the load:
+          // profiles/r01c, 11 % of all warp-cycles before this line existed).
+          asm volatile("" ::"f"(tri[it].q1.w), "f"(tri[it].q2.w));
+        }
+      }
+      // F: next triangles
+      bool more = has_node;
+      if (active) {
+#pragma unroll
+        for (int it = 0; it < kTrisPerStep; ++it) {
+          tri_fetch(sc, s, tst, tsp, tri[it]);
+          more = more || tri[it].li != kMiss;
+        }
+        if (!more) {  // nothing requested, nothing pending: the ray is finished
           hits[ridx] = make_uint2(__float_as_uint(r.t), r.li);
           active = false;
         }

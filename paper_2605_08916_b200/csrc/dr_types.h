@@ -10,7 +10,10 @@ constexpr int kMaxPathLen = 16;        // L <= 16, d = 2L <= 32 (BASELINE.json c
 constexpr int kMaxPlanes = 8;          // d / 4 float4 planes
 constexpr int kMaxMix = 16;
 constexpr int kMaxLeafTris = 3;        // triangles per leaf (unary count in the child's meta byte)
-constexpr int kMaxSmemNodes = 585;     // 1 + 8 + 64 + 512: the top four BVH8 levels, staged in shared memory
+#ifndef DR_SMEM_NODES
+#define DR_SMEM_NODES 585
+#endif
+constexpr int kMaxSmemNodes = DR_SMEM_NODES;     // 1 + 8 + 64 + 512: the top four BVH8 levels, staged in shared memory
 constexpr int kMaxBvhDepth = 30;       // traversal stack entries per ray = depth + 1 (shared memory)
 
 // BVH8 node, 80 bytes = five 16-byte words.  Child boxes are quantised to 8 bits per plane on a per-node
