@@ -281,9 +281,11 @@ def main():
     stream_gbs = stream_bytes_per_mutation(desc.dim, grad) * n_local / (stream_ms * 1e-3) / 1e9
     launches_per_frame = sum(v["launches"] for v in prof.values()) / prof_frames
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "trace_traffic.json")
+    tp = os.path.join(ROOT, "profiles", "trace_traffic.txt")     # from the last ncu --set full capture of k_trace
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get("dram_bytes_per_launch")
+        for line in open(tp):
+            if line.startswith("dram_bytes_per_launch"):
+                traffic = int(line.split()[1])
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
