@@ -293,3 +293,68 @@ def test_sharded_chains_reproduce_the_unsharded_run(dr, torch_):
     assert parts[0][2] + parts[1][2] == full.stats()["tours"]
     summed = (parts[0][1] + parts[1][1]).cpu().numpy()
     assert np.allclose(summed, full.accum.cpu().numpy(), rtol=1e-4, atol=1e-7)
+
+
+# ---- BASELINE.json full sizes, in the launch configuration bench.py times ------------------------------------------------
+FULL = [("cornell", S.cornell, 65536, 2), ("caustic", S.caustic, 262144, 3), ("machines", S.machines, 589824, 4)]
+
+
+@pytest.mark.parametrize("case", FULL, ids=[c[0] for c in FULL])
+def test_full_size_configs(dr, oracle, torch_, case):
+    """configs[1..3] at their full chain counts: bit-exact RNG / queue / counters, and sampled states re-evaluated
+    one by one by the oracle (the stored (f/p_hat, p, pixel, score, signature) of a chain is the evaluation of its x)."""
+    name, make, N, seed = case
+    desc = make()
+    gsc, osc = dr.Scene(desc), oracle.Scene(desc, oracle.F32)
+    method = "diffusion_restore"
+    gch = dr.Chains(gsc, method, N, seed=seed)
+    gch.init(0)
+    rng = np.random.default_rng(7)
+    ids = np.unique(np.concatenate([rng.integers(0, N, 3000), [0, 1, 255, 256, N - 257, N - 1]]))
+    gs = gch.download()
+    # init states are the Philox uniforms of (chain, iteration 0, slot, REGEN_U, epoch 0): bit-exact
+    for i in ids[:200]:
+        for j in range(desc.dim // 4):
+            w = oracle.stream_block(seed, int(i), 0, j, 0, 0)
+            want = (w >> 8).astype(np.float64) * 2.0 ** -24
+            assert (gs["x"][i, 4 * j:4 * j + 4].astype(np.float64) == want).all()
+
+    def check_sample(gs):
+        e = osc.eval(np.ascontiguousarray(gs["x"][ids]), True)
+        assert (gs["pix"][ids] == e["pix"]).all()                                # splat pixel indices: bit-exact
+        ok = gs["sig"][ids] == e["sig"]
+        # Whole-path signatures (up to 16 hit triangles and lobes each): a path that grazes a triangle edge within
+        # fp32 rounding continues from the neighbour on one side.  Counted; bound 1e-3 per path, 5e-3 for the
+        # machines scene (14 segments per path over 0.01-0.2 wide facets, specular chains; DESIGN.md Q15).
+        assert (~ok).mean() < (5e-3 if name == "machines" else 1e-3), (~ok).sum()
+        p, fop = gs["p"][ids][ok].astype(np.float64), gs["fop"][ids][ok].astype(np.float64)
+        assert (np.abs(p - e["p"][ok]) <= 1e-4 * np.maximum(e["p"][ok], 1e-8)).all()
+        want = e["f"][ok] / (e["p"][ok][:, None] + 1e-8)
+        assert (np.abs(fop - want) <= 1e-4 * np.maximum(np.abs(want), 1e-8)).all()
+        tol = 1e-4 * np.abs(e["g"][ok]) + 2e-4 / 5e-3
+        assert (np.abs(gs["g"][ids][ok] - e["g"][ok]) <= tol).all()
+
+    check_sample(gs)
+    kills = int(gs["killed"].sum())
+    for it in range(1, 3):
+        gch.step(1)
+        gs = gch.download()
+        st = gch.stats()
+        assert st["mutations"] == N * (it + 1) and st["iteration"] == it and st["nonfinite"] == 0
+        assert (gs["x"] >= 0).all() and (gs["x"] < 1).all()
+        q = gch.queue()
+        assert (q == np.flatnonzero(gs["killed"])).all()                        # regeneration queue: bit-exact, ascending
+        kills += len(q)
+        assert st["tours"] == kills and st["kills_last_step"] == len(q)
+        check_sample(gs)
+    if name != "machines":      # the oracle runs these two in full in seconds: whole-ensemble teacher-forced step
+        och = oracle.Chains(osc, method, N, seed=seed)
+        och.init(0)
+        och.step(2)
+        gch.upload(och.state(), 2)
+        gch.step(1)
+        och.step(1)
+        div, rep = compare_states(gch.download(), och.state(), gch.last_step(), och.last(), float(gch.cfg.stddev))
+        assert div.mean() < 1e-3, rep
+        if not div.any():
+            assert (gch.queue() == och.queue()).all()
