@@ -141,8 +141,10 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   const uint32_t n = *cnt;
   if (n == 0) return;
   for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 5u; k += kTraceBlock) smem[k] = sc.nodes[k];
+  if (threadIdx.x == 0) smem[5u * sc.smem_nodes].x = 0x3F800000u;   // one 16-byte word between the nodes and the stacks
   __syncthreads();
-  SmemStack st{reinterpret_cast<uint2*>(smem + 5u * sc.smem_nodes) + threadIdx.x};
+  const uint32_t one = *(volatile uint32_t*)&smem[5u * sc.smem_nodes].x;  // bits of 1.0f in a register the compiler cannot fold (dr_traverse.cuh qmagic)
+  SmemStack st{reinterpret_cast<uint2*>(smem + 5u * sc.smem_nodes + 1u) + threadIdx.x};
   SmemStack tst{st.base + (size_t)sc.stack_cap * kTraceBlock};
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr unsigned kFull = 0xFFFFFFFFu;
@@ -154,7 +156,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   TriSlot tri[kTrisPerStep];
   int tsp = 0;  // postponed triangle groups
   uint32_t ridx = 0, nn = 0, nt = 0;
-  trav_setup(r, 0.f, 0.f, 0.f, 1.f, 1.f, 1.f);
+  trav_setup(r, 0.f, 0.f, 0.f, 1.f, 1.f, 1.f, one);
   trav_begin(s);
   w0 = w1 = w2 = w3 = w4 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
@@ -176,7 +178,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
       if (mine) {
         ridx = wnext + rank;
         const float4 o = q[ridx], d = q[(size_t)cap + ridx];
-        trav_setup(r, o.x, o.y, o.z, d.x, d.y, d.z);
+        trav_setup(r, o.x, o.y, o.z, d.x, d.y, d.z, one);
         trav_begin(s);   // one work bit: the root, requested by part N of the first step
         tsp = 0;
         active = true;
