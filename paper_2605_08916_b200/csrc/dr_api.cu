@@ -314,7 +314,7 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   dev.n_nodes = (uint32_t)bvh.nodes.size();
   dev.smem_nodes = dev.n_nodes < (uint32_t)kMaxSmemNodes ? dev.n_nodes : (uint32_t)kMaxSmemNodes;
   dev.stack_cap = bvh.depth + 1;  // node groups: at most one per level
-  const size_t stack_bytes = (size_t)(dev.stack_cap + kTriStack) * sizeof(uint2) * kTraceBlock + 16;  // + the constant word of k_trace
+  const size_t stack_bytes = ((size_t)(dev.stack_cap + kTriStack) * sizeof(uint2) + (size_t)kTriStack * sizeof(uint32_t)) * kTraceBlock + 16;  // + the constant word of k_trace
   if (stack_bytes + (size_t)dev.smem_nodes * sizeof(NodeC) > kMaxDynSmem)
     dev.smem_nodes = (uint32_t)((kMaxDynSmem - stack_bytes) / sizeof(NodeC));
   s->trace_smem = (size_t)dev.smem_nodes * sizeof(NodeC) + stack_bytes;

@@ -32,6 +32,9 @@ struct Node2 {
 };
 
 constexpr int kBins = 32;
+#ifndef DR_SPLIT_BUDGET
+#define DR_SPLIT_BUDGET 1.0   // extra references per triangle the pre-splitting may create
+#endif
 
 struct Builder {
   const std::vector<Box>& tb;
@@ -106,6 +109,132 @@ struct Builder {
   }
 };
 
+// Reference splitting before the build ("early split clipping", restated from the published idea of Ernst and
+// Greiner 2007 / Karras and Aila 2013): a triangle whose bounding box is much larger than the triangle itself (long,
+// thin, rotated: the cylinder and gear meshes of configs[3]) is cut by axis-aligned planes into several references,
+// each with the tight box of its clipped piece.  All references of a triangle point at the same triangle, so the
+// closest hit is unchanged; only the boxes the traversal sees get tighter.  The worst references (largest box area in
+// excess of the piece's own projected area) are split first until the budget of extra references is used up.
+struct Ref {
+  Box box;
+  uint32_t tri;
+};
+
+struct Poly {
+  int n = 0;
+  double p[10][3];
+};
+
+void clip_poly(const Poly& in, int axis, double plane, bool keep_low, Poly& out) {
+  out.n = 0;
+  for (int i = 0; i < in.n; ++i) {
+    const double* a = in.p[i];
+    const double* b = in.p[(i + 1) % in.n];
+    const double da = keep_low ? plane - a[axis] : a[axis] - plane, db = keep_low ? plane - b[axis] : b[axis] - plane;
+    if (da >= 0.0 && out.n < 10) { for (int k = 0; k < 3; ++k) out.p[out.n][k] = a[k]; ++out.n; }
+    if ((da > 0.0 && db < 0.0) || (da < 0.0 && db > 0.0)) {
+      const double t = da / (da - db);
+      if (out.n < 10) {
+        for (int k = 0; k < 3; ++k) out.p[out.n][k] = a[k] + t * (b[k] - a[k]);
+        out.p[out.n][axis] = plane;
+        ++out.n;
+      }
+    }
+  }
+}
+
+Box poly_box(const Poly& q) {
+  Box b;
+  for (int i = 0; i < q.n; ++i) {
+    const float f[3] = {(float)q.p[i][0], (float)q.p[i][1], (float)q.p[i][2]};
+    // round outwards: the float box must contain the double-precision piece
+    float lo[3], hi[3];
+    for (int k = 0; k < 3; ++k) {
+      lo[k] = (double)f[k] > q.p[i][k] ? std::nextafter(f[k], -FLT_MAX) : f[k];
+      hi[k] = (double)f[k] < q.p[i][k] ? std::nextafter(f[k], FLT_MAX) : f[k];
+    }
+    b.grow(lo);
+    b.grow(hi);
+  }
+  return b;
+}
+
+double poly_ideal_area(const Poly& q) {  // surface area of the tightest possible box of a flat piece: 2 * sum of projections
+  double n[3] = {0, 0, 0};
+  for (int i = 1; i + 1 < q.n; ++i) {
+    const double u[3] = {q.p[i][0] - q.p[0][0], q.p[i][1] - q.p[0][1], q.p[i][2] - q.p[0][2]};
+    const double v[3] = {q.p[i + 1][0] - q.p[0][0], q.p[i + 1][1] - q.p[0][1], q.p[i + 1][2] - q.p[0][2]};
+    n[0] += u[1] * v[2] - u[2] * v[1]; n[1] += u[2] * v[0] - u[0] * v[2]; n[2] += u[0] * v[1] - u[1] * v[0];
+  }
+  return std::fabs(n[0]) + std::fabs(n[1]) + std::fabs(n[2]);  // 2 * (1/2) * |n| components
+}
+
+void presplit(const float* verts, const uint32_t* idx, uint32_t nt, double budget_factor, std::vector<Ref>& refs) {
+  struct Piece { Poly poly; Box box; uint32_t tri; };
+  typedef std::pair<double, uint32_t> Key;  // (excess area, piece index): worst first
+  std::priority_queue<Key> pq;
+  std::vector<Piece> pool;
+  refs.clear();
+  refs.reserve((size_t)(nt * (1.0 + budget_factor)) + 8);
+  std::vector<double> excess(nt);
+  double total_area = 0.0;
+  Poly tp;
+  tp.n = 3;
+  auto load = [&](uint32_t t, Box& box) {
+    box = Box();
+    for (int k = 0; k < 3; ++k) {
+      for (int a = 0; a < 3; ++a) tp.p[k][a] = verts[3 * idx[3 * t + k] + a];
+      box.grow(&verts[3 * idx[3 * t + k]]);
+    }
+  };
+  for (uint32_t t = 0; t < nt; ++t) {
+    Box box;
+    load(t, box);
+    const double ideal = poly_ideal_area(tp);
+    excess[t] = (double)box.area() - ideal;
+    total_area += ideal;
+  }
+  // pieces whose excess is below a share of the mean triangle area are never worth a split
+  const double floor_excess = 0.5 * total_area / std::max(1u, nt);
+  long budget = (long)(budget_factor * nt);
+  for (uint32_t t = 0; t < nt; ++t) {
+    Box box;
+    load(t, box);
+    if (budget > 0 && excess[t] > floor_excess) {
+      pq.push(Key(excess[t], (uint32_t)pool.size()));
+      pool.push_back({tp, box, t});
+    } else {
+      refs.push_back({box, t});
+    }
+  }
+  while (!pq.empty()) {
+    const Key key = pq.top();
+    pq.pop();
+    const Piece it = pool[key.second];
+    if (budget <= 0 || key.first <= floor_excess) { refs.push_back({it.box, it.tri}); continue; }
+    int axis = 0;
+    float ext = -1.f;
+    for (int a = 0; a < 3; ++a) if (it.box.hi[a] - it.box.lo[a] > ext) { ext = it.box.hi[a] - it.box.lo[a]; axis = a; }
+    const double plane = 0.5 * ((double)it.box.lo[axis] + (double)it.box.hi[axis]);
+    Piece lo, hi;
+    clip_poly(it.poly, axis, plane, true, lo.poly);
+    clip_poly(it.poly, axis, plane, false, hi.poly);
+    if (lo.poly.n < 3 || hi.poly.n < 3) { refs.push_back({it.box, it.tri}); continue; }
+    lo.tri = hi.tri = it.tri;
+    lo.box = poly_box(lo.poly);
+    hi.box = poly_box(hi.poly);
+    for (int a = 0; a < 3; ++a) {  // pieces never leave the parent's box
+      lo.box.lo[a] = std::max(lo.box.lo[a], it.box.lo[a]); lo.box.hi[a] = std::min(lo.box.hi[a], it.box.hi[a]);
+      hi.box.lo[a] = std::max(hi.box.lo[a], it.box.lo[a]); hi.box.hi[a] = std::min(hi.box.hi[a], it.box.hi[a]);
+    }
+    --budget;
+    pool[key.second] = lo;  // reuse the parent's entry
+    pq.push(Key((double)lo.box.area() - poly_ideal_area(lo.poly), key.second));
+    pq.push(Key((double)hi.box.area() - poly_ideal_area(hi.poly), (uint32_t)pool.size()));
+    pool.push_back(hi);
+  }
+}
+
 // Places up to eight children in the octant slots: child c goes to the free slot s that maximises
 // dot(centre(c) - centre(node), corner(s)), greedily over all (child, slot) pairs.
 void assign_slots(const std::vector<Node2>& n2, const uint32_t* kids, int nk, int* slot_of) {
@@ -136,13 +265,19 @@ void assign_slots(const std::vector<Node2>& n2, const uint32_t* kids, int nk, in
 
 }  // namespace
 
+static double g_split_budget = DR_SPLIT_BUDGET;
+void set_split_budget(double extra_refs_per_triangle) { g_split_budget = extra_refs_per_triangle; }
+
 void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t nt, const uint32_t* tri_mat, BuiltBvh& out) {
   (void)nv;
-  std::vector<Box> tb(nt);
-  std::vector<float> cen(3 * (size_t)nt);
+  std::vector<Ref> refs;
+  presplit(verts, idx, nt, g_split_budget, refs);
+  const uint32_t nr = (uint32_t)refs.size();
+  std::vector<Box> tb(nr);
+  std::vector<float> cen(3 * (size_t)nr);
   Box scene;
-  for (uint32_t t = 0; t < nt; ++t) {
-    for (int k = 0; k < 3; ++k) tb[t].grow(&verts[3 * idx[3 * t + k]]);
+  for (uint32_t t = 0; t < nr; ++t) {
+    tb[t] = refs[t].box;
     for (int a = 0; a < 3; ++a) cen[3 * t + a] = 0.5f * (tb[t].lo[a] + tb[t].hi[a]);
     scene.grow(tb[t]);
   }
@@ -168,7 +303,7 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
     return;
   }
   Builder b(tb, cen);
-  b.build(0, nt);
+  b.build(0, nr);
   const std::vector<Node2>& n2 = b.nodes;
 
   auto emit_tri = [&](uint32_t id) {
@@ -180,7 +315,7 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
     tp.id = id; tp.mat = tri_mat[id]; tp.pad = 0;
     out.tris.push_back(tp);
   };
-  out.tris.reserve(nt);
+  out.tris.reserve(nr);
 
   // collapse to BVH8, breadth-first; a node's index is its position in the queue order
   struct Item { uint32_t n2; uint32_t depth; };
@@ -255,12 +390,10 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
       if (kid_in_slot[s] < 0) continue;
       const Node2& c = n2[kids[kid_in_slot[s]]];
       if (c.count) {
-        const uint32_t off = (uint32_t)out.tris.size() - node.tri_base;
-        node.meta[s] = (uint8_t)((((1u << c.count) - 1u) << 5) | off);
-        for (uint32_t k = 0; k < c.count; ++k) emit_tri(b.order[c.first + k]);
+        node.trimask |= ((1u << c.count) - 1u) << (3 * s);
+        for (uint32_t k = 0; k < c.count; ++k) emit_tri(refs[b.order[c.first + k]].tri);
         sah += (double)c.box.area() / root_area * c.count;
       } else {
-        node.meta[s] = (uint8_t)((1u << 5) | (24u + (uint32_t)s));
         node.imask |= (uint8_t)(1u << s);
         ++next_index;
         q.push({kids[kid_in_slot[s]], it.depth + 1});

@@ -95,16 +95,21 @@ __global__ void __launch_bounds__(kShadeBlock) k_raygen(DevScene sc, EvalWs ws, 
 
 // ---- a4: closest hit, persistent ---------------------------------------------------------------------------------
 // Per-thread stacks in shared memory, entry e of thread t at base[e * kTraceBlock] (bank = lane: conflict-free).
-// Node groups grow up from entry 0; postponed triangle groups live in their own kTriStack entries above them.
+// Node groups grow up from entry 0; postponed triangle groups (tx, ty | tm) live in their own kTriStack entries above them.
 struct SmemStack {
   uint2* base;
   __device__ __forceinline__ void push(int sp, uint2 v) { base[sp * kTraceBlock] = v; }
   __device__ __forceinline__ uint2 pop(int sp) const { return base[sp * kTraceBlock]; }
 };
+struct SmemTriStack {
+  uint2* base;     // (tx, ty)
+  uint32_t* base3; // tm
+  __device__ __forceinline__ void push(int sp, const TravState& s) { base[sp * kTraceBlock] = make_uint2(s.tx, s.ty); base3[sp * kTraceBlock] = s.tm; }
+  __device__ __forceinline__ void pop(int sp, TravState& s) const { const uint2 e = base[sp * kTraceBlock]; s.tx = e.x; s.ty = e.y; s.tm = base3[sp * kTraceBlock]; }
+};
 
 __device__ __forceinline__ void tri_one(const DevScene& sc, TravRay& r, TravState& s) {
-  const uint32_t li = s.tx + low_bit(s.ty);
-  s.ty &= s.ty - 1u;
+  const uint32_t li = trav_next_tri(s);
   tri_test(__ldg(&sc.tris[3 * li]), __ldg(&sc.tris[3 * li + 1]), __ldg(&sc.tris[3 * li + 2]), li, r);
 }
 
@@ -114,11 +119,10 @@ struct TriSlot {
   uint32_t li;  // leaf-order index, kMiss = empty
 };
 
-__device__ __forceinline__ void tri_fetch(const DevScene& sc, TravState& s, SmemStack& tst, int& tsp, TriSlot& t) {
-  if (!s.ty && tsp > 0) { const uint2 e = tst.pop(--tsp); s.tx = e.x; s.ty = e.y; }
+__device__ __forceinline__ void tri_fetch(const DevScene& sc, TravState& s, SmemTriStack& tst, int& tsp, TriSlot& t) {
+  if (!s.ty && tsp > 0) tst.pop(--tsp, s);
   if (s.ty) {
-    t.li = s.tx + low_bit(s.ty);
-    s.ty &= s.ty - 1u;
+    t.li = trav_next_tri(s);
     const float4* p = sc.tris + 3 * (size_t)t.li;
     t.q0 = __ldg(p); t.q1 = __ldg(p + 1); t.q2 = __ldg(p + 2);
   }
@@ -145,7 +149,8 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   __syncthreads();
   const uint32_t one = *(volatile uint32_t*)&smem[5u * sc.smem_nodes].x;  // bits of 1.0f in a register the compiler cannot fold (dr_traverse.cuh qmagic)
   SmemStack st{reinterpret_cast<uint2*>(smem + 5u * sc.smem_nodes + 1u) + threadIdx.x};
-  SmemStack tst{st.base + (size_t)sc.stack_cap * kTraceBlock};
+  SmemTriStack tst{st.base + (size_t)sc.stack_cap * kTraceBlock, nullptr};
+  tst.base3 = reinterpret_cast<uint32_t*>(tst.base + (size_t)kTriStack * kTraceBlock - threadIdx.x) + threadIdx.x;
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr unsigned kFull = 0xFFFFFFFFu;
   uint32_t wnext = 0, wend = 0;  // this warp's private range of the queue
@@ -198,11 +203,12 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
         const uint32_t nty = h & 0x00FFFFFFu;
         if (nty) {
           if (s.ty) {  // triangles still pending from an earlier node: postpone them (or test them now if full)
-            if (tsp < kTriStack) tst.push(tsp++, make_uint2(s.tx, s.ty));
+            if (tsp < kTriStack) tst.push(tsp++, s);
             else while (s.ty) { if (STATS) ++nt; tri_one(sc, r, s); }
           }
           s.tx = w1.y;
           s.ty = nty;
+          s.tm = w1.z;
         }
         s.gx = w1.x;
         s.gy = (h & 0xFF000000u) | (w0.w >> 24);

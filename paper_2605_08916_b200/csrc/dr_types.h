@@ -9,7 +9,7 @@ namespace dr {
 constexpr int kMaxPathLen = 16;        // L <= 16, d = 2L <= 32 (BASELINE.json configs[3])
 constexpr int kMaxPlanes = 8;          // d / 4 float4 planes
 constexpr int kMaxMix = 16;
-constexpr int kMaxLeafTris = 3;        // triangles per leaf (unary count in the child's meta byte)
+constexpr int kMaxLeafTris = 3;        // triangles per leaf (three bits per slot in the node's triangle mask)
 #ifndef DR_SMEM_NODES
 #define DR_SMEM_NODES 585
 #endif
@@ -19,12 +19,14 @@ constexpr int kMaxBvhDepth = 30;       // traversal stack entries per ray = dept
 // BVH8 node, 80 bytes = five 16-byte words.  Child boxes are quantised to 8 bits per plane on a per-node
 // grid (origin p, per-axis power-of-two cell 2^(e-127)), rounded outwards, so a node costs five 128-bit loads.
 //   w0 = (p.x, p.y, p.z, e_x | e_y << 8 | e_z << 16 | imask << 24)      imask: bit s = slot s is an internal node
-//   w1 = (child_base, tri_base, meta[0..3], meta[4..7])
+//   w1 = (child_base, tri_base, trimask, 0)
 //   w2 = (qlo_x[0..3], qlo_x[4..7], qlo_y[0..3], qlo_y[4..7])
 //   w3 = (qlo_z[0..3], qlo_z[4..7], qhi_x[0..3], qhi_x[4..7])
 //   w4 = (qhi_y[0..3], qhi_y[4..7], qhi_z[0..3], qhi_z[4..7])
-// meta[s]: 0 = empty slot; internal child: 0b001_11sss (one work bit at position 24 + s);
-//          leaf with n <= 3 triangles at tri_base + off (off <= 23): ((1 << n) - 1) << 5 | off.
+// trimask: bit 3 s + k is set iff slot s is a leaf with more than k triangles (k < 3).  The triangles of a node are
+// stored contiguously from tri_base in the order of their bits: the triangle of bit b is
+// tri_base + popcount(trimask & ((1 << b) - 1)).  Fixed bit positions let the node test build its work mask with one
+// select per child (dr_traverse.cuh node_hits); an empty slot has inverted boxes and no bit in either mask.
 // Internal children of a node are stored contiguously from child_base in slot order: the child in slot s is
 // node child_base + popcount(imask & ((1 << s) - 1)).  Slots are assigned so that children lie towards corner
 // (s&4 ? +x : -x, s&2 ? +y : -y, s&1 ? +z : -z) of the node: visiting slots in the order of descending
@@ -34,7 +36,7 @@ struct alignas(16) NodeC {
   uint8_t e[3];
   uint8_t imask;
   uint32_t child_base, tri_base;
-  uint8_t meta[8];
+  uint32_t trimask, pad;
   uint8_t qlo[3][8];
   uint8_t qhi[3][8];
 };
@@ -66,6 +68,7 @@ struct BuiltBvh {
 };
 
 // Binned-SAH BVH2 -> BVH8 collapse -> slot assignment -> quantisation (host).  verts: 3*nv floats, idx: 3*nt, tri_mat: nt.
+void set_split_budget(double extra_refs_per_triangle);  // tuning hook (default DR_SPLIT_BUDGET)
 void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t nt, const uint32_t* tri_mat, BuiltBvh& out);
 
 }  // namespace dr
