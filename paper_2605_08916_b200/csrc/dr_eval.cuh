@@ -22,7 +22,7 @@ namespace dr {
 #define DR_TRI_STACK 12
 #endif
 #ifndef DR_TRIS_PER_STEP
-#define DR_TRIS_PER_STEP 2
+#define DR_TRIS_PER_STEP 1
 #endif
 #ifndef DR_REFILL_BELOW
 #define DR_REFILL_BELOW 30
@@ -196,61 +196,76 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
     if (!act) break;
     // ---- lockstep traversal
     do {
+      // The four parts are written without branches (selects and predicated loads / stores) so that the compiler can
+      // interleave their dependency chains: with branches around every part each warp waited out the fixed latencies
+      // of its bookkeeping one after the other (profiles/r01d: 53 % of the instructions took 78 % of the time).
       // A: node test
-      if (has_node) {
-        if (STATS) ++nn;
-        const uint32_t h = node_hits(w0, w1, w2, w3, w4, r);
+      {
+        if (STATS) nn += has_node ? 1u : 0u;
+        uint32_t h = node_hits(w0, w1, w2, w3, w4, r);
+        h = has_node ? h : 0u;
         const uint32_t nty = h & 0x00FFFFFFu;
-        if (nty) {
-          if (s.ty) {  // triangles still pending from an earlier node: postpone them (or test them now if full)
-            if (tsp < kTriStack) tst.push(tsp++, s);
-            else while (s.ty) { if (STATS) ++nt; tri_one(sc, r, s); }
-          }
-          s.tx = w1.y;
-          s.ty = nty;
-          s.tm = w1.z;
+        const bool newtri = nty != 0u;
+        bool keep_old = newtri && s.ty != 0u;  // triangles still pending from an earlier node: postpone them
+        if (keep_old && tsp >= kTriStack) {    // (or test them now if their stack is full: rare)
+          while (s.ty) { if (STATS) ++nt; tri_one(sc, r, s); }
+          keep_old = false;
         }
-        s.gx = w1.x;
-        s.gy = (h & 0xFF000000u) | (w0.w >> 24);
-        has_node = false;
+        if (keep_old) tst.push(tsp, s);
+        tsp += keep_old ? 1 : 0;
+        s.tx = newtri ? w1.y : s.tx;
+        s.ty = newtri ? nty : s.ty;
+        s.tm = newtri ? w1.z : s.tm;
+        s.gx = has_node ? w1.x : s.gx;
+        s.gy = has_node ? ((h & 0xFF000000u) | (w0.w >> 24)) : s.gy;
       }
       // N: next node
-      if (active) {
-        if (!(s.gy & 0xFF000000u) && s.sp > 0) { const uint2 e = st.pop(--s.sp); s.gx = e.x; s.gy = e.y; }
-        if (s.gy & 0xFF000000u) {
-          const uint32_t node = trav_next_node(s, st, r);
+      {
+        const bool popn = active && !(s.gy & 0xFF000000u) && s.sp > 0;
+        s.sp -= popn ? 1 : 0;
+        if (popn) { const uint2 e = st.pop(s.sp); s.gx = e.x; s.gy = e.y; }
+        const bool go = active && (s.gy & 0xFF000000u) != 0u;
+        const uint32_t bit = top_bit(s.gy | 0x01000000u);
+        const uint32_t rest = s.gy & ~(1u << bit);
+        const bool keep = go && (rest & 0xFF000000u) != 0u;
+        if (keep) st.push(s.sp, make_uint2(s.gx, rest));
+        s.sp += keep ? 1 : 0;
+        const uint32_t slot = (bit - 24u) ^ (r.octinv4 & 7u);
+        const uint32_t node = s.gx + popc32(rest & ~(0xFFFFFFFFu << slot) & 0xFFu);
+        s.gy = go ? rest : s.gy;
+        if (go) {
           const uint4* np = node < sc.smem_nodes ? smem + 5u * node : sc.nodes + 5u * (size_t)node;
           w0 = np[0]; w1 = np[1]; w2 = np[2]; w3 = np[3]; w4 = np[4];
-          has_node = true;
         }
+        has_node = go;
       }
-      // T: triangle tests
-#pragma unroll
-      for (int it = 0; it < kTrisPerStep; ++it) {
-        if (tri[it].li != kMiss) {
-          if (STATS) ++nt;
-          tri_test(tri[it].q0, tri[it].q1, tri[it].q2, tri[it].li, r);
-          tri[it].li = kMiss;
-        }
-        {
-          // The fourth words of q1 / q2 are not read by the test; keeping them "live" up to here stops the register
-          // allocator from reusing them while the 128-bit loads are in flight (a write-after-write wait on the load:
-          // profiles/r01c, 11 % of all warp-cycles before this line existed).
-          asm volatile("" ::"f"(tri[it].q1.w), "f"(tri[it].q2.w));
-        }
+      // T: triangle test
+      static_assert(kTrisPerStep == 1, "the branch-free step tests one triangle");
+      {
+        const bool valid = tri[0].li != kMiss;
+        if (STATS) nt += valid ? 1u : 0u;
+        tri_test_bf(tri[0].q0, tri[0].q1, tri[0].q2, tri[0].li, valid, r);
+        // The fourth words of q1 / q2 are not read by the test; keeping them "live" up to here stops the register
+        // allocator from reusing them while the 128-bit loads are in flight (a write-after-write wait on the load).
+        asm volatile("" ::"f"(tri[0].q1.w), "f"(tri[0].q2.w));
       }
-      // F: next triangles
-      bool more = has_node;
-      if (active) {
-#pragma unroll
-        for (int it = 0; it < kTrisPerStep; ++it) {
-          tri_fetch(sc, s, tst, tsp, tri[it]);
-          more = more || tri[it].li != kMiss;
+      // F: next triangle
+      {
+        const bool popt = active && s.ty == 0u && tsp > 0;
+        tsp -= popt ? 1 : 0;
+        if (popt) tst.pop(tsp, s);
+        const bool have = active && s.ty != 0u;
+        const uint32_t b = low_bit(s.ty | 0x80000000u);
+        const uint32_t li = s.tx + popc32(s.tm & ~(0xFFFFFFFFu << b));
+        s.ty = have ? (s.ty & (s.ty - 1u)) : s.ty;
+        tri[0].li = have ? li : kMiss;
+        if (have) {
+          const float4* p = sc.tris + 3 * (size_t)li;
+          tri[0].q0 = __ldg(p); tri[0].q1 = __ldg(p + 1); tri[0].q2 = __ldg(p + 2);
         }
-        if (!more) {  // nothing requested, nothing pending: the ray is finished
-          hits[ridx] = make_uint2(__float_as_uint(r.t), r.li);
-          active = false;
-        }
+        const bool done = active && !(has_node || have);  // nothing requested, nothing pending: the ray is finished
+        if (done) hits[ridx] = make_uint2(__float_as_uint(r.t), r.li);
+        active = active && !done;
       }
       act = __ballot_sync(kFull, active);
     } while (drained ? act != 0u : __popc(act) >= kRefillBelow);
