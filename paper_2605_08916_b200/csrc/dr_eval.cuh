@@ -110,12 +110,13 @@ struct SmemTriStack {
 
 __device__ __forceinline__ void tri_one(const DevScene& sc, TravRay& r, TravState& s) {
   const uint32_t li = trav_next_tri(s);
-  tri_test(__ldg(&sc.tris[3 * li]), __ldg(&sc.tris[3 * li + 1]), __ldg(&sc.tris[3 * li + 2]), li, r);
+  tri_test(__ldg(&sc.tris[3 * li]), __ldg(&sc.tris[3 * li + 1]), __ldg(reinterpret_cast<const float2*>(&sc.tris[3 * li + 2])), li, r);
 }
 
 // One prefetched triangle of a lane: its three words are requested one step before they are tested.
 struct TriSlot {
-  float4 q0, q1, q2;
+  float4 t0, t1;
+  float2 t2;
   uint32_t li;  // leaf-order index, kMiss = empty
 };
 
@@ -124,7 +125,7 @@ __device__ __forceinline__ void tri_fetch(const DevScene& sc, TravState& s, Smem
   if (s.ty) {
     t.li = trav_next_tri(s);
     const float4* p = sc.tris + 3 * (size_t)t.li;
-    t.q0 = __ldg(p); t.q1 = __ldg(p + 1); t.q2 = __ldg(p + 2);
+    t.t0 = __ldg(p); t.t1 = __ldg(p + 1); t.t2 = __ldg(reinterpret_cast<const float2*>(p + 2));
   }
 }
 
@@ -165,7 +166,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   trav_begin(s);
   w0 = w1 = w2 = w3 = w4 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
-  for (int it = 0; it < kTrisPerStep; ++it) { tri[it].li = kMiss; tri[it].q0 = tri[it].q1 = tri[it].q2 = make_float4(0.f, 0.f, 0.f, 0.f); }
+  for (int it = 0; it < kTrisPerStep; ++it) { tri[it].li = kMiss; tri[it].t0 = tri[it].t1 = make_float4(0.f, 0.f, 0.f, 0.f); tri[it].t2 = make_float2(0.f, 0.f); }
   for (;;) {
     // ---- hand rays to the idle lanes
     unsigned want = __ballot_sync(kFull, !active);
@@ -244,10 +245,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
       {
         const bool valid = tri[0].li != kMiss;
         if (STATS) nt += valid ? 1u : 0u;
-        tri_test_bf(tri[0].q0, tri[0].q1, tri[0].q2, tri[0].li, valid, r);
-        // The fourth words of q1 / q2 are not read by the test; keeping them "live" up to here stops the register
-        // allocator from reusing them while the 128-bit loads are in flight (a write-after-write wait on the load).
-        asm volatile("" ::"f"(tri[0].q1.w), "f"(tri[0].q2.w));
+        tri_test_bf(tri[0].t0, tri[0].t1, tri[0].t2, tri[0].li, valid, r);  // reads every loaded word (dr_types.h TriPacked)
       }
       // F: next triangle
       {
@@ -261,7 +259,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
         tri[0].li = have ? li : kMiss;
         if (have) {
           const float4* p = sc.tris + 3 * (size_t)li;
-          tri[0].q0 = __ldg(p); tri[0].q1 = __ldg(p + 1); tri[0].q2 = __ldg(p + 2);
+          tri[0].t0 = __ldg(p); tri[0].t1 = __ldg(p + 1); tri[0].t2 = __ldg(reinterpret_cast<const float2*>(p + 2));
         }
         const bool done = active && !(has_node || have);  // nothing requested, nothing pending: the ray is finished
         if (done) hits[ridx] = make_uint2(__float_as_uint(r.t), r.li);
@@ -305,14 +303,15 @@ __global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, E
       f0 = T0 * sc.env[0]; f1 = T1 * sc.env[1]; f2 = T2 * sc.env[2];
     } else {
       const uint32_t li = h.y;
-      const float4 q0 = __ldg(&sc.tris[3 * li]), q1 = __ldg(&sc.tris[3 * li + 1]), q2 = __ldg(&sc.tris[3 * li + 2]);
-      sig = fnv(sig, __float_as_uint(q0.w) + 1u);
-      const uint32_t mi = __float_as_uint(q1.w);
+      const float4 t0 = __ldg(&sc.tris[3 * li]), t1 = __ldg(&sc.tris[3 * li + 1]), t2 = __ldg(&sc.tris[3 * li + 2]);
+      const float3 e1 = make_float3(t0.w, t1.x, t1.y), e2 = make_float3(t1.z, t1.w, t2.x);  // dr_types.h TriPacked
+      sig = fnv(sig, __float_as_uint(t2.y) + 1u);
+      const uint32_t mi = __float_as_uint(t2.z);
       const float4 m0 = __ldg(&sc.mats[3 * mi]), m1 = __ldg(&sc.mats[3 * mi + 1]);
       const uint32_t kind = __float_as_uint(m0.x);
       Frame fr;
       float dn;
-      tri_frame(xyz(q1), xyz(q2), d, fr, dn);
+      tri_frame(e1, e2, d, fr, dn);
       if (kind == 3u) {  // emitter: front face emits, path stops
         if (dn < 0.f) {
           sig = fnv(sig, 4u);
@@ -424,13 +423,14 @@ __global__ void __launch_bounds__(kGradBlock) k_grad(DevScene sc, EvalWs ws, Eva
     const float4 rc = ws.rec[(size_t)k * cap + s];
     const uint32_t li = __float_as_uint(rc.w);
     const float3 din = xyz(rc);
-    const float4 q1 = __ldg(&sc.tris[3 * li + 1]), q2 = __ldg(&sc.tris[3 * li + 2]);
-    const uint32_t mi = __float_as_uint(q1.w);
+    const float4 t0 = __ldg(&sc.tris[3 * li]), t1 = __ldg(&sc.tris[3 * li + 1]), t2 = __ldg(&sc.tris[3 * li + 2]);
+    const float3 e1 = make_float3(t0.w, t1.x, t1.y), e2 = make_float3(t1.z, t1.w, t2.x);
+    const uint32_t mi = __float_as_uint(t2.z);
     const float4 m0 = __ldg(&sc.mats[3 * mi]), m1 = __ldg(&sc.mats[3 * mi + 1]);
     const uint32_t kind = __float_as_uint(m0.x);
     Frame fr;
     float dn;
-    tri_frame(xyz(q1), xyz(q2), din, fr, dn);
+    tri_frame(e1, e2, din, fr, dn);
     const float2 u = x_pair(io, s, k);
     const bool live = db0 != 0.f || db1 != 0.f || db2 != 0.f;
     if (kind == 0u) {

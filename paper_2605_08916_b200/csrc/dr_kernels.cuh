@@ -323,7 +323,7 @@ __global__ void k_unpack_hits(DevScene sc, const uint2* hits, uint32_t n, float*
   if (i >= n) return;
   const uint2 h = hits[i];
   if (h.y == kMiss) { t[i] = -1.f; prim[i] = 0xFFFFFFFFu; }
-  else { t[i] = __uint_as_float(h.x); prim[i] = __float_as_uint(sc.tris[3 * h.y].w); }
+  else { t[i] = __uint_as_float(h.x); prim[i] = __float_as_uint(sc.tris[3 * h.y + 2].y); }
 }
 
 __global__ void k_philox_blocks(uint64_t seed, const uint32_t* ctr, uint32_t n, uint32_t* out) {

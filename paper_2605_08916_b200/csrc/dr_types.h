@@ -42,12 +42,16 @@ struct alignas(16) NodeC {
 };
 static_assert(sizeof(NodeC) == 80, "NodeC must be 80 bytes");
 
-// Triangle in leaf order, 48 bytes: three float4.
-//   q0 = (v0.xyz, bits(original triangle id)), q1 = (e1.xyz, bits(material id)), q2 = (e2.xyz, 0)
+// Triangle in leaf order, 48 bytes = three 16-byte words:
+//   t0 = (v0.x, v0.y, v0.z, e1.x), t1 = (e1.y, e1.z, e2.x, e2.y), t2 = (e2.z, bits(original id), bits(material id), 0)
+// The traversal loads t0, t1 and the first half of t2 (40 bytes), so that every register a load writes is read by
+// the triangle test (a loaded-but-unread register is free for reuse while the load is still in flight, which made
+// the next write to it wait for the whole load: profiles/r01e).
 struct TriPacked {
-  float v0[3]; uint32_t id;
-  float e1[3]; uint32_t mat;
-  float e2[3]; uint32_t pad;
+  float v0[3];
+  float e1[3];
+  float e2[3];
+  uint32_t id, mat, pad;
 };
 static_assert(sizeof(TriPacked) == 48, "TriPacked must be 48 bytes");
 
