@@ -1,4 +1,5 @@
 // C-ABI entry points (include/dr.h): argument validation, scene upload, state layout, kernel launches.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -312,7 +313,7 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   }
   dev.nodes = (const uint4*)s->d_nodes; dev.tris = (const float4*)s->d_tris; dev.mats = (const float4*)s->d_mats;
   dev.n_nodes = (uint32_t)bvh.nodes.size();
-  dev.smem_nodes = dev.n_nodes < (uint32_t)kMaxSmemNodes ? dev.n_nodes : (uint32_t)kMaxSmemNodes;
+  dev.smem_nodes = std::min<uint32_t>(dev.n_nodes, (uint32_t)kMaxSmemNodes);
   dev.stack_cap = bvh.depth + 1;  // node groups: at most one per level
   const size_t stack_bytes = ((size_t)(dev.stack_cap + kTriStack) * sizeof(uint2) + (size_t)kTriStack * sizeof(uint32_t)) * kTraceBlock + 16;  // + the constant word of k_trace
   if (stack_bytes + (size_t)dev.smem_nodes * sizeof(NodeC) > kMaxDynSmem)

@@ -19,7 +19,7 @@ namespace dr {
 #define DR_TRACE_BLOCK 640
 #endif
 #ifndef DR_TRI_STACK
-#define DR_TRI_STACK 12
+#define DR_TRI_STACK 8
 #endif
 #ifndef DR_TRIS_PER_STEP
 #define DR_TRIS_PER_STEP 1
@@ -27,12 +27,21 @@ namespace dr {
 #ifndef DR_REFILL_BELOW
 #define DR_REFILL_BELOW 30
 #endif
+#ifndef DR_NODE_LD
+#define DR_NODE_LD __ldg
+#endif
+#ifndef DR_TRI_LD
+#define DR_TRI_LD __ldg
+#endif
+#ifndef DR_FETCH_CHUNK
+#define DR_FETCH_CHUNK 16
+#endif
 constexpr int kTraceBlock = DR_TRACE_BLOCK;   // one persistent block per SM
 constexpr int kTriStack = DR_TRI_STACK;      // postponed triangle groups per ray
 constexpr int kTrisPerStep = DR_TRIS_PER_STEP;    // triangle tests per lockstep step
 constexpr int kShadeBlock = 256;
 constexpr int kGradBlock = 128;
-constexpr uint32_t kFetchChunk = 64;   // rays a warp takes from the queue per atomic
+constexpr uint32_t kFetchChunk = DR_FETCH_CHUNK;   // rays a warp takes from the queue per atomic
 constexpr int kRefillBelow = DR_REFILL_BELOW;       // a warp goes back to the queue when fewer lanes than this hold a ray
 constexpr uint32_t kSigInit = 2166136261u;
 constexpr uint32_t kMiss = 0xFFFFFFFFu;
@@ -235,8 +244,13 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
         const uint32_t node = s.gx + popc32(rest & ~(0xFFFFFFFFu << slot) & 0xFFu);
         s.gy = go ? rest : s.gy;
         if (go) {
+#if DR_SMEM_NODES == 0
+          const uint4* np = sc.nodes + 5u * (size_t)node;
+          w0 = DR_NODE_LD(np); w1 = DR_NODE_LD(np + 1); w2 = DR_NODE_LD(np + 2); w3 = DR_NODE_LD(np + 3); w4 = DR_NODE_LD(np + 4);
+#else
           const uint4* np = node < sc.smem_nodes ? smem + 5u * node : sc.nodes + 5u * (size_t)node;
           w0 = np[0]; w1 = np[1]; w2 = np[2]; w3 = np[3]; w4 = np[4];
+#endif
         }
         has_node = go;
       }
@@ -259,7 +273,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
         tri[0].li = have ? li : kMiss;
         if (have) {
           const float4* p = sc.tris + 3 * (size_t)li;
-          tri[0].t0 = __ldg(p); tri[0].t1 = __ldg(p + 1); tri[0].t2 = __ldg(reinterpret_cast<const float2*>(p + 2));
+          tri[0].t0 = DR_TRI_LD(p); tri[0].t1 = DR_TRI_LD(p + 1); tri[0].t2 = DR_TRI_LD(reinterpret_cast<const float2*>(p + 2));
         }
         const bool done = active && !(has_node || have);  // nothing requested, nothing pending: the ray is finished
         if (done) hits[ridx] = make_uint2(__float_as_uint(r.t), r.li);

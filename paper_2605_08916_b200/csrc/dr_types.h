@@ -11,9 +11,10 @@ constexpr int kMaxPlanes = 8;          // d / 4 float4 planes
 constexpr int kMaxMix = 16;
 constexpr int kMaxLeafTris = 3;        // triangles per leaf (three bits per slot in the node's triangle mask)
 #ifndef DR_SMEM_NODES
-#define DR_SMEM_NODES 585
+#define DR_SMEM_NODES 0
 #endif
-constexpr int kMaxSmemNodes = DR_SMEM_NODES;     // 1 + 8 + 64 + 512: the top four BVH8 levels, staged in shared memory
+constexpr int kMaxSmemNodes = DR_SMEM_NODES;     // top BVH8 levels staged in shared memory (585 = four levels).  0 (default): none --
+                                                 // the shared memory is worth more as L1 (sweep in DESIGN.md section 6)
 constexpr int kMaxBvhDepth = 30;       // traversal stack entries per ray = depth + 1 (shared memory)
 
 // BVH8 node, 80 bytes = five 16-byte words.  Child boxes are quantised to 8 bits per plane on a per-node
