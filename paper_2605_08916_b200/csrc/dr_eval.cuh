@@ -22,7 +22,7 @@ namespace dr {
 #define DR_TRI_STACK 8
 #endif
 #ifndef DR_TRIS_PER_STEP
-#define DR_TRIS_PER_STEP 1
+#define DR_TRIS_PER_STEP 2
 #endif
 #ifndef DR_REFILL_BELOW
 #define DR_REFILL_BELOW 30
@@ -254,28 +254,33 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
         }
         has_node = go;
       }
-      // T: triangle test
-      static_assert(kTrisPerStep == 1, "the branch-free step tests one triangle");
-      {
-        const bool valid = tri[0].li != kMiss;
+      // T: triangle tests
+#pragma unroll
+      for (int it = 0; it < kTrisPerStep; ++it) {
+        const bool valid = tri[it].li != kMiss;
         if (STATS) nt += valid ? 1u : 0u;
-        tri_test_bf(tri[0].t0, tri[0].t1, tri[0].t2, tri[0].li, valid, r);  // reads every loaded word (dr_types.h TriPacked)
+        tri_test_bf(tri[it].t0, tri[it].t1, tri[it].t2, tri[it].li, valid, r);  // reads every loaded word (dr_types.h TriPacked)
       }
-      // F: next triangle
+      // F: next triangles
       {
-        const bool popt = active && s.ty == 0u && tsp > 0;
-        tsp -= popt ? 1 : 0;
-        if (popt) tst.pop(tsp, s);
-        const bool have = active && s.ty != 0u;
-        const uint32_t b = low_bit(s.ty | 0x80000000u);
-        const uint32_t li = s.tx + popc32(s.tm & ~(0xFFFFFFFFu << b));
-        s.ty = have ? (s.ty & (s.ty - 1u)) : s.ty;
-        tri[0].li = have ? li : kMiss;
-        if (have) {
-          const float4* p = sc.tris + 3 * (size_t)li;
-          tri[0].t0 = DR_TRI_LD(p); tri[0].t1 = DR_TRI_LD(p + 1); tri[0].t2 = DR_TRI_LD(reinterpret_cast<const float2*>(p + 2));
+        bool have_any = false;
+#pragma unroll
+        for (int it = 0; it < kTrisPerStep; ++it) {
+          const bool popt = active && s.ty == 0u && tsp > 0;
+          tsp -= popt ? 1 : 0;
+          if (popt) tst.pop(tsp, s);
+          const bool have = active && s.ty != 0u;
+          const uint32_t b = low_bit(s.ty | 0x80000000u);
+          const uint32_t li = s.tx + popc32(s.tm & ~(0xFFFFFFFFu << b));
+          s.ty = have ? (s.ty & (s.ty - 1u)) : s.ty;
+          tri[it].li = have ? li : kMiss;
+          if (have) {
+            const float4* p = sc.tris + 3 * (size_t)li;
+            tri[it].t0 = DR_TRI_LD(p); tri[it].t1 = DR_TRI_LD(p + 1); tri[it].t2 = DR_TRI_LD(reinterpret_cast<const float2*>(p + 2));
+          }
+          have_any = have_any || have;
         }
-        const bool done = active && !(has_node || have);  // nothing requested, nothing pending: the ray is finished
+        const bool done = active && !(has_node || have_any);  // nothing requested, nothing pending: the ray is finished
         if (done) hits[ridx] = make_uint2(__float_as_uint(r.t), r.li);
         active = active && !done;
       }
