@@ -400,6 +400,7 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
         sah += (double)c.box.area() / root_area;
       }
     }
+    node.imask32 = node.imask;
     out.nodes.push_back(node);
   }
   out.sah_cost = (float)sah;

@@ -227,7 +227,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
         s.ty = newtri ? nty : s.ty;
         s.tm = newtri ? w1.z : s.tm;
         s.gx = has_node ? w1.x : s.gx;
-        s.gy = has_node ? ((h & 0xFF000000u) | (w0.w >> 24)) : s.gy;
+        s.gy = has_node ? ((h & 0xFF000000u) | w1.w) : s.gy;
       }
       // N: next node
       {

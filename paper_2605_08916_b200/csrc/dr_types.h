@@ -20,7 +20,7 @@ constexpr int kMaxBvhDepth = 30;       // traversal stack entries per ray = dept
 // BVH8 node, 80 bytes = five 16-byte words.  Child boxes are quantised to 8 bits per plane on a per-node
 // grid (origin p, per-axis power-of-two cell 2^(e-127)), rounded outwards, so a node costs five 128-bit loads.
 //   w0 = (p.x, p.y, p.z, e_x | e_y << 8 | e_z << 16 | imask << 24)      imask: bit s = slot s is an internal node
-//   w1 = (child_base, tri_base, trimask, 0)
+//   w1 = (child_base, tri_base, trimask, imask)      imask again as a word: every loaded register is read (see TriPacked)
 //   w2 = (qlo_x[0..3], qlo_x[4..7], qlo_y[0..3], qlo_y[4..7])
 //   w3 = (qlo_z[0..3], qlo_z[4..7], qhi_x[0..3], qhi_x[4..7])
 //   w4 = (qhi_y[0..3], qhi_y[4..7], qhi_z[0..3], qhi_z[4..7])
@@ -37,7 +37,7 @@ struct alignas(16) NodeC {
   uint8_t e[3];
   uint8_t imask;
   uint32_t child_base, tri_base;
-  uint32_t trimask, pad;
+  uint32_t trimask, imask32;
   uint8_t qlo[3][8];
   uint8_t qhi[3][8];
 };
