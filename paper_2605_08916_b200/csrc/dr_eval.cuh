@@ -129,15 +129,6 @@ struct TriSlot {
   uint32_t li;  // leaf-order index, kMiss = empty
 };
 
-__device__ __forceinline__ void tri_fetch(const DevScene& sc, TravState& s, SmemTriStack& tst, int& tsp, TriSlot& t) {
-  if (!s.ty && tsp > 0) tst.pop(--tsp, s);
-  if (s.ty) {
-    t.li = trav_next_tri(s);
-    const float4* p = sc.tris + 3 * (size_t)t.li;
-    t.t0 = __ldg(p); t.t1 = __ldg(p + 1); t.t2 = __ldg(reinterpret_cast<const float2*>(p + 2));
-  }
-}
-
 // q: planes Q0, Q1 of the queue (o, d).  Every warp takes kFetchChunk rays at a time from *head and keeps its lanes
 // supplied from that private range.  The traversal runs in lockstep steps, software-pipelined one step deep so that
 // every load has a phase of arithmetic between its issue and its first use (profiles/r01b: the un-pipelined loop
@@ -208,7 +199,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
     do {
       // The four parts are written without branches (selects and predicated loads / stores) so that the compiler can
       // interleave their dependency chains: with branches around every part each warp waited out the fixed latencies
-      // of its bookkeeping one after the other (profiles/r01d: 53 % of the instructions took 78 % of the time).
+      // of its bookkeeping one after the other (profiles/r01f_k_trace_full.md, step r01e: 53 % of the instructions took 78 % of the time).
       // A: node test
       {
         if (STATS) nn += has_node ? 1u : 0u;

@@ -47,7 +47,7 @@ static_assert(sizeof(NodeC) == 80, "NodeC must be 80 bytes");
 //   t0 = (v0.x, v0.y, v0.z, e1.x), t1 = (e1.y, e1.z, e2.x, e2.y), t2 = (e2.z, bits(original id), bits(material id), 0)
 // The traversal loads t0, t1 and the first half of t2 (40 bytes), so that every register a load writes is read by
 // the triangle test (a loaded-but-unread register is free for reuse while the load is still in flight, which made
-// the next write to it wait for the whole load: profiles/r01e).
+// the next write to it wait for the whole load: profiles/r01f_k_trace_full.md, step r01e).
 struct TriPacked {
   float v0[3];
   float e1[3];
