@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdr.so")
 SOURCES = ["dr_api.cu", "dr_bvh.cpp"]
-DEPS = SOURCES + ["dr_kernels.cuh", "dr_eval.cuh", "dr_traverse.cuh", "dr_path.cuh", "dr_rng.cuh", "dr_types.h", "../../include/dr.h"]
+DEPS = SOURCES + ["dr_kernels.cuh", "dr_eval.cuh", "dr_wave.cuh", "dr_traverse.cuh", "dr_path.cuh", "dr_rng.cuh", "dr_types.h", "../../include/dr.h"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 

@@ -8,6 +8,7 @@
 
 #include "../../include/dr.h"
 #include "dr_kernels.cuh"
+#include "dr_wave.cuh"
 
 using namespace dr;
 
@@ -27,6 +28,7 @@ dr_status fail(dr_status s, const std::string& msg) { g_err = msg; return s; }
 
 size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
+constexpr uint32_t kWaveMinStates = 1u << 18;   // smaller evaluations use the per-segment loop (ring capacity, dr_wave.cuh)
 constexpr size_t kMaxDynSmem = 227 * 1024;  // opt-in shared memory per block on sm_100
 
 bool finite3(const float* v) { return std::isfinite(v[0]) && std::isfinite(v[1]) && std::isfinite(v[2]); }
@@ -174,6 +176,15 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, const EvalWs& ws, con
   }
   CUDA_TRY(cudaMemsetAsync(ws.ctl, 0, 4 * kCtlWords, s));
   { ProfScope ps(prof, DR_PROF_RAYGEN, s); k_raygen<<<g, kShadeBlock, 0, s>>>(dev, ws, io, n); }
+  static const int wave_mode = std::getenv("DR_WAVE") ? std::atoi(std::getenv("DR_WAVE")) : 1;   // DR_WAVE=0: per-segment loop (A/B runs)
+  if (wave_mode && !stats && n >= kWaveMinStates && n < (1u << kWaveKShift)) {
+    // one persistent kernel for all segments (dr_wave.cuh)
+    ProfScope ps(prof, DR_PROF_TRACE, s);
+    CUDA_TRY(cudaMemsetAsync(ws.hits, 0, sizeof(uint2) * (size_t)ws.cap, s));   // ready words of the ring (dr_wave.cuh)
+    k_wave_begin<<<g, kShadeBlock, 0, s>>>(ws, n);
+    if (grad) k_wave<true><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
+    else k_wave<false><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
+  } else
   for (uint32_t k = 1; k <= dev.L; ++k) {
     const float4* q = (k & 1u) ? ws.qa : ws.qb;
     {
@@ -321,6 +332,8 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   s->trace_smem = (size_t)dev.smem_nodes * sizeof(NodeC) + stack_bytes;
   e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e != cudaSuccess) {
     dr_scene_destroy(s);
     return fail(DR_ERR_CUDA, std::string("k_trace shared memory: ") + cudaGetErrorString(e));

@@ -129,6 +129,106 @@ struct TriSlot {
   uint32_t li;  // leaf-order index, kMiss = empty
 };
 
+// One lockstep step of the traversal for this lane (parts A, N, T, F of the comment above k_trace).  Returns true if
+// the lane's ray finished in this step (its closest hit is in r; the caller stores it and clears `active`).
+struct TravLane {
+  TravRay r;
+  TravState s;
+  uint4 w0, w1, w2, w3, w4;      // words of the node to test next (valid if has_node)
+  TriSlot tri[kTrisPerStep];
+  int tsp;                       // postponed triangle groups
+  bool active, has_node;
+};
+
+template <bool STATS>
+__device__ __forceinline__ bool trav_step(const DevScene& sc, const uint4* smem, SmemStack& st, SmemTriStack& tst, TravLane& L,
+                                          uint32_t& nn, uint32_t& nt) {
+  TravRay& r = L.r;
+  TravState& s = L.s;
+  uint4 &w0 = L.w0, &w1 = L.w1, &w2 = L.w2, &w3 = L.w3, &w4 = L.w4;
+  TriSlot* tri = L.tri;
+  int& tsp = L.tsp;
+  const bool active = L.active;
+  bool& has_node = L.has_node;
+  (void)smem;
+  // The four parts are written without branches (selects and predicated loads / stores) so that the compiler can
+  // interleave their dependency chains: with branches around every part each warp waited out the fixed latencies
+  // of its bookkeeping one after the other (profiles/r01f_k_trace_full.md, step r01e: 53 % of the instructions took 78 % of the time).
+  // A: node test
+  {
+    if (STATS) nn += has_node ? 1u : 0u;
+    uint32_t h = node_hits(w0, w1, w2, w3, w4, r);
+    h = has_node ? h : 0u;
+    const uint32_t nty = h & 0x00FFFFFFu;
+    const bool newtri = nty != 0u;
+    bool keep_old = newtri && s.ty != 0u;  // triangles still pending from an earlier node: postpone them
+    if (keep_old && tsp >= kTriStack) {    // (or test them now if their stack is full: rare)
+      while (s.ty) { if (STATS) ++nt; tri_one(sc, r, s); }
+      keep_old = false;
+    }
+    if (keep_old) tst.push(tsp, s);
+    tsp += keep_old ? 1 : 0;
+    s.tx = newtri ? w1.y : s.tx;
+    s.ty = newtri ? nty : s.ty;
+    s.tm = newtri ? w1.z : s.tm;
+    s.gx = has_node ? w1.x : s.gx;
+    s.gy = has_node ? ((h & 0xFF000000u) | w1.w) : s.gy;
+  }
+  // N: next node
+  {
+    const bool popn = active && !(s.gy & 0xFF000000u) && s.sp > 0;
+    s.sp -= popn ? 1 : 0;
+    if (popn) { const uint2 e = st.pop(s.sp); s.gx = e.x; s.gy = e.y; }
+    const bool go = active && (s.gy & 0xFF000000u) != 0u;
+    const uint32_t bit = top_bit(s.gy | 0x01000000u);
+    const uint32_t rest = s.gy & ~(1u << bit);
+    const bool keep = go && (rest & 0xFF000000u) != 0u;
+    if (keep) st.push(s.sp, make_uint2(s.gx, rest));
+    s.sp += keep ? 1 : 0;
+    const uint32_t slot = (bit - 24u) ^ (r.octinv4 & 7u);
+    const uint32_t node = s.gx + popc32(rest & ~(0xFFFFFFFFu << slot) & 0xFFu);
+    s.gy = go ? rest : s.gy;
+    if (go) {
+#if DR_SMEM_NODES == 0
+      const uint4* np = sc.nodes + 5u * (size_t)node;
+      w0 = DR_NODE_LD(np); w1 = DR_NODE_LD(np + 1); w2 = DR_NODE_LD(np + 2); w3 = DR_NODE_LD(np + 3); w4 = DR_NODE_LD(np + 4);
+#else
+      const uint4* np = node < sc.smem_nodes ? smem + 5u * node : sc.nodes + 5u * (size_t)node;
+      w0 = np[0]; w1 = np[1]; w2 = np[2]; w3 = np[3]; w4 = np[4];
+#endif
+    }
+    has_node = go;
+  }
+  // T: triangle tests
+#pragma unroll
+  for (int it = 0; it < kTrisPerStep; ++it) {
+    const bool valid = tri[it].li != kMiss;
+    if (STATS) nt += valid ? 1u : 0u;
+    tri_test_bf(tri[it].t0, tri[it].t1, tri[it].t2, tri[it].li, valid, r);  // reads every loaded word (dr_types.h TriPacked)
+  }
+  // F: next triangles
+  {
+    bool have_any = false;
+#pragma unroll
+    for (int it = 0; it < kTrisPerStep; ++it) {
+      const bool popt = active && s.ty == 0u && tsp > 0;
+      tsp -= popt ? 1 : 0;
+      if (popt) tst.pop(tsp, s);
+      const bool have = active && s.ty != 0u;
+      const uint32_t b = low_bit(s.ty | 0x80000000u);
+      const uint32_t li = s.tx + popc32(s.tm & ~(0xFFFFFFFFu << b));
+      s.ty = have ? (s.ty & (s.ty - 1u)) : s.ty;
+      tri[it].li = have ? li : kMiss;
+      if (have) {
+        const float4* p = sc.tris + 3 * (size_t)li;
+        tri[it].t0 = DR_TRI_LD(p); tri[it].t1 = DR_TRI_LD(p + 1); tri[it].t2 = DR_TRI_LD(reinterpret_cast<const float2*>(p + 2));
+      }
+      have_any = have_any || have;
+    }
+    return active && !(has_node || have_any);  // nothing requested, nothing pending: the ray is finished
+  }
+}
+
 // q: planes Q0, Q1 of the queue (o, d).  Every warp takes kFetchChunk rays at a time from *head and keeps its lanes
 // supplied from that private range.  The traversal runs in lockstep steps, software-pipelined one step deep so that
 // every load has a phase of arithmetic between its issue and its first use (profiles/r01b: the un-pipelined loop
@@ -285,6 +385,94 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   }
 }
 
+// Vertex k of one ray: emission / termination, direction sampling, throughput (rows a3 / a5).  Q0..Q2 = the ray's queue
+// entry, h = (bits(t), triangle in leaf order or kMiss).  A finished path writes f, p, signature of state s; a
+// continuing one returns the next ray in n0..n2 (n0.w = Q0.w).  Shared by k_shade and k_wave.
+template <bool GRAD>
+__device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t k, const float4& Q0,
+                                             const float4& Q1, const float4& Q2, const uint2& h, uint32_t s, bool& cont,
+                                             bool& want_grad, uint32_t& bad, float4& n0, float4& n1, float4& n2) {
+  const size_t cap = ws.cap;
+  uint32_t sig = __float_as_uint(Q1.w), info = __float_as_uint(Q2.w);
+  const float3 o = xyz(Q0), d = xyz(Q1);
+  float T0 = Q2.x, T1 = Q2.y, T2 = Q2.z;
+  float f0 = 0.f, f1 = 0.f, f2 = 0.f;
+  bool done = true;
+  if (h.y == kMiss) {
+    sig = fnv(sig, 0u);
+    f0 = T0 * sc.env[0]; f1 = T1 * sc.env[1]; f2 = T2 * sc.env[2];
+  } else {
+    const uint32_t li = h.y;
+    const float4 t0 = __ldg(&sc.tris[3 * li]), t1 = __ldg(&sc.tris[3 * li + 1]), t2 = __ldg(&sc.tris[3 * li + 2]);
+    const float3 e1 = make_float3(t0.w, t1.x, t1.y), e2 = make_float3(t1.z, t1.w, t2.x);  // dr_types.h TriPacked
+    sig = fnv(sig, __float_as_uint(t2.y) + 1u);
+    const uint32_t mi = __float_as_uint(t2.z);
+    const float4 m0 = __ldg(&sc.mats[3 * mi]), m1 = __ldg(&sc.mats[3 * mi + 1]);
+    const uint32_t kind = __float_as_uint(m0.x);
+    Frame fr;
+    float dn;
+    tri_frame(e1, e2, d, fr, dn);
+    if (kind == 3u) {  // emitter: front face emits, path stops
+      if (dn < 0.f) {
+        sig = fnv(sig, 4u);
+        const float4 m2 = __ldg(&sc.mats[3 * mi + 2]);
+        f0 = T0 * m1.z; f1 = T1 * m1.w; f2 = T2 * m2.x;
+      } else {
+        sig = fnv(sig, 5u);
+      }
+    } else if (k < sc.L) {
+      const float3 hit = o + d * __uint_as_float(h.x);
+      const float2 u = x_pair(io, s, k);
+      if (GRAD) ws.rec[(size_t)k * cap + s] = make_float4(d.x, d.y, d.z, __uint_as_float(li));
+      V3<float> din{d.x, d.y, d.z}, dnew;
+      float off = 1.f;
+      if (kind == 0u) {
+        sig = fnv(sig, 0u);
+        dnew = lambert_dir<float>(fr, u.x, u.y);
+        T0 *= m0.y; T1 *= m0.z; T2 *= m0.w;
+      } else if (kind == 1u) {
+        const float eta = dn < 0.f ? m1.x : 1.0f / m1.x;
+        const float F = fresnel_dielectric(-dot3(d, fr.nf), eta);
+        const bool reflect = u.x < F;
+        sig = fnv(sig, reflect ? 1u : 2u);
+        if (!reflect) { off = -1.f; info |= 1u << k; }
+        dnew = dielectric_dir<float>(fr, eta, reflect, din);
+      } else {
+        sig = fnv(sig, 3u);
+        info |= 1u << 16;
+        float c5, G1;
+        if (!ggx_dir<float>(fr, m1.y, din, u.x, u.y, dnew, c5, G1)) {
+          T0 = T1 = T2 = 0.f;
+        } else {
+          T0 *= (m0.y + (1.0f - m0.y) * c5) * G1;
+          T1 *= (m0.z + (1.0f - m0.z) * c5) * G1;
+          T2 *= (m0.w + (1.0f - m0.w) * c5) * G1;
+        }
+      }
+      if (!(T0 == 0.f && T1 == 0.f && T2 == 0.f)) {
+        done = false;
+        const float3 on = hit + fr.nf * (sc.eps_ray * off);
+        n0 = make_float4(on.x, on.y, on.z, Q0.w);
+        n1 = make_float4(dnew.x, dnew.y, dnew.z, __uint_as_float(sig));
+        n2 = make_float4(T0, T1, T2, __uint_as_float(info));
+      }
+    }
+  }
+  cont = !done;
+  if (done) {
+    float p = f0 * 0.2126f + f1 * 0.7152f + f2 * 0.0722f;
+    if (!(isfinite(f0) && isfinite(f1) && isfinite(f2) && isfinite(p))) { f0 = f1 = f2 = p = 0.f; bad = 1; }
+    io.f[s] = make_float4(f0, f1, f2, p);
+    io.sig[s] = sig;
+    if (io.nrays) io.nrays[s] = k;
+    if (GRAD) {
+      ws.pinfo[s] = (info & 0xFFFFu) | (k << 16);
+      // only GGX weights depend on x: no GGX vertex or p == 0  =>  score == 0 exactly
+      want_grad = (info >> 16) && p > 0.f;
+    }
+  }
+}
+
 // ---- a3 / a5: shade vertex k of every ray of segment k -------------------------------------------------------------
 template <bool GRAD>
 __global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, EvalIO io, uint32_t k) {
@@ -301,86 +489,8 @@ __global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, E
   uint32_t bad = 0, s = 0;
   if (j < n) {
     const float4 Q0 = qin[j], Q1 = qin[cap + j], Q2 = qin[2 * cap + j];
-    const uint2 h = ws.hits[j];
     s = __float_as_uint(Q0.w);
-    uint32_t sig = __float_as_uint(Q1.w), info = __float_as_uint(Q2.w);
-    const float3 o = xyz(Q0), d = xyz(Q1);
-    float T0 = Q2.x, T1 = Q2.y, T2 = Q2.z;
-    float f0 = 0.f, f1 = 0.f, f2 = 0.f;
-    bool done = true;
-    if (h.y == kMiss) {
-      sig = fnv(sig, 0u);
-      f0 = T0 * sc.env[0]; f1 = T1 * sc.env[1]; f2 = T2 * sc.env[2];
-    } else {
-      const uint32_t li = h.y;
-      const float4 t0 = __ldg(&sc.tris[3 * li]), t1 = __ldg(&sc.tris[3 * li + 1]), t2 = __ldg(&sc.tris[3 * li + 2]);
-      const float3 e1 = make_float3(t0.w, t1.x, t1.y), e2 = make_float3(t1.z, t1.w, t2.x);  // dr_types.h TriPacked
-      sig = fnv(sig, __float_as_uint(t2.y) + 1u);
-      const uint32_t mi = __float_as_uint(t2.z);
-      const float4 m0 = __ldg(&sc.mats[3 * mi]), m1 = __ldg(&sc.mats[3 * mi + 1]);
-      const uint32_t kind = __float_as_uint(m0.x);
-      Frame fr;
-      float dn;
-      tri_frame(e1, e2, d, fr, dn);
-      if (kind == 3u) {  // emitter: front face emits, path stops
-        if (dn < 0.f) {
-          sig = fnv(sig, 4u);
-          const float4 m2 = __ldg(&sc.mats[3 * mi + 2]);
-          f0 = T0 * m1.z; f1 = T1 * m1.w; f2 = T2 * m2.x;
-        } else {
-          sig = fnv(sig, 5u);
-        }
-      } else if (k < sc.L) {
-        const float3 hit = o + d * __uint_as_float(h.x);
-        const float2 u = x_pair(io, s, k);
-        if (GRAD) ws.rec[(size_t)k * cap + s] = make_float4(d.x, d.y, d.z, __uint_as_float(li));
-        V3<float> din{d.x, d.y, d.z}, dnew;
-        float off = 1.f;
-        if (kind == 0u) {
-          sig = fnv(sig, 0u);
-          dnew = lambert_dir<float>(fr, u.x, u.y);
-          T0 *= m0.y; T1 *= m0.z; T2 *= m0.w;
-        } else if (kind == 1u) {
-          const float eta = dn < 0.f ? m1.x : 1.0f / m1.x;
-          const float F = fresnel_dielectric(-dot3(d, fr.nf), eta);
-          const bool reflect = u.x < F;
-          sig = fnv(sig, reflect ? 1u : 2u);
-          if (!reflect) { off = -1.f; info |= 1u << k; }
-          dnew = dielectric_dir<float>(fr, eta, reflect, din);
-        } else {
-          sig = fnv(sig, 3u);
-          info |= 1u << 16;
-          float c5, G1;
-          if (!ggx_dir<float>(fr, m1.y, din, u.x, u.y, dnew, c5, G1)) {
-            T0 = T1 = T2 = 0.f;
-          } else {
-            T0 *= (m0.y + (1.0f - m0.y) * c5) * G1;
-            T1 *= (m0.z + (1.0f - m0.z) * c5) * G1;
-            T2 *= (m0.w + (1.0f - m0.w) * c5) * G1;
-          }
-        }
-        if (!(T0 == 0.f && T1 == 0.f && T2 == 0.f)) {
-          done = false;
-          const float3 on = hit + fr.nf * (sc.eps_ray * off);
-          n0 = make_float4(on.x, on.y, on.z, Q0.w);
-          n1 = make_float4(dnew.x, dnew.y, dnew.z, __uint_as_float(sig));
-          n2 = make_float4(T0, T1, T2, __uint_as_float(info));
-        }
-      }
-    }
-    cont = !done;
-    if (done) {
-      float p = f0 * 0.2126f + f1 * 0.7152f + f2 * 0.0722f;
-      if (!(isfinite(f0) && isfinite(f1) && isfinite(f2) && isfinite(p))) { f0 = f1 = f2 = p = 0.f; bad = 1; }
-      io.f[s] = make_float4(f0, f1, f2, p);
-      io.sig[s] = sig;
-      if (io.nrays) io.nrays[s] = k;
-      if (GRAD) {
-        ws.pinfo[s] = (info & 0xFFFFu) | (k << 16);
-        // only GGX weights depend on x: no GGX vertex or p == 0  =>  score == 0 exactly
-        want_grad = (info >> 16) && p > 0.f;
-      }
-    }
+    shade_vertex<GRAD>(sc, ws, io, k, Q0, Q1, Q2, ws.hits[j], s, cont, want_grad, bad, n0, n1, n2);
   }
   const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
   if (GRAD) {  // reverse-pass list: one atomic per warp
