@@ -21,7 +21,7 @@ import numpy as np  # noqa: E402
 METRIC = "chain mutations/s at 1024x576 (Diffusion Restore, transparent-machines scene)"
 UNIT = "mutations/s"
 # Algorithmic FLOPs of the path evaluation: one BVH8 node visit = 8 slab tests of
-# 6 FMA + 12 min/max = 192 FLOP; one Moeller-Trumbore test = 50 FLOP (k_trace does no shading).
+# 6 FMA + 12 min/max = 192 FLOP; one Moeller-Trumbore test = 50 FLOP.  The shading that k_wave also does is not counted.
 F_NODE, F_TRI = 192.0, 50.0
 # Algorithmic bytes per mutation of the state-streaming kernels (propose + decide + scan + scatter), d = 2L:
 # read x, score (2 * 4d) + write x, score (2 * 4d) + p, f/p_hat, pixel, flags read and written (2 * 21).
@@ -281,10 +281,13 @@ def main():
     stream_gbs = stream_bytes_per_mutation(desc.dim, grad) * n_local / (stream_ms * 1e-3) / 1e9
     launches_per_frame = sum(v["launches"] for v in prof.values()) / prof_frames
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "trace_traffic.txt")     # from the last ncu --set full capture of k_trace
+    # large evaluations run traversal + shading of all segments as one persistent kernel (k_wave, one launch per frame);
+    # small ones, or DR_WAVE=0, the per-segment loop (k_trace + k_shade, L launches each per frame)
+    wave = prof["shade"]["launches"] == 0
+    tp = os.path.join(ROOT, "profiles", "trace_traffic.txt")     # from the last ncu --set full capture of that kernel
     if os.path.exists(tp):
         for line in open(tp):
-            if line.startswith("dram_bytes_per_launch"):
+            if line.startswith("dram_bytes_per_launch_k_wave" if wave else "dram_bytes_per_launch_k_trace"):
                 traffic = int(line.split()[1])
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -305,7 +308,7 @@ def main():
         "kernel_launches_per_frame": launches_per_frame,
         "gpu_launches": int(round(launches_per_frame * args.steps)),
         "clocks": clocks,
-        "roofline": {"kernel": "k_trace", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+        "roofline": {"kernel": "k_wave" if wave else "k_trace", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                      "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": traffic,
                      "peak_source": f"148 SM x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
                      "flop_per_ray": flop_per_ray, "rays_per_launch": rays_per_launch, "launch_ms": trace_ms,

@@ -29,6 +29,8 @@ dr_status fail(dr_status s, const std::string& msg) { g_err = msg; return s; }
 size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
 constexpr uint32_t kWaveMinStates = 1u << 18;   // smaller evaluations use the per-segment loop (ring capacity, dr_wave.cuh)
+constexpr uint32_t kWaveMaxStates = 1u << 21;   // and so do very large ones: their launches are long enough for the tail not to matter, and
+                                                // k_trace's 20 trace warps beat k_wave's 17 (profiles/r01g_sweep.md vs r01f_sweep.md at 4 M chains)
 constexpr size_t kMaxDynSmem = 227 * 1024;  // opt-in shared memory per block on sm_100
 
 bool finite3(const float* v) { return std::isfinite(v[0]) && std::isfinite(v[1]) && std::isfinite(v[2]); }
@@ -177,11 +179,11 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, const EvalWs& ws, con
   CUDA_TRY(cudaMemsetAsync(ws.ctl, 0, 4 * kCtlWords, s));
   { ProfScope ps(prof, DR_PROF_RAYGEN, s); k_raygen<<<g, kShadeBlock, 0, s>>>(dev, ws, io, n); }
   static const int wave_mode = std::getenv("DR_WAVE") ? std::atoi(std::getenv("DR_WAVE")) : 1;   // DR_WAVE=0: per-segment loop (A/B runs)
-  if (wave_mode && !stats && n >= kWaveMinStates && n < (1u << kWaveKShift)) {
+  if (wave_mode && !stats && n >= kWaveMinStates && n < kWaveMaxStates) {
     // one persistent kernel for all segments (dr_wave.cuh)
-    ProfScope ps(prof, DR_PROF_TRACE, s);
     CUDA_TRY(cudaMemsetAsync(ws.hits, 0, sizeof(uint2) * (size_t)ws.cap, s));   // ready words of the ring (dr_wave.cuh)
-    k_wave_begin<<<g, kShadeBlock, 0, s>>>(ws, n);
+    { ProfScope pb(prof, DR_PROF_RAYGEN, s); k_wave_begin<<<g, kShadeBlock, 0, s>>>(ws, n); }
+    ProfScope ps(prof, DR_PROF_TRACE, s);
     if (grad) k_wave<true><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
     else k_wave<false><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
   } else
