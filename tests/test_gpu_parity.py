@@ -358,3 +358,41 @@ def test_full_size_configs(dr, oracle, torch_, case):
         assert div.mean() < 1e-3, rep
         if not div.any():
             assert (gch.queue() == och.queue()).all()
+
+
+# ---- the two forms of the evaluation (k_wave vs per-segment loop) -------------------------------------------------
+_EVAL_SNIPPET = """
+import sys, numpy as np, torch
+sys.path.insert(0, {root!r})
+import paper_2605_08916_b200 as dr
+from dr_inputs import scenes as S
+desc = getattr(S, {scene!r})()
+x = torch.from_numpy(S.seeded_states({n}, desc.dim, 11)).cuda()
+e = dr.Scene(desc).eval_states(x, True)
+torch.cuda.synchronize()
+np.savez({out!r}, **{{k: v.cpu().numpy() for k, v in e.items()}})
+"""
+
+
+@pytest.mark.parametrize("scene", ["mini_machines", "ggx_room"])
+def test_wave_kernel_equals_segment_loop(dr, torch_, tmp_path, scene):
+    """2^18 states evaluated by k_wave (one persistent kernel, dr_wave.cuh) and, in a second process with DR_WAVE=0, by
+    the per-segment loop k_trace / k_shade: both run the same shade_vertex on the same closest hits, so f, p, pixel,
+    rays per path, signature and score must be identical bit for bit -- anything else is a ray lost, duplicated or
+    read before it was written in the ring.  (The small parity scenes above never reach k_wave: it starts at 2^18.)"""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    n = 1 << 18
+    res = {}
+    for mode in ("1", "0"):
+        out = str(tmp_path / f"eval_{mode}.npz")
+        env = dict(os.environ, DR_WAVE=mode)
+        subprocess.run([sys.executable, "-c", _EVAL_SNIPPET.format(root=root, scene=scene, n=n, out=out)], check=True, env=env,
+                       timeout=600)
+        res[mode] = np.load(out)
+    a, b = res["1"], res["0"]
+    assert int(a["nrays"].sum()) == int(b["nrays"].sum()) and a["nrays"].sum() > n      # paths do bounce
+    for k in ("f", "p", "pix", "nrays", "sig", "g"):
+        assert np.array_equal(a[k].view(np.uint32), b[k].view(np.uint32)), k
