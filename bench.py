@@ -180,8 +180,7 @@ def main():
     def frame():
         chains.step(1)
         if world > 1:
-            acc, tours, muts = sharding.allreduce_frame(chains.accum, chains)
-            chains.resolve_sharded(acc, tours, muts)
+            sharding.resolve_frame(chains)
         else:
             chains.resolve()
 

@@ -14,8 +14,8 @@
  *    accumulation buffer and the output image are CALLER-OWNED DEVICE MEMORY (e.g. torch
  *    tensors); the library never frees them and they must outlive the dr_chains handle.
  *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  All work is
- *    asynchronous on that stream; only dr_chains_stats and the *_download / *_upload hooks
- *    synchronise it.
+ *    asynchronous on that stream; only dr_chains_stats, dr_profile_*, dr_chains_work_stats and the
+ *    *_download / *_upload hooks synchronise it.
  *  - one GPU (the current device), fp32 arithmetic, sm_100a only, no CPU fallback.
  */
 #ifndef DR_H_
@@ -30,7 +30,7 @@ extern "C" {
 
 typedef enum {
   DR_OK = 0,
-  DR_WARN_NO_TOURS = 1,      /* resolve before any tour completed: zero image, no division */
+  DR_WARN_NO_TOURS = 1,      /* dr_chains_stats: a resolve ran before any tour completed: zero image, no division */
   DR_ERR_INVALID_ARG = -1,
   DR_ERR_UNSUPPORTED = -2,
   DR_ERR_CUDA = -3,
@@ -107,6 +107,7 @@ typedef struct {
   uint32_t regen_queue_len;
   uint32_t iteration;        /* n of the last completed iteration (0 = init) */
   float p_lambda, kappa0, lambda;
+  uint32_t no_tour_resolves; /* resolves since init that found tourCount == 0 and wrote a zero image */
 } dr_stats;
 
 typedef struct {
@@ -146,14 +147,24 @@ dr_status dr_chains_init(dr_chains* chains, uint32_t frame_index, void* stream);
 dr_status dr_step(dr_chains* chains, int32_t method, uint32_t iterations, void* stream);
 
 /* Alg. 3: dev_rgb_out[W*H*3] = N_pix * kappa0 / tourCount * accum (Restore) or N_pix * p_lambda / N_mut * accum
- * (plain MH).  Returns DR_WARN_NO_TOURS and writes zeros if tourCount == 0 (the check synchronises the stream). */
+ * (plain MH).  Asynchronous: if tourCount == 0 the kernel writes zeros (no division) and counts the event in
+ * dr_stats.no_tour_resolves; the next dr_chains_stats then returns DR_WARN_NO_TOURS. */
 dr_status dr_resolve_image(dr_chains* chains, float* dev_rgb_out, void* stream);
 
 /* Alg. 3 for a run sharded over several GPUs: dev_accum_sum is the all-reduced accumulation buffer
  * (W*H float4), tours_total / mutations_total the all-reduced counters (mutations_total > 0).  p_lambda and kappa0
- * are this shard's; they are identical on every shard when p_lambda_override is used.  Asynchronous. */
+ * are this shard's; they are identical on every shard when p_lambda_override is used.  Asynchronous; tours_total == 0
+ * is handled as in dr_resolve_image. */
 dr_status dr_resolve_image_sharded(dr_chains* chains, const float* dev_accum_sum, uint64_t tours_total,
                                    uint64_t mutations_total, float* dev_rgb_out, void* stream);
+
+/* The same with ONE collective and no host synchronisation per frame: dr_pack_frame writes dr_frame_floats(chains) =
+ * W*H*4 + 8 floats into dev_buf (16-byte aligned): this shard's accumulation buffer followed by tourCount and the mutation
+ * count as four 16-bit limbs each, stored as floats, so that an fp32 all-reduce(sum) over up to 256 shards adds them exactly;
+ * dr_resolve_image_packed takes the all-reduced buffer.  Both asynchronous. */
+size_t dr_frame_floats(const dr_chains* chains);
+dr_status dr_pack_frame(dr_chains* chains, float* dev_buf, void* stream);
+dr_status dr_resolve_image_packed(dr_chains* chains, const float* dev_buf_sum, float* dev_rgb_out, void* stream);
 
 /* Per-kernel timing with CUDA events on the caller's stream (bench.py's roofline).  dr_profile_enable(on) resets
  * the totals; while on, every kernel launch of dr_chains_init / dr_step / dr_resolve_image* is bracketed by two
@@ -167,7 +178,7 @@ dr_status dr_profile_read(dr_chains* chains, double* host_ms, uint64_t* host_lau
  * proposals (re-evaluated with counters; values only).  Synchronises. */
 dr_status dr_chains_work_stats(dr_chains* chains, uint64_t* host_out3, void* stream);
 
-/* Synchronises the stream and copies the counters. */
+/* Synchronises the stream and copies the counters.  DR_WARN_NO_TOURS (with host_out filled) if no_tour_resolves != 0. */
 dr_status dr_chains_stats(dr_chains* chains, dr_stats* host_out, void* stream);
 
 /* ---- test hooks (parity harness; same library) ---------------------------------------------------------- */
@@ -191,6 +202,13 @@ dr_status dr_trace_rays(const dr_scene* scene, const float* dev_o, const float* 
  * non-NULL), nrays[n], sig[n]. */
 dr_status dr_eval_states(const dr_scene* scene, const float* dev_x, uint32_t n, float* dev_f, float* dev_p,
                          uint32_t* dev_pix, float* dev_score, uint32_t* dev_nrays, uint32_t* dev_sig, void* stream);
+/* The same, choosing the form of rows a3-a5 (identical results, state by state): 0 = default, 1 = one k_trace + k_shade
+ * launch per segment, 2 = one persistent k_wave launch (csrc/dr_wave.cuh).  dr_chains_set_eval_form does the same for
+ * the evaluations inside dr_chains_init / dr_step. */
+dr_status dr_eval_states_form(const dr_scene* scene, const float* dev_x, uint32_t n, float* dev_f, float* dev_p,
+                              uint32_t* dev_pix, float* dev_score, uint32_t* dev_nrays, uint32_t* dev_sig, int32_t form,
+                              void* stream);
+dr_status dr_chains_set_eval_form(dr_chains* chains, int32_t form);
 /* Work statistics for n states (device x[n*d], values only): dev_out3[0..2] += {rays, BVH8 node visits, triangle
  * tests}.  bench.py derives the algorithmic FLOPs per ray of its roofline from these. */
 dr_status dr_eval_work_stats(const dr_scene* scene, const float* dev_x, uint32_t n, uint64_t* dev_out3, void* stream);

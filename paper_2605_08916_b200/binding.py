@@ -12,7 +12,7 @@ import numpy as np
 import torch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libdr.so")
+LIB_PATH = os.environ.get("DR_LIB") or os.path.join(HERE, "libdr.so")   # DR_LIB: a build_variant() library (tests)
 
 DR_OK, DR_WARN_NO_TOURS = 0, 1
 DR_ERR_INVALID_ARG, DR_ERR_UNSUPPORTED, DR_ERR_CUDA, DR_ERR_NONFINITE, DR_ERR_OOM = -1, -2, -3, -4, -5
@@ -24,7 +24,8 @@ EXPORTS = [
     "dr_chains_state_bytes", "dr_chains_create", "dr_chains_destroy", "dr_chains_init", "dr_step", "dr_resolve_image",
     "dr_chains_stats", "dr_chains_download", "dr_chains_upload", "dr_chains_last_step", "dr_regen_queue_download",
     "dr_trace_rays", "dr_eval_states", "dr_philox_blocks", "dr_rng_transforms", "dr_resolve_image_sharded",
-    "dr_eval_work_stats", "dr_profile_enable", "dr_profile_read", "dr_chains_work_stats",
+    "dr_eval_work_stats", "dr_profile_enable", "dr_profile_read", "dr_chains_work_stats", "dr_eval_states_form",
+    "dr_chains_set_eval_form", "dr_frame_floats", "dr_pack_frame", "dr_resolve_image_packed",
 ]
 PROF_NAMES = ["propose", "raygen", "trace", "shade", "grad", "decide", "scan", "scatter", "resolve"]
 
@@ -56,7 +57,8 @@ class dr_config(C.Structure):
 class dr_stats(C.Structure):
     _fields_ = [("tours", C.c_uint64), ("mutations", C.c_uint64), ("rays", C.c_uint64), ("mh_accepts", C.c_uint64),
                 ("nonfinite", C.c_uint64), ("kills_last_step", C.c_uint32), ("regen_queue_len", C.c_uint32),
-                ("iteration", C.c_uint32), ("p_lambda", C.c_float), ("kappa0", C.c_float), ("lambda_", C.c_float)]
+                ("iteration", C.c_uint32), ("p_lambda", C.c_float), ("kappa0", C.c_float), ("lambda_", C.c_float),
+                ("no_tour_resolves", C.c_uint32)]
 
 
 class dr_scene_info(C.Structure):
@@ -95,6 +97,12 @@ def _load():
     L.dr_regen_queue_download.argtypes = [vp, vp, C.POINTER(u32), vp]
     L.dr_trace_rays.argtypes = [vp, vp, vp, u32, vp, vp, vp]
     L.dr_eval_states.argtypes = [vp, vp, u32, vp, vp, vp, vp, vp, vp, vp]
+    L.dr_eval_states_form.argtypes = [vp, vp, u32, vp, vp, vp, vp, vp, vp, i32, vp]
+    L.dr_chains_set_eval_form.argtypes = [vp, i32]
+    L.dr_frame_floats.restype = C.c_size_t
+    L.dr_frame_floats.argtypes = [vp]
+    L.dr_pack_frame.argtypes = [vp, vp, vp]
+    L.dr_resolve_image_packed.argtypes = [vp, vp, vp, vp]
     L.dr_resolve_image_sharded.argtypes = [vp, vp, u64, u64, vp, vp]
     L.dr_eval_work_stats.argtypes = [vp, vp, u32, vp, vp]
     L.dr_profile_enable.argtypes = [vp, i32, vp]
@@ -103,7 +111,7 @@ def _load():
     L.dr_philox_blocks.argtypes = [u64, vp, u32, vp, vp]
     L.dr_rng_transforms.argtypes = [vp, u32, vp, vp]
     for name in EXPORTS:
-        if name not in ("dr_last_error", "dr_chains_state_bytes"):
+        if name not in ("dr_last_error", "dr_chains_state_bytes", "dr_frame_floats"):
             getattr(L, name).restype = i32
     return L
 
@@ -189,7 +197,7 @@ class Scene:
         r, n, t = (int(v) for v in out.cpu())
         return dict(rays=r, node_visits=n, tri_tests=t)
 
-    def eval_states(self, x: torch.Tensor, want_score=True):
+    def eval_states(self, x: torch.Tensor, want_score=True, form=0):
         x = x.contiguous()
         n = x.shape[0]
         dev = dict(device="cuda")
@@ -197,8 +205,8 @@ class Scene:
                    pix=torch.empty(n, dtype=torch.int32, **dev), nrays=torch.empty(n, dtype=torch.int32, **dev),
                    sig=torch.empty(n, dtype=torch.int32, **dev))
         g = torch.zeros(n, self.dim, dtype=torch.float32, **dev) if want_score else None
-        _check(lib.dr_eval_states(self.h, _dp(x), n, _dp(out["f"]), _dp(out["p"]), _dp(out["pix"]),
-                                  _dp(g) if want_score else None, _dp(out["nrays"]), _dp(out["sig"]), _stream()))
+        _check(lib.dr_eval_states_form(self.h, _dp(x), n, _dp(out["f"]), _dp(out["p"]), _dp(out["pix"]),
+                                       _dp(g) if want_score else None, _dp(out["nrays"]), _dp(out["sig"]), int(form), _stream()))
         out["g"] = g
         return out
 
@@ -232,6 +240,9 @@ class Chains:
             lib.dr_chains_destroy(self.h)
             self.h = None
 
+    def set_eval_form(self, form: int):
+        _check(lib.dr_chains_set_eval_form(self.h, int(form)))
+
     def init(self, frame=0):
         _check(lib.dr_chains_init(self.h, int(frame), _stream()))
 
@@ -239,6 +250,7 @@ class Chains:
         _check(lib.dr_step(self.h, self.method, int(iterations), _stream()))
 
     def resolve(self):
+        """Asynchronous; (image, 0).  A resolve before the first completed tour shows in stats()["status"]."""
         status = _check(lib.dr_resolve_image(self.h, _dp(self.image), _stream()), allow_warn=True)
         return self.image, status
 
@@ -246,6 +258,17 @@ class Chains:
         status = _check(lib.dr_resolve_image_sharded(self.h, _dp(accum_sum), int(tours_total), int(mutations_total),
                                                      _dp(self.image), _stream()), allow_warn=True)
         return self.image, status
+
+    def pack_frame(self) -> torch.Tensor:
+        """This shard's frame (accumulation buffer + counters as limbs) in one buffer, ready for one all-reduce(sum)."""
+        if getattr(self, "frame", None) is None:
+            self.frame = torch.empty(lib.dr_frame_floats(self.h), dtype=torch.float32, device="cuda")
+        _check(lib.dr_pack_frame(self.h, _dp(self.frame), _stream()))
+        return self.frame
+
+    def resolve_packed(self, frame_sum: torch.Tensor):
+        _check(lib.dr_resolve_image_packed(self.h, _dp(frame_sum), _dp(self.image), _stream()))
+        return self.image
 
     def profile_enable(self, on=True):
         _check(lib.dr_profile_enable(self.h, int(on), _stream()))
@@ -263,8 +286,9 @@ class Chains:
 
     def stats(self) -> dict:
         o = dr_stats()
-        _check(lib.dr_chains_stats(self.h, C.byref(o), _stream()))
+        status = _check(lib.dr_chains_stats(self.h, C.byref(o), _stream()), allow_warn=True)
         d = {k: getattr(o, k) for k, _ in o._fields_}
+        d["status"] = status
         d["lambda"] = d.pop("lambda_")
         return d
 

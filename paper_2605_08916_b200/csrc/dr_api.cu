@@ -28,16 +28,15 @@ dr_status fail(dr_status s, const std::string& msg) { g_err = msg; return s; }
 
 size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
-constexpr uint32_t kWaveMinStates = 1u << 18;   // smaller evaluations use the per-segment loop (ring capacity, dr_wave.cuh)
-constexpr uint32_t kWaveMaxStates = 1u << 21;   // and so do very large ones: their launches are long enough for the tail not to matter, and
-                                                // k_trace's 20 trace warps beat k_wave's 17 (profiles/r01g_sweep.md vs r01f_sweep.md at 4 M chains)
+constexpr uint32_t kWaveMaxStates = 1u << 21;   // very large evaluations use the per-segment loop: their launches are long enough for the tail
+                                                // not to matter, and k_trace's 20 trace warps beat k_wave's 17 (profiles/r01g_sweep.md vs r01f_sweep.md)
 constexpr size_t kMaxDynSmem = 227 * 1024;  // opt-in shared memory per block on sm_100
 
 bool finite3(const float* v) { return std::isfinite(v[0]) && std::isfinite(v[1]) && std::isfinite(v[2]); }
 
-void normalize(float* v) {
-  const float n = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
-  v[0] /= n; v[1] /= n; v[2] /= n;
+void normalize(float* v) {   // a * (1 / |a|), the form used everywhere (dr_path.cuh)
+  const float inv = 1.0f / std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+  v[0] *= inv; v[1] *= inv; v[2] *= inv;
 }
 void cross(const float* a, const float* b, float* c) {
   c[0] = a[1] * b[2] - a[2] * b[1];
@@ -55,6 +54,7 @@ struct dr_scene {
   dr_scene_info info{};
   int n_sm = 1;            // persistent k_trace grid: one block per SM
   size_t trace_smem = 0;   // staged top-level nodes + per-thread traversal stacks
+  bool wave_ok = false;    // k_wave's shared memory (trace_smem + kWaveExtraSmem) fits; otherwise every evaluation uses the loop
 };
 
 struct dr_chains {
@@ -76,6 +76,8 @@ struct dr_chains {
   double prof_ms[DR_PROF_COUNT] = {};
   uint64_t prof_launches[DR_PROF_COUNT] = {};
   EvalWs ws{};
+  uint32_t eval_tag = 0;           // k_wave: tag of the last evaluation (dr_wave.cuh)
+  int eval_form = 0;               // test hook dr_chains_set_eval_form: 0 = default choice, 1 = per-segment loop, 2 = k_wave
   ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
 };
 
@@ -83,7 +85,7 @@ namespace {
 
 struct Layout {
   size_t x, g, fp, pix, sig, killed, y, gy, fy, pixy, sigy, kind, accepted, weight, order, blockcnt, blockoff, partial, ctr;
-  size_t qa, qb, hits, rec, pinfo, gradlist, ctl;   // evaluation workspace (dr_eval.cuh EvalWs)
+  size_t q, hits, ring, rec, pinfo, gradlist, ctl;   // evaluation workspace (dr_eval.cuh EvalWs)
   size_t total;
 };
 
@@ -111,9 +113,9 @@ Layout make_layout(uint32_t N, uint32_t planes, uint32_t Lseg, bool grad) {
   L.blockoff = take(4 * nb);
   L.partial = take(8 * nb);
   L.ctr = take(sizeof(Counters));
-  L.qa = take(3 * sizeof(float4) * (size_t)N);
-  L.qb = take(3 * sizeof(float4) * (size_t)N);
+  L.q = take(6 * sizeof(float4) * (size_t)N);           // qa | qb, or the 64-byte ray records of k_wave
   L.hits = take(sizeof(uint2) * (size_t)N);
+  L.ring = take(sizeof(uint2) * (size_t)N * Lseg);      // one entry per ray of an evaluation, never reused (dr_wave.cuh)
   L.rec = take(grad ? sizeof(float4) * (size_t)N * Lseg : 0);
   L.pinfo = take(grad ? 4 * (size_t)N : 0);
   L.gradlist = take(grad ? 4 * (size_t)N : 0);
@@ -163,10 +165,11 @@ struct ProfScope {
   ~ProfScope() { if (on) cudaEventRecord(c->ev[2 * k + 1], s); }
 };
 
-// Rows a3-a6 for n states (dr_eval.cuh): raygen, then trace + shade per segment, then the reverse pass.
-// prof may be null (test hooks).  io.g must be zero on entry when grad is set.
-dr_status launch_eval(dr_chains* prof, const dr_scene* sc, const EvalWs& ws, const EvalIO& io, uint32_t n, bool grad, bool stats,
-                      cudaStream_t s) {
+// Rows a3-a6 for n states (dr_eval.cuh): raygen, then trace + shade of every segment, then the reverse pass.
+// prof may be null (test hooks).  io.g must be zero on entry when grad is set.  form: 0 = default (one persistent
+// k_wave launch; the per-segment loop for the counting pass and for very large n), 1 = loop, 2 = k_wave.
+dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const EvalIO& io, uint32_t n, bool grad, bool stats,
+                      int form, cudaStream_t s) {
   const DevScene& dev = sc->dev;
   const uint32_t g = (n + kShadeBlock - 1) / kShadeBlock;
   if (dev.analytic) {
@@ -176,13 +179,14 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, const EvalWs& ws, con
     CUDA_TRY(cudaGetLastError());
     return DR_OK;
   }
+  const bool wave = !stats && sc->wave_ok && (form == 2 || (form == 0 && n < kWaveMaxStates));
   CUDA_TRY(cudaMemsetAsync(ws.ctl, 0, 4 * kCtlWords, s));
-  { ProfScope ps(prof, DR_PROF_RAYGEN, s); k_raygen<<<g, kShadeBlock, 0, s>>>(dev, ws, io, n); }
-  static const int wave_mode = std::getenv("DR_WAVE") ? std::atoi(std::getenv("DR_WAVE")) : 1;   // DR_WAVE=0: per-segment loop (A/B runs)
-  if (wave_mode && !stats && n >= kWaveMinStates && n < kWaveMaxStates) {
-    // one persistent kernel for all segments (dr_wave.cuh)
-    CUDA_TRY(cudaMemsetAsync(ws.hits, 0, sizeof(uint2) * (size_t)ws.cap, s));   // ready words of the ring (dr_wave.cuh)
-    { ProfScope pb(prof, DR_PROF_RAYGEN, s); k_wave_begin<<<g, kShadeBlock, 0, s>>>(ws, n); }
+  {
+    ProfScope ps(prof, DR_PROF_RAYGEN, s);
+    if (wave) k_raygen<true><<<g, kShadeBlock, 0, s>>>(dev, ws, io, n);
+    else k_raygen<false><<<g, kShadeBlock, 0, s>>>(dev, ws, io, n);
+  }
+  if (wave) {
     ProfScope ps(prof, DR_PROF_TRACE, s);
     if (grad) k_wave<true><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
     else k_wave<false><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
@@ -205,6 +209,18 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, const EvalWs& ws, con
   return DR_OK;
 }
 
+// Every evaluation of a chain ensemble gets its own tag (dr_wave.cuh): the state memory is zeroed by dr_chains_init and
+// tags start at 1, so queue entries of earlier evaluations never look published.
+EvalWs next_ws(dr_chains* c, cudaStream_t s) {
+  if (++c->eval_tag == 0) {   // 2^32 evaluations later: clear the queue once and start over
+    cudaMemsetAsync(c->ws.ring, 0, sizeof(uint2) * (size_t)c->ws.cap * c->scene->dev.L, s);
+    c->eval_tag = 1;
+  }
+  EvalWs ws = c->ws;
+  ws.tag = c->eval_tag;
+  return ws;
+}
+
 EvalIO chain_io(const dr_chains* c, bool use_order) {
   EvalIO io{};
   io.x = c->st.y; io.stride = c->cp.N; io.order = use_order ? c->st.order : nullptr;
@@ -219,7 +235,7 @@ dr_status launch_iteration(dr_chains* c, uint32_t n, bool init, cudaStream_t s) 
   const uint32_t gb = c->nblocks;
   { ProfScope ps(c, DR_PROF_PROPOSE, s); k_propose<<<gb, kBlock, 0, s>>>(cp, c->st, n, init ? 1 : 0); }
   // evaluation order: alive chains first, then the regeneration queue (a9), once the queue exists
-  const dr_status es = launch_eval(c, c->scene, c->ws, chain_io(c, !init && cp.restore), cp.N, cp.grad != 0, false, s);
+  const dr_status es = launch_eval(c, c->scene, next_ws(c, s), chain_io(c, !init && cp.restore), cp.N, cp.grad != 0, false, c->eval_form, s);
   if (es != DR_OK) return es;
   if (init) {
     k_psum_partial<<<gb, kBlock, 0, s>>>(cp, c->st);
@@ -246,21 +262,22 @@ struct DevBuf {
 struct HookEval {
   DevBuf ws_mem, xpl, gpl, f4;
   EvalWs ws{};
-  cudaError_t setup(const dr_scene* sc, uint32_t n, bool grad) {
+  cudaError_t setup(const dr_scene* sc, uint32_t n, bool grad, cudaStream_t stream) {
     const size_t N = n, L = sc->dev.L;
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o = align256(o + bytes); return at; };
-    const size_t qa = take(48 * N), qb = take(48 * N), hits = take(8 * N), rec = take(grad ? 16 * N * L : 0), pinfo = take(grad ? 4 * N : 0),
-                 gl = take(grad ? 4 * N : 0), ctl = take(4 * kCtlWords);
+    const size_t q = take(96 * N), hits = take(8 * N), ring = take(8 * N * L), rec = take(grad ? 16 * N * L : 0),
+                 pinfo = take(grad ? 4 * N : 0), gl = take(grad ? 4 * N : 0), ctl = take(4 * kCtlWords);
     cudaError_t e = ws_mem.alloc(o);
     if (e == cudaSuccess) e = xpl.alloc(16 * N * sc->dev.planes);
     if (e == cudaSuccess) e = gpl.alloc(grad ? 16 * N * sc->dev.planes : 0);
     if (e == cudaSuccess) e = f4.alloc(16 * N);
     if (e != cudaSuccess) return e;
     char* b = ws_mem.as<char>();
-    ws.qa = (float4*)(b + qa); ws.qb = (float4*)(b + qb); ws.hits = (uint2*)(b + hits); ws.rec = (float4*)(b + rec);
+    ws.qa = (float4*)(b + q); ws.qb = ws.qa + 3 * N; ws.hits = (uint2*)(b + hits); ws.ring = (uint2*)(b + ring); ws.rec = (float4*)(b + rec);
     ws.pinfo = (uint32_t*)(b + pinfo); ws.gradlist = (uint32_t*)(b + gl); ws.ctl = (uint32_t*)(b + ctl); ws.cap = n;
-    return cudaSuccess;
+    ws.tag = 1;
+    return cudaMemsetAsync(ws.ring, 0, 8 * N * L, stream);   // fresh memory: no entry carries tag 1
   }
 };
 
@@ -332,6 +349,7 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   if (stack_bytes + (size_t)dev.smem_nodes * sizeof(NodeC) > kMaxDynSmem)
     dev.smem_nodes = (uint32_t)((kMaxDynSmem - stack_bytes) / sizeof(NodeC));
   s->trace_smem = (size_t)dev.smem_nodes * sizeof(NodeC) + stack_bytes;
+  s->wave_ok = DR_SMEM_NODES == 0 && s->trace_smem + kWaveExtraSmem <= kMaxDynSmem;
   e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
@@ -436,13 +454,21 @@ dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_stat
   h->nblocks = (cp.N + kBlock - 1) / kBlock;
   h->state_bytes = L.total; h->state_base = dev_state;
   EvalWs& ws = h->ws;
-  ws.qa = (float4*)(b + L.qa); ws.qb = (float4*)(b + L.qb); ws.hits = (uint2*)(b + L.hits); ws.rec = (float4*)(b + L.rec);
+  ws.qa = (float4*)(b + L.q); ws.qb = ws.qa + 3 * (size_t)cp.N; ws.hits = (uint2*)(b + L.hits); ws.ring = (uint2*)(b + L.ring);
+  ws.rec = (float4*)(b + L.rec);
   ws.pinfo = (uint32_t*)(b + L.pinfo); ws.gradlist = (uint32_t*)(b + L.gradlist); ws.ctl = (uint32_t*)(b + L.ctl); ws.cap = cp.N;
   *out = h;
   return DR_OK;
 }
 
 dr_status dr_chains_destroy(dr_chains* c) { delete c; return DR_OK; }
+
+dr_status dr_chains_set_eval_form(dr_chains* c, int32_t form) {
+  if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
+  if (form < 0 || form > 2) return fail(DR_ERR_INVALID_ARG, "form must be 0, 1 or 2");
+  c->eval_form = form;
+  return DR_OK;
+}
 
 dr_status dr_chains_init(dr_chains* c, uint32_t frame_index, void* stream) {
   if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
@@ -471,15 +497,9 @@ dr_status dr_step(dr_chains* c, int32_t method, uint32_t iterations, void* strea
 dr_status dr_resolve_image(dr_chains* c, float* dev_rgb, void* stream) {
   if (!c || !dev_rgb) return fail(DR_ERR_INVALID_ARG, "null argument");
   cudaStream_t s = (cudaStream_t)stream;
-  { ProfScope ps(c, DR_PROF_RESOLVE, s); k_resolve<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, s>>>(c->cp, c->st.ctr, c->accum, dev_rgb, c->npix, 0ull, 0ull); }
+  { ProfScope ps(c, DR_PROF_RESOLVE, s); k_resolve<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, s>>>(c->cp, c->st.ctr, c->accum, dev_rgb, c->npix, 0ull, 0ull, nullptr); }
   CUDA_TRY(cudaGetLastError());
-  if (c->cp.restore) {
-    unsigned long long tours = 0;
-    CUDA_TRY(cudaMemcpyAsync(&tours, &c->st.ctr->tours, sizeof(tours), cudaMemcpyDeviceToHost, s));
-    CUDA_TRY(cudaStreamSynchronize(s));
-    if (tours == 0) { g_err = "no tour has completed yet: zero image"; return DR_WARN_NO_TOURS; }
-  }
-  return DR_OK;
+  return DR_OK;   // asynchronous: a resolve before the first completed tour writes zeros and is counted (dr_stats.no_tour_resolves)
 }
 
 dr_status dr_resolve_image_sharded(dr_chains* c, const float* dev_accum_sum, uint64_t tours_total, uint64_t mutations_total,
@@ -490,10 +510,31 @@ dr_status dr_resolve_image_sharded(dr_chains* c, const float* dev_accum_sum, uin
     ProfScope ps(c, DR_PROF_RESOLVE, (cudaStream_t)stream);
     k_resolve<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, (cudaStream_t)stream>>>(
         c->cp, c->st.ctr, (const float4*)dev_accum_sum, dev_rgb, c->npix, (unsigned long long)tours_total,
-        (unsigned long long)mutations_total);
+        (unsigned long long)mutations_total, nullptr);
   }
   CUDA_TRY(cudaGetLastError());
-  if (c->cp.restore && tours_total == 0) { g_err = "no tour has completed yet: zero image"; return DR_WARN_NO_TOURS; }
+  return DR_OK;
+}
+
+size_t dr_frame_floats(const dr_chains* c) { return c ? 4 * (size_t)c->npix + kTailFloats : 0; }
+
+dr_status dr_pack_frame(dr_chains* c, float* dev_buf, void* stream) {
+  if (!c || !dev_buf) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if ((uintptr_t)dev_buf & 15u) return fail(DR_ERR_INVALID_ARG, "dev_buf must be 16-byte aligned");
+  k_pack_frame<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, (cudaStream_t)stream>>>(c->st.ctr, c->accum, dev_buf, c->npix);
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;
+}
+
+dr_status dr_resolve_image_packed(dr_chains* c, const float* dev_buf_sum, float* dev_rgb, void* stream) {
+  if (!c || !dev_rgb || !dev_buf_sum) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if ((uintptr_t)dev_buf_sum & 15u) return fail(DR_ERR_INVALID_ARG, "dev_buf_sum must be 16-byte aligned");
+  {
+    ProfScope ps(c, DR_PROF_RESOLVE, (cudaStream_t)stream);
+    k_resolve<<<(c->npix + kBlock - 1) / kBlock, kBlock, 0, (cudaStream_t)stream>>>(
+        c->cp, c->st.ctr, (const float4*)dev_buf_sum, dev_rgb, c->npix, 0ull, 0ull, dev_buf_sum + 4 * (size_t)c->npix);
+  }
+  CUDA_TRY(cudaGetLastError());
   return DR_OK;
 }
 
@@ -525,7 +566,7 @@ dr_status dr_chains_work_stats(dr_chains* c, uint64_t* host_out3, void* stream) 
   EvalIO io = chain_io(c, false);
   io.rays_ctr = d.as<unsigned long long>(); io.nonfinite_ctr = nullptr; io.work = d.as<unsigned long long>() + 1;
   if (c->cp.grad) CUDA_TRY(cudaMemsetAsync(c->st.gy, 0, sizeof(float4) * (size_t)c->cp.planes * c->cp.N, s));
-  const dr_status r = launch_eval(nullptr, c->scene, c->ws, io, c->cp.N, c->cp.grad != 0, true, s);
+  const dr_status r = launch_eval(nullptr, c->scene, next_ws(c, s), io, c->cp.N, c->cp.grad != 0, true, 0, s);
   if (r != DR_OK) return r;
   CUDA_TRY(cudaMemcpyAsync(host_out3, d.p, 24, cudaMemcpyDeviceToHost, s));
   CUDA_TRY(cudaStreamSynchronize(s));
@@ -539,7 +580,8 @@ dr_status dr_chains_stats(dr_chains* c, dr_stats* o, void* stream) {
   CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
   o->tours = h.tours; o->mutations = h.mutations; o->rays = h.rays; o->mh_accepts = h.mh_accepts; o->nonfinite = h.nonfinite;
   o->kills_last_step = h.kills_last; o->regen_queue_len = h.queue_len; o->iteration = c->iteration;
-  o->p_lambda = h.p_lambda; o->kappa0 = h.kappa0; o->lambda = h.lambda;
+  o->p_lambda = h.p_lambda; o->kappa0 = h.kappa0; o->lambda = h.lambda; o->no_tour_resolves = h.no_tour_resolves;
+  if (h.no_tour_resolves) { g_err = "a resolve ran before any tour had completed: zero image"; return DR_WARN_NO_TOURS; }
   return DR_OK;
 }
 
@@ -658,12 +700,12 @@ dr_status dr_trace_rays(const dr_scene* sc, const float* o, const float* d, uint
 namespace {
 // Evaluates n row-major states through the wavefront path.  Any output may be null.  work3: {rays, nodes, tris} counters.
 dr_status eval_rows(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score, uint32_t* nrays,
-                    uint32_t* sig, unsigned long long* work3, cudaStream_t s) {
+                    uint32_t* sig, unsigned long long* work3, int form, cudaStream_t s) {
   const bool grad = score != nullptr;
   const uint32_t d = sc->dev.d, planes = sc->dev.planes, g = (n + 255) / 256;
   HookEval he;
   DevBuf tpix, tsig;
-  CUDA_TRY(he.setup(sc, n, grad));
+  CUDA_TRY(he.setup(sc, n, grad, s));
   CUDA_TRY(tpix.alloc(4 * (size_t)n));
   CUDA_TRY(tsig.alloc(4 * (size_t)n));
   k_rows_to_planes<<<g, 256, 0, s>>>(x, he.xpl.as<float4>(), n, d, planes);
@@ -672,7 +714,7 @@ dr_status eval_rows(const dr_scene* sc, const float* x, uint32_t n, float* f, fl
   io.x = he.xpl.as<float4>(); io.stride = n; io.order = nullptr; io.g = he.gpl.as<float4>(); io.f = he.f4.as<float4>();
   io.pix = pix ? pix : tpix.as<uint32_t>(); io.sig = sig ? sig : tsig.as<uint32_t>(); io.nrays = nrays;
   io.rays_ctr = work3; io.nonfinite_ctr = nullptr; io.work = work3 ? work3 + 1 : nullptr;
-  const dr_status r = launch_eval(nullptr, sc, he.ws, io, n, grad, work3 != nullptr, s);
+  const dr_status r = launch_eval(nullptr, sc, he.ws, io, n, grad, work3 != nullptr, form, s);
   if (r != DR_OK) return r;
   if (f || p) k_fp_split<<<g, 256, 0, s>>>(he.f4.as<float4>(), p, f, n);
   if (grad) k_planes_to_rows<<<g, 256, 0, s>>>(he.gpl.as<float4>(), score, n, d, planes);
@@ -684,10 +726,16 @@ dr_status eval_rows(const dr_scene* sc, const float* x, uint32_t n, float* f, fl
 
 dr_status dr_eval_states(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score,
                          uint32_t* nrays, uint32_t* sig, void* stream) {
+  return dr_eval_states_form(sc, x, n, f, p, pix, score, nrays, sig, 0, stream);
+}
+
+dr_status dr_eval_states_form(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score,
+                              uint32_t* nrays, uint32_t* sig, int32_t form, void* stream) {
   if (!sc) return fail(DR_ERR_INVALID_ARG, "null scene");
+  if (form < 0 || form > 2) return fail(DR_ERR_INVALID_ARG, "form must be 0, 1 or 2");
   if (!n) return DR_OK;  // empty input
   if (!x || !f || !p || !pix || !nrays || !sig) return fail(DR_ERR_INVALID_ARG, "null argument");
-  return eval_rows(sc, x, n, f, p, pix, score, nrays, sig, nullptr, (cudaStream_t)stream);
+  return eval_rows(sc, x, n, f, p, pix, score, nrays, sig, nullptr, form, (cudaStream_t)stream);
 }
 
 dr_status dr_eval_work_stats(const dr_scene* sc, const float* x, uint32_t n, uint64_t* dev_out3, void* stream) {
@@ -695,7 +743,7 @@ dr_status dr_eval_work_stats(const dr_scene* sc, const float* x, uint32_t n, uin
   if (!n) return DR_OK;
   if (!x || !dev_out3) return fail(DR_ERR_INVALID_ARG, "null argument");
   if (sc->dev.analytic) return DR_OK;
-  return eval_rows(sc, x, n, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, (unsigned long long*)dev_out3, (cudaStream_t)stream);
+  return eval_rows(sc, x, n, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, (unsigned long long*)dev_out3, 0, (cudaStream_t)stream);
 }
 
 dr_status dr_philox_blocks(uint64_t seed, const uint32_t* ctr, uint32_t n, uint32_t* out, void* stream) {

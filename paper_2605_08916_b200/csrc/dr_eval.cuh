@@ -52,17 +52,22 @@ constexpr int kCtlHead = 20;   // head[k]: fetch counter of k_trace for segment 
 constexpr int kCtlGrad = 40;   // states on the reverse-pass list
 constexpr int kCtlWords = 64;
 
-// Workspace for up to `cap` states.  A ray-queue entry is three float4 (planes of `cap` entries):
-//   Q0 = (o.xyz, bits(state)), Q1 = (d.xyz, bits(path signature)), Q2 = (T.rgb, bits(refract mask | has_ggx << 16)).
+// Workspace for up to `cap` states.  Two forms of the same evaluation use it (same results, state by state):
+//  * per-segment loop (k_trace / k_shade): ray queues qa, qb; an entry is three float4 in planes of `cap` entries,
+//      Q0 = (o.xyz, bits(state)), Q1 = (d.xyz, bits(path signature)), Q2 = (T.rgb, bits(refract mask | has_ggx << 16));
+//  * k_wave (dr_wave.cuh): the same three words live in a 64-byte record per STATE (rayrec[4 s + 0..2], the memory of
+//      qa | qb), and `ring` holds one 8-byte entry per ray: (state | (k - 1) << 27, tag of this evaluation).
 struct EvalWs {
-  float4* qa;          // 3 * cap
+  float4* qa;          // 3 * cap; qb = qa + 3 * cap (one allocation of 6 * cap float4: k_wave uses the first 4 * cap as records)
   float4* qb;          // 3 * cap
-  uint2* hits;         // cap: (bits(t), triangle in leaf order or kMiss)
+  uint2* hits;         // cap: (bits(t), triangle in leaf order or kMiss)   (loop form)
+  uint2* ring;         // L * cap ray entries, written once per evaluation, never reused                 (k_wave)
   float4* rec;         // L * cap (score only): incoming direction and triangle of vertex k of state s at [k * cap + s]
   uint32_t* pinfo;     // cap (score only): refract mask | rays << 16 of the finished path
   uint32_t* gradlist;  // cap (score only)
   uint32_t* ctl;       // kCtlWords
   uint32_t cap;
+  uint32_t tag;        // k_wave: tag of this evaluation, != 0; ring entries of earlier evaluations carry other tags
 };
 
 // Inputs and outputs of one evaluation, all indexed by state s (planes: [plane * stride + s]).
@@ -89,17 +94,27 @@ __device__ __forceinline__ void g_pair(const EvalIO& io, uint32_t s, uint32_t k,
 }
 
 // ---- a3: camera rays -------------------------------------------------------------------------------------------
+// WAVE: the ray goes into the state's record and ring entry t (dr_wave.cuh); otherwise into slot t of queue qa.
+constexpr int kCtlWaveReserve = 48, kCtlWaveHead = 50, kCtlWaveDone = 51;   // control words of k_wave
+template <bool WAVE>
 __global__ void __launch_bounds__(kShadeBlock) k_raygen(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
   const uint32_t t = blockIdx.x * kShadeBlock + threadIdx.x;
-  if (t == 0) ws.ctl[kCtlCnt + 1] = n;
+  if (t == 0) ws.ctl[WAVE ? kCtlWaveReserve : kCtlCnt + 1] = n;
   if (t >= n) return;
   const uint32_t s = io.order ? io.order[t] : t;
   const float4 x = io.x[s];
   io.pix[s] = pixel_of(x.x, x.y, sc.W, sc.H);
   const V3<float> d = camera_dir<float>(sc, x.x, x.y);
-  ws.qa[t] = make_float4(sc.cam_pos[0], sc.cam_pos[1], sc.cam_pos[2], __uint_as_float(s));
-  ws.qa[(size_t)ws.cap + t] = make_float4(d.x, d.y, d.z, __uint_as_float(kSigInit));
-  ws.qa[2 * (size_t)ws.cap + t] = make_float4(1.f, 1.f, 1.f, __uint_as_float(0u));
+  const float4 q0 = make_float4(sc.cam_pos[0], sc.cam_pos[1], sc.cam_pos[2], __uint_as_float(s));
+  const float4 q1 = make_float4(d.x, d.y, d.z, __uint_as_float(kSigInit));
+  const float4 q2 = make_float4(1.f, 1.f, 1.f, __uint_as_float(0u));
+  if (WAVE) {
+    float4* r = ws.qa + 4 * (size_t)s;
+    r[0] = q0; r[1] = q1; r[2] = q2;
+    ws.ring[t] = make_uint2(s, ws.tag);   // segment 1
+  } else {
+    ws.qa[t] = q0; ws.qa[(size_t)ws.cap + t] = q1; ws.qa[2 * (size_t)ws.cap + t] = q2;
+  }
 }
 
 // ---- a4: closest hit, persistent ---------------------------------------------------------------------------------
@@ -119,7 +134,7 @@ struct SmemTriStack {
 
 __device__ __forceinline__ void tri_one(const DevScene& sc, TravRay& r, TravState& s) {
   const uint32_t li = trav_next_tri(s);
-  tri_test(__ldg(&sc.tris[3 * li]), __ldg(&sc.tris[3 * li + 1]), __ldg(reinterpret_cast<const float2*>(&sc.tris[3 * li + 2])), li, r);
+  tri_test_bf(__ldg(&sc.tris[3 * li]), __ldg(&sc.tris[3 * li + 1]), __ldg(reinterpret_cast<const float2*>(&sc.tris[3 * li + 2])), li, true, r);
 }
 
 // One prefetched triangle of a lane: its three words are requested one step before they are tested.
@@ -139,6 +154,15 @@ struct TravLane {
   int tsp;                       // postponed triangle groups
   bool active, has_node;
 };
+
+__device__ __forceinline__ void trav_lane_init(TravLane& L, uint32_t one) {   // an idle lane
+  L.active = false; L.has_node = false; L.tsp = 0;
+  trav_setup(L.r, 0.f, 0.f, 0.f, 1.f, 1.f, 1.f, one);
+  trav_begin(L.s);
+  L.w0 = L.w1 = L.w2 = L.w3 = L.w4 = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+  for (int it = 0; it < kTrisPerStep; ++it) { L.tri[it].li = kMiss; L.tri[it].t0 = L.tri[it].t1 = make_float4(0.f, 0.f, 0.f, 0.f); L.tri[it].t2 = make_float2(0.f, 0.f); }
+}
 
 template <bool STATS>
 __device__ __forceinline__ bool trav_step(const DevScene& sc, const uint4* smem, SmemStack& st, SmemTriStack& tst, TravLane& L,
@@ -255,21 +279,13 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr unsigned kFull = 0xFFFFFFFFu;
   uint32_t wnext = 0, wend = 0;  // this warp's private range of the queue
-  bool drained = false, active = false, has_node = false;
-  TravRay r;
-  TravState s;
-  uint4 w0, w1, w2, w3, w4;      // words of the node to test next (valid if has_node)
-  TriSlot tri[kTrisPerStep];
-  int tsp = 0;  // postponed triangle groups
+  bool drained = false;
+  TravLane L;
   uint32_t ridx = 0, nn = 0, nt = 0;
-  trav_setup(r, 0.f, 0.f, 0.f, 1.f, 1.f, 1.f, one);
-  trav_begin(s);
-  w0 = w1 = w2 = w3 = w4 = make_uint4(0u, 0u, 0u, 0u);
-#pragma unroll
-  for (int it = 0; it < kTrisPerStep; ++it) { tri[it].li = kMiss; tri[it].t0 = tri[it].t1 = make_float4(0.f, 0.f, 0.f, 0.f); tri[it].t2 = make_float2(0.f, 0.f); }
+  trav_lane_init(L, one);
   for (;;) {
     // ---- hand rays to the idle lanes
-    unsigned want = __ballot_sync(kFull, !active);
+    unsigned want = __ballot_sync(kFull, !L.active);
     while (want && !drained) {
       if (wnext == wend) {
         uint32_t b = 0;
@@ -284,98 +300,23 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
       if (mine) {
         ridx = wnext + rank;
         const float4 o = q[ridx], d = q[(size_t)cap + ridx];
-        trav_setup(r, o.x, o.y, o.z, d.x, d.y, d.z, one);
-        trav_begin(s);   // one work bit: the root, requested by part N of the first step
-        tsp = 0;
-        active = true;
+        trav_setup(L.r, o.x, o.y, o.z, d.x, d.y, d.z, one);
+        trav_begin(L.s);   // one work bit: the root, requested by part N of the first step
+        L.tsp = 0;
+        L.active = true;
       }
       const unsigned got = __ballot_sync(kFull, mine);
       wnext += __popc(got);
       want &= ~got;
     }
-    unsigned act = __ballot_sync(kFull, active);
+    unsigned act = __ballot_sync(kFull, L.active);
     if (!act) break;
     // ---- lockstep traversal
     do {
-      // The four parts are written without branches (selects and predicated loads / stores) so that the compiler can
-      // interleave their dependency chains: with branches around every part each warp waited out the fixed latencies
-      // of its bookkeeping one after the other (profiles/r01f_k_trace_full.md, step r01e: 53 % of the instructions took 78 % of the time).
-      // A: node test
-      {
-        if (STATS) nn += has_node ? 1u : 0u;
-        uint32_t h = node_hits(w0, w1, w2, w3, w4, r);
-        h = has_node ? h : 0u;
-        const uint32_t nty = h & 0x00FFFFFFu;
-        const bool newtri = nty != 0u;
-        bool keep_old = newtri && s.ty != 0u;  // triangles still pending from an earlier node: postpone them
-        if (keep_old && tsp >= kTriStack) {    // (or test them now if their stack is full: rare)
-          while (s.ty) { if (STATS) ++nt; tri_one(sc, r, s); }
-          keep_old = false;
-        }
-        if (keep_old) tst.push(tsp, s);
-        tsp += keep_old ? 1 : 0;
-        s.tx = newtri ? w1.y : s.tx;
-        s.ty = newtri ? nty : s.ty;
-        s.tm = newtri ? w1.z : s.tm;
-        s.gx = has_node ? w1.x : s.gx;
-        s.gy = has_node ? ((h & 0xFF000000u) | w1.w) : s.gy;
-      }
-      // N: next node
-      {
-        const bool popn = active && !(s.gy & 0xFF000000u) && s.sp > 0;
-        s.sp -= popn ? 1 : 0;
-        if (popn) { const uint2 e = st.pop(s.sp); s.gx = e.x; s.gy = e.y; }
-        const bool go = active && (s.gy & 0xFF000000u) != 0u;
-        const uint32_t bit = top_bit(s.gy | 0x01000000u);
-        const uint32_t rest = s.gy & ~(1u << bit);
-        const bool keep = go && (rest & 0xFF000000u) != 0u;
-        if (keep) st.push(s.sp, make_uint2(s.gx, rest));
-        s.sp += keep ? 1 : 0;
-        const uint32_t slot = (bit - 24u) ^ (r.octinv4 & 7u);
-        const uint32_t node = s.gx + popc32(rest & ~(0xFFFFFFFFu << slot) & 0xFFu);
-        s.gy = go ? rest : s.gy;
-        if (go) {
-#if DR_SMEM_NODES == 0
-          const uint4* np = sc.nodes + 5u * (size_t)node;
-          w0 = DR_NODE_LD(np); w1 = DR_NODE_LD(np + 1); w2 = DR_NODE_LD(np + 2); w3 = DR_NODE_LD(np + 3); w4 = DR_NODE_LD(np + 4);
-#else
-          const uint4* np = node < sc.smem_nodes ? smem + 5u * node : sc.nodes + 5u * (size_t)node;
-          w0 = np[0]; w1 = np[1]; w2 = np[2]; w3 = np[3]; w4 = np[4];
-#endif
-        }
-        has_node = go;
-      }
-      // T: triangle tests
-#pragma unroll
-      for (int it = 0; it < kTrisPerStep; ++it) {
-        const bool valid = tri[it].li != kMiss;
-        if (STATS) nt += valid ? 1u : 0u;
-        tri_test_bf(tri[it].t0, tri[it].t1, tri[it].t2, tri[it].li, valid, r);  // reads every loaded word (dr_types.h TriPacked)
-      }
-      // F: next triangles
-      {
-        bool have_any = false;
-#pragma unroll
-        for (int it = 0; it < kTrisPerStep; ++it) {
-          const bool popt = active && s.ty == 0u && tsp > 0;
-          tsp -= popt ? 1 : 0;
-          if (popt) tst.pop(tsp, s);
-          const bool have = active && s.ty != 0u;
-          const uint32_t b = low_bit(s.ty | 0x80000000u);
-          const uint32_t li = s.tx + popc32(s.tm & ~(0xFFFFFFFFu << b));
-          s.ty = have ? (s.ty & (s.ty - 1u)) : s.ty;
-          tri[it].li = have ? li : kMiss;
-          if (have) {
-            const float4* p = sc.tris + 3 * (size_t)li;
-            tri[it].t0 = DR_TRI_LD(p); tri[it].t1 = DR_TRI_LD(p + 1); tri[it].t2 = DR_TRI_LD(reinterpret_cast<const float2*>(p + 2));
-          }
-          have_any = have_any || have;
-        }
-        const bool done = active && !(has_node || have_any);  // nothing requested, nothing pending: the ray is finished
-        if (done) hits[ridx] = make_uint2(__float_as_uint(r.t), r.li);
-        active = active && !done;
-      }
-      act = __ballot_sync(kFull, active);
+      const bool done = trav_step<STATS>(sc, smem, st, tst, L, nn, nt);
+      if (done) hits[ridx] = make_uint2(__float_as_uint(L.r.t), L.r.li);
+      L.active = L.active && !done;
+      act = __ballot_sync(kFull, L.active);
     } while (drained ? act != 0u : __popc(act) >= kRefillBelow);
   }
   if (STATS) {
@@ -421,7 +362,10 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
         sig = fnv(sig, 5u);
       }
     } else if (k < sc.L) {
-      const float3 hit = o + d * __uint_as_float(h.x);
+      // hit point on the triangle's plane, t = ((v0 - o).n) / (d.n): the traversal's t decided WHICH triangle
+      const float3 nn = fr.nf * (dn < 0.f ? 1.f : -1.f);   // the geometric normal n again (exact: * +-1)
+      const float tp = dot3(xyz(t0) - o, nn) / dot3(d, nn);
+      const float3 hit = o + d * tp;
       const float2 u = x_pair(io, s, k);
       if (GRAD) ws.rec[(size_t)k * cap + s] = make_float4(d.x, d.y, d.z, __uint_as_float(li));
       V3<float> din{d.x, d.y, d.z}, dnew;

@@ -13,7 +13,7 @@ constexpr int kBlock = 256;      // streaming kernels
 
 struct Counters {
   unsigned long long tours, mutations, rays, mh_accepts, nonfinite;
-  uint32_t kills_last, queue_len, iteration, pad;
+  uint32_t kills_last, queue_len, iteration, no_tour_resolves;
   float p_lambda, kappa0, lambda, pad2;
   double psum;
 };
@@ -144,10 +144,10 @@ __global__ void __launch_bounds__(kBlock) k_bootstrap(ChainParams cp, ChainState
   }
 }
 
-__device__ __forceinline__ float log_q_plane(float4 a, float4 ga, float4 b, float h) {
+__device__ __forceinline__ float log_q_plane(float acc, float4 a, float4 ga, float4 b, float h) {   // acc += |delta|^2, coordinate by coordinate
   const float d0 = min_image(b.x - a.x - h * ga.x), d1 = min_image(b.y - a.y - h * ga.y);
   const float d2 = min_image(b.z - a.z - h * ga.z), d3 = min_image(b.w - a.w - h * ga.w);
-  return d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3;
+  return (((acc + d0 * d0) + d1 * d1) + d2 * d2) + d3 * d3;
 }
 
 // a11: warp-aggregated vector atomic.  Lanes that splat to the same pixel are summed first, then one
@@ -192,8 +192,8 @@ __global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st
         for (uint32_t j = 0; j < cp.planes; ++j) {
           const size_t at = (size_t)j * cp.N + i;
           const float4 x = st.x[at], y = st.y[at], gx = st.g[at], gy = st.gy[at];
-          bwd += log_q_plane(y, gy, x, cp.half_s2);
-          fwd += log_q_plane(x, gx, y, cp.half_s2);
+          bwd = log_q_plane(bwd, y, gy, x, cp.half_s2);
+          fwd = log_q_plane(fwd, x, gx, y, cp.half_s2);
         }
         const float den = 2.0f * cp.stddev * cp.stddev;
         a *= expf((-bwd / den) - (-fwd / den));
@@ -295,18 +295,38 @@ __global__ void __launch_bounds__(kBlock) k_scatter(ChainParams cp, ChainState s
   }
 }
 
-// a12: Alg. 3 with the pixel-count factor (Q2); plain MH: p_lambda / N_mut.  ext_* != 0: use externally
-// reduced totals (sharded runs) instead of this shard's counters.
-__global__ void __launch_bounds__(kBlock) k_resolve(ChainParams cp, const Counters* c, const float4* accum, float* rgb,
-                                                    uint32_t npix, unsigned long long ext_tours, unsigned long long ext_mut) {
+// a12: Alg. 3 with the pixel-count factor (Q2); plain MH: p_lambda / N_mut.  Totals: this shard's counters, or
+// (sharded runs) externally reduced ones: ext_* != 0, or `tail` = the eight floats behind an all-reduced
+// packed frame (k_pack_frame).
+constexpr int kTailFloats = 8;
+__device__ __forceinline__ unsigned long long limbs_to_u64(const float* t) {   // four sums of 16-bit limbs, each < 2^24: exact in fp32
+  return (unsigned long long)t[0] + ((unsigned long long)t[1] << 16) + ((unsigned long long)t[2] << 32) + ((unsigned long long)t[3] << 48);
+}
+__global__ void __launch_bounds__(kBlock) k_resolve(ChainParams cp, Counters* c, const float4* accum, float* rgb,
+                                                    uint32_t npix, unsigned long long ext_tours, unsigned long long ext_mut,
+                                                    const float* tail) {
   const uint32_t q = blockIdx.x * kBlock + threadIdx.x;
   if (q >= npix) return;
-  const unsigned long long tours = ext_mut ? ext_tours : c->tours, mut = ext_mut ? ext_mut : c->mutations;
+  unsigned long long tours = c->tours, mut = c->mutations;
+  if (tail) { tours = limbs_to_u64(tail); mut = limbs_to_u64(tail + 4); }
+  else if (ext_mut) { tours = ext_tours; mut = ext_mut; }
+  if (q == 0 && cp.restore && tours == 0) c->no_tour_resolves += 1;   // zero image, no division; reported by dr_chains_stats
   float scale;
   if (cp.restore) scale = tours ? (float)npix * c->kappa0 / (float)tours : 0.f;
   else scale = mut ? (float)npix * c->p_lambda / (float)mut : 0.f;
   const float4 a = accum[q];
   rgb[3 * q] = scale * a.x; rgb[3 * q + 1] = scale * a.y; rgb[3 * q + 2] = scale * a.z;
+}
+
+// Sharded runs: one buffer per frame for ONE all-reduce(sum): the accumulation buffer followed by tourCount and the
+// mutation count as 16-bit limbs in floats (sums over <= 256 ranks stay below 2^24, hence exact).
+__global__ void __launch_bounds__(kBlock) k_pack_frame(const Counters* c, const float4* accum, float* buf, uint32_t npix) {
+  const uint32_t q = blockIdx.x * kBlock + threadIdx.x;
+  if (q < npix) reinterpret_cast<float4*>(buf)[q] = accum[q];
+  if (q < (uint32_t)kTailFloats) {
+    const unsigned long long v = q < 4 ? c->tours : c->mutations;
+    buf[4 * (size_t)npix + q] = (float)((v >> (16 * (q & 3u))) & 0xFFFFull);
+  }
 }
 
 // ---- test hooks -------------------------------------------------------------------------------------------

@@ -1,3 +1,7 @@
+// Arithmetic note: the library is compiled with -fmad=false (build.py), and the value formulas below are written in the
+// operation order of DESIGN.md Q4-Q8, so that a path's hit points, directions and weights round exactly as a plain fp32
+// evaluation of those formulas does; only sincosf / logf (a few ulps) can differ.  Near-threshold decisions (which facet
+// an edge-grazing ray hits) then fall the same way on both sides of a parity check (Q15).
 // Target evaluation on the device, per-vertex pieces: x -> (f, p, pixel, score)  (rows a3, a5, a6).
 //   a3 camera ray and direction sampling at a vertex, a5 throughput / emission, a6 the local Jacobians of the
 //   reverse pass (forward-mode numbers with a handful of tangents).  The wavefront kernels that call these are
@@ -63,20 +67,35 @@ template <int K> __device__ __forceinline__ Du<K> operator/(Du<K> a, Du<K> b) {
   return r;
 }
 template <int K> __device__ __forceinline__ Du<K> operator/(float a, Du<K> b) { return du_const<K>(a) / b; }
+template <int K> __device__ __forceinline__ Du<K> operator/(Du<K> a, float b) { Du<K> r; r.v = a.v / b; for (int i = 0; i < K; ++i) r.d[i] = a.d[i] / b; return r; }
 template <int K> __device__ __forceinline__ Du<K> sqrt_t(Du<K> a) {
   Du<K> r; r.v = sqrtf(a.v); const float k = a.v > 0.f ? 0.5f / r.v : 0.f;
   for (int i = 0; i < K; ++i) r.d[i] = a.d[i] * k;
   return r;
 }
+#ifndef DR_SINCOS_F64
+#define DR_SINCOS_F64 0
+#endif
+// sin and cos of an angle in [0, 2 pi).  DR_SINCOS_F64: evaluated in double and rounded once, i.e. the correctly rounded
+// fp32 values (what a good host libm returns); otherwise sincosf (2 ulp).
+__device__ __forceinline__ void sincos_f(float a, float* s, float* c) {
+#if DR_SINCOS_F64
+  double sd, cd;
+  sincos((double)a, &sd, &cd);
+  *s = (float)sd; *c = (float)cd;
+#else
+  sincosf(a, s, c);
+#endif
+}
 template <int K> __device__ __forceinline__ void sincos_t(Du<K> a, Du<K>& s, Du<K>& c) {
-  float sv, cv; sincosf(a.v, &sv, &cv);
+  float sv, cv; sincos_f(a.v, &sv, &cv);
   s.v = sv; c.v = cv;
   for (int i = 0; i < K; ++i) { s.d[i] = a.d[i] * cv; c.d[i] = -a.d[i] * sv; }
 }
 template <int K> __device__ __forceinline__ float val(Du<K> a) { return a.v; }
 template <int K> __device__ __forceinline__ Du<K> clamp0(Du<K> a) { return a.v < 0.f ? du_const<K>(0.f) : a; }
 __device__ __forceinline__ float sqrt_t(float a) { return sqrtf(a); }
-__device__ __forceinline__ void sincos_t(float a, float& s, float& c) { sincosf(a, &s, &c); }
+__device__ __forceinline__ void sincos_t(float a, float& s, float& c) { sincos_f(a, &s, &c); }
 __device__ __forceinline__ float val(float a) { return a; }
 __device__ __forceinline__ float clamp0(float a) { return a < 0.f ? 0.f : a; }
 
@@ -132,8 +151,8 @@ template <class T> __device__ __forceinline__ V3<T> dielectric_dir(const Frame& 
     r.x = d.x + k * fr.nf.x; r.y = d.y + k * fr.nf.y; r.z = d.z + k * fr.nf.z;
   } else {
     const float ie = 1.0f / eta;
-    const T ct = sqrt_t(1.0f - (1.0f - cos_i * cos_i) * (ie * ie));
-    const T k = cos_i * ie - ct;
+    const T ct = sqrt_t(1.0f - (1.0f - cos_i * cos_i) / (eta * eta));
+    const T k = cos_i / eta - ct;
     r.x = d.x * ie + k * fr.nf.x; r.y = d.y * ie + k * fr.nf.y; r.z = d.z * ie + k * fr.nf.z;
   }
   return r;
@@ -162,8 +181,7 @@ template <class T> __device__ __forceinline__ bool ggx_dir(const Frame& fr, floa
   wi.x = hm.x * k2 - wo.x; wi.y = hm.y * k2 - wo.y; wi.z = hm.z * k2 - wo.z;
   if (!(val(wi.z) > 0.f)) return false;
   const T c1 = 1.0f - woh;
-  const T c2 = c1 * c1;
-  c5 = c2 * c2 * c1;
+  c5 = c1 * c1 * c1 * c1 * c1;
   G1 = (wi.z * 2.0f) / (wi.z + sqrt_t((wi.x * wi.x + wi.y * wi.y) * (al * al) + wi.z * wi.z));
   out = from_frame<T>(fr, wi.x, wi.y, wi.z);
   return true;
@@ -173,9 +191,9 @@ template <class T> __device__ __forceinline__ V3<T> camera_dir(const DevScene& s
   const T sx = (x0 * 2.0f - 1.0f) * sc.tan_half_aspect;
   const T sy = (x1 * 2.0f - 1.0f) * sc.tan_half;
   V3<T> v;
-  v.x = sx * sc.cam_r[0] - sy * sc.cam_v[0] + sc.cam_w[0];
-  v.y = sx * sc.cam_r[1] - sy * sc.cam_v[1] + sc.cam_w[1];
-  v.z = sx * sc.cam_r[2] - sy * sc.cam_v[2] + sc.cam_w[2];
+  v.x = (sc.cam_w[0] + sx * sc.cam_r[0]) - sy * sc.cam_v[0];
+  v.y = (sc.cam_w[1] + sx * sc.cam_r[1]) - sy * sc.cam_v[1];
+  v.z = (sc.cam_w[2] + sx * sc.cam_r[2]) - sy * sc.cam_v[2];
   const T inv = 1.0f / sqrt_t(dott(v, v));
   v.x = v.x * inv; v.y = v.y * inv; v.z = v.z * inv;
   return v;

@@ -33,6 +33,19 @@ def allreduce_totals(accum: torch.Tensor, tours: int, mutations: int):
     return acc, int(cnt[0].item()), int(cnt[1].item())
 
 
-def allreduce_frame(accum: torch.Tensor, chains):
-    st = chains.stats()
-    return allreduce_totals(accum, st["tours"], st["mutations"])
+def resolve_frame(chains):
+    """One sharded frame's exchange: dr_pack_frame, ONE all-reduce(sum), dr_resolve_image_packed.  No host synchronisation:
+    the counters travel as 16-bit limbs in the tail of the same fp32 buffer (exact for up to 256 ranks)."""
+    buf = chains.pack_frame()
+    if dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(buf, op=dist.ReduceOp.SUM)
+    return chains.resolve_packed(buf)
+
+
+def limbs(value: int) -> list:
+    """The four 16-bit limbs of a counter, as the floats k_pack_frame writes (host mirror for the tests)."""
+    return [float((int(value) >> (16 * k)) & 0xFFFF) for k in range(4)]
+
+
+def from_limbs(t) -> int:
+    return sum(int(round(float(v))) << (16 * k) for k, v in enumerate(t))

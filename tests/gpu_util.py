@@ -41,3 +41,48 @@ def compare_states(gs, os_, g_last, o_last, stddev, check_score=True):
 def oracle_chains(desc, method, n, seed, prec=O.F32, **kw):
     sc = O.Scene(desc, prec)
     return sc, O.Chains(sc, method, n, seed=seed, **kw)
+
+
+def splats(state, last):
+    """Per-chain splat of the last Accumulate (Alg. 1 L522-L525 + the ratio channel of Q12): (pixel, [w f/p_hat, w/p_hat])."""
+    _, w = last
+    w = np.asarray(w, dtype=np.float64)
+    p = np.asarray(state["p"], dtype=np.float64)
+    on = p > 0
+    v = np.concatenate([w[:, None] * np.asarray(state["fop"], dtype=np.float64), (w / (p + 1e-8))[:, None]], axis=1)
+    return state["pix"], v * on[:, None]
+
+
+def accum_without(accum, state, last, mask):
+    """accum (npix x 4, float64) minus the splats of the chains in `mask`."""
+    pix, v = splats(state, last)
+    out = np.array(accum, dtype=np.float64)
+    np.subtract.at(out, pix[mask], v[mask])
+    return out
+
+
+def largest_addend(state, last, npix):
+    """Per pixel, the largest |splat| component that went into it (scale of the fp32 rounding of its atomic sum)."""
+    pix, v = splats(state, last)
+    out = np.zeros(npix)
+    np.maximum.at(out, pix, np.abs(v).max(1))
+    return out
+
+
+def compare_bulk(gch, och, gs, os_, g_last, o_last, div, tours_g, tours_o):
+    """Queue, tourCount delta and accumulation buffer of one teacher-forced step, with the diverged chains masked out
+    (their own splats subtracted on each side) instead of skipping the comparison."""
+    keep = ~div
+    gq, oq = gch.queue(), och.queue()
+    assert np.array_equal(gq[keep[gq]], oq[keep[oq]])                                   # regeneration queue: bit-exact, ascending
+    assert np.array_equal(gq, np.flatnonzero(gs["killed"])) and np.array_equal(oq, np.flatnonzero(os_["killed"]))
+    assert tours_g - int(gs["killed"][div].sum()) == tours_o - int(os_["killed"][div].sum())
+    npix = gch.scene.npix
+    ga = accum_without(gch.accum.cpu().numpy(), gs, g_last, div)
+    oa = accum_without(och.accum(), os_, o_last, div)
+    # per pixel: 1e-4 relative + rounding of an fp32 atomic sum (a few ulps of the largest addend per addend)
+    big = np.maximum(largest_addend(gs, g_last, npix), largest_addend(os_, o_last, npix))
+    cnt = np.bincount(os_["pix"], minlength=npix) + 2
+    tol = 1e-4 * np.abs(oa) + (4e-7 * cnt * big)[:, None] + 1e-30
+    bad = np.abs(ga - oa) > tol
+    assert not bad.any(), (int(bad.sum()), float((np.abs(ga - oa) / tol).max()))

@@ -6,7 +6,7 @@ from dr_inputs import scenes as S
 
 pytestmark = pytest.mark.gpu
 
-from gpu_util import METHODS, compare_states, min_image  # noqa: E402
+from gpu_util import METHODS, compare_bulk, compare_states, min_image  # noqa: E402
 
 
 @pytest.fixture(scope="module")
@@ -36,7 +36,35 @@ def test_philox_bit_exact(dr, oracle, torch_):
         for k in range(0, 5000, 7):
             want = oracle.philox([seed & 0xFFFFFFFF, seed >> 32], ctr[k])
             assert (got[k] == want).all()
-    # three-way: cuRAND's own Philox4x32-10 is checked against the same words in test_gpu_curand.py if nvcc is present
+
+
+def test_philox_three_way_with_curand(dr, oracle, torch_, tmp_path):
+    """SURVEY.md 8c pin: the kernels' generator, the oracle's and cuRAND's own device function (curand_philox4x32_x.h,
+    compiled here into a test-only library) give the same words for the same (key, counter)."""
+    import ctypes
+    import os
+    import shutil
+    import subprocess
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    assert os.path.exists(nvcc), "nvcc is part of the image"
+    so = str(tmp_path / "curand_check.so")
+    src = os.path.join(os.path.dirname(os.path.abspath(__file__)), "curand_check.cu")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O2", "-shared", "-Xcompiler", "-fPIC", "-o", so, src], check=True)
+    lib = ctypes.CDLL(so)
+    lib.curand_philox_blocks.argtypes = [ctypes.c_uint64, ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p]
+    rng = np.random.default_rng(5)
+    ctr = rng.integers(0, 2**32, size=(4096, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0
+    ctr[1] = 0xFFFFFFFF
+    dctr = torch_.from_numpy(ctr.view(np.int32)).cuda()
+    for seed in (0, 0xFFFFFFFFFFFFFFFF, 0x0123456789ABCDEF):
+        ours = dr.philox_blocks(seed, dctr).cpu().numpy().view(np.uint32)
+        theirs = torch_.empty_like(dctr)
+        assert lib.curand_philox_blocks(seed, dctr.data_ptr(), len(ctr), theirs.data_ptr()) == 0
+        theirs = theirs.cpu().numpy().view(np.uint32)
+        assert np.array_equal(ours, theirs)
+        for k in range(0, len(ctr), 97):
+            assert (theirs[k] == oracle.philox([seed & 0xFFFFFFFF, seed >> 32], ctr[k])).all()
 
 
 def test_rng_transforms(dr, oracle, torch_):
@@ -88,6 +116,62 @@ def test_trace_degenerate_rays(dr, oracle, torch_):
     assert t0.numel() == 0
 
 
+def _tri_soup(n, seed):
+    rng = np.random.default_rng(seed)
+    c = rng.uniform(0, 4, size=(n, 1, 3))
+    v = (c + rng.uniform(-0.4, 0.4, size=(n, 3, 3))).astype(np.float32)
+    return v
+
+
+def test_tie_rule_coincident_triangles(dr, oracle, torch_):
+    """Q8: equal t -> smaller triangle index.  Every triangle of a soup exists twice (ids i and a shuffled partner): the
+    two copies give bit-identical t on either side, so the winner is decided by the tie rule alone, and the oracle's
+    brute force names it."""
+    n = 600
+    v = _tri_soup(n, 1)
+    perm = np.random.default_rng(2).permutation(n)
+    verts = np.concatenate([v, v[perm]]).reshape(-1, 3)                 # ids n + j duplicate id perm[j]
+    idx = np.arange(6 * n, dtype=np.uint32).reshape(-1, 3)
+    desc = S.SceneDesc(verts, idx, np.zeros(2 * n, np.uint32), np.stack([S.material(S.MAT_LAMBERT, (0.5,) * 3)]), max_path_len=2)
+    o, d = S.seeded_rays(desc, 40000, 3)
+    t, prim = dr.Scene(desc).trace_rays(torch_.from_numpy(o).cuda(), torch_.from_numpy(d).cuda())
+    t, prim = t.cpu().numpy(), prim.cpu().numpy()
+    ot, otri = oracle.Scene(desc, oracle.F32).trace(o, d, brute=True)
+    assert (otri[otri >= 0] < n).all()                                  # the oracle follows the rule
+    hit = otri >= 0
+    assert hit.sum() > 5000
+    assert (prim[hit] < n).all()                                        # never the duplicate with the larger id
+    mism = prim != otri
+    assert mism.mean() < 1e-4, mism.sum()
+    ok = ~mism & hit
+    assert np.all(np.abs(t[ok] - ot[ok]) <= 2e-6 * np.abs(ot[ok]))
+
+
+def test_tie_rule_coplanar_box_on_floor(dr, oracle, torch_):
+    """A box standing on the floor: its bottom face is coplanar with the floor (the configuration commit 6a75dbf took
+    out of ggx_room).  Different triangles in one plane give t that differ by rounding, so either may win; what must
+    hold: same t as the oracle to 1e-5, and where the triangle differs both are faces of that plane."""
+    mesh = S._Mesh()
+    mesh.quad((0, 0, 0), (0, 0, 4), (4, 0, 4), (4, 0, 0), 0, div=2)     # floor, 8 triangles (ids 0-7)
+    S._box_faces(mesh, (2.0, 0.5, 2.0), (0.75, 0.5, 0.75), np.eye(3), 0)  # ids 8-19; face k = ids 8 + 2k, 9 + 2k; k = 3 is -y
+    v, i, m = mesh.finish()
+    desc = S.SceneDesc(v, i, m, np.stack([S.material(S.MAT_LAMBERT, (0.5,) * 3)]), max_path_len=2)
+    rng = np.random.default_rng(4)
+    n = 30000
+    o = np.stack([rng.uniform(0.5, 3.5, n), rng.uniform(-3, -0.5, n), rng.uniform(0.5, 3.5, n)], 1).astype(np.float32)   # from below
+    tgt = np.stack([rng.uniform(1.3, 2.7, n), np.zeros(n), rng.uniform(1.3, 2.7, n)], 1)
+    d = tgt - o
+    d = (d / np.linalg.norm(d, axis=1, keepdims=True)).astype(np.float32)
+    t, prim = dr.Scene(desc).trace_rays(torch_.from_numpy(o).cuda(), torch_.from_numpy(d).cuda())
+    t, prim = t.cpu().numpy(), prim.cpu().numpy()
+    ot, otri = oracle.Scene(desc, oracle.F32).trace(o, d, brute=True)
+    plane = lambda a: (a < 8) | (a == 14) | (a == 15)
+    assert plane(otri).all() and plane(prim).all()
+    assert np.all(np.abs(t - ot) <= 1e-5 * np.abs(ot))
+    both = np.isin(otri, [14, 15]).mean()
+    assert 0.05 < both < 0.95                                           # both outcomes occur: the tie path is exercised
+
+
 # ---- a3, a5, a6: target evaluation --------------------------------------------------------------------------------
 @pytest.mark.parametrize("scene", ["furnace", "cornell", "mini_machines", "ggx_room", "closed_furnace", "mixture3"])
 def test_eval_matches_oracle(dr, oracle, torch_, scene):
@@ -119,13 +203,22 @@ def test_eval_matches_oracle(dr, oracle, torch_, scene):
     assert np.allclose(g2["p"].cpu().numpy(), g["p"], rtol=1e-6, atol=0) and (g2["sig"].cpu().numpy() == g["sig"]).all()
 
 
-def test_furnace_states_hit_the_closed_form_exactly(dr, torch_):
+def test_furnace_states_hit_the_closed_form_exactly(dr, oracle, torch_):
     desc = S.furnace()
     gsc = dr.Scene(desc)
     x = S.seeded_states(100000, desc.dim, 9)
     g = gsc.eval_states(torch_.from_numpy(x).cuda(), want_score=True)
     f, nr = g["f"].cpu().numpy(), g["nrays"].cpu().numpy()
-    assert ((f == 0.5) | (f == 1.0)).all()
+    # The fp32 Moeller-Trumbore test of Q8 is not watertight: about one ray in 1e5 slips between two facets of the
+    # sphere (u < 0 on one side of the shared edge, u + v > 1 on the other) and is then trapped inside -- in the
+    # oracle's fp32 evaluation as well (state 61404 of this set).  Counted, at most 3; every other state is exact.
+    e = oracle.Scene(desc, oracle.F32).eval(x, False)
+    leak = ~(((f == 0.5) | (f == 1.0)).all(1))
+    leak_o = ~(((e["f"] == 0.5) | (e["f"] == 1.0)).all(1))
+    assert leak.sum() <= 3 and leak_o.sum() <= 3, (leak.sum(), leak_o.sum())
+    both = ~leak & ~leak_o
+    assert np.array_equal(f[both].astype(np.float64), e["f"][both]) and np.array_equal(nr[both], e["nrays"][both])
+    f, nr, x = f[~leak], nr[~leak], x[~leak]
     assert (f[nr == 2] == 0.5).all() and (f[nr == 1] == 1.0).all()
     assert (g["g"].cpu().numpy() == 0).all()
     r = np.hypot(x[:, 0] * 64 - 32, x[:, 1] * 64 - 32)
@@ -156,12 +249,13 @@ def test_teacher_forced_parity(dr, oracle, torch_, method, case):
     assert (gs["x"].astype(np.float64) == os_["x"]).all()                       # RNG streams: bit-exact
     gst, ost = gch.stats(), och.stats()
     assert np.isclose(gst["p_lambda"], ost["p_lambda"], rtol=2e-6) and np.isclose(gst["kappa0"], ost["kappa0"], rtol=2e-6)
-    assert gst["mutations"] == ost["mutations"] == N and gst["rays"] == ost["rays"] or name != "furnace"
-    div, rep = compare_states(gs, os_, gch.last_step(), och.last(), stddev)
+    assert gst["mutations"] == ost["mutations"] == N
+    g_last, o_last = gch.last_step(), och.last()
+    div, rep = compare_states(gs, os_, g_last, o_last, stddev)
     assert div.mean() < 1e-3, rep
-    if not div.any():
-        assert (gch.queue() == och.queue()).all()                               # regeneration queue: bit-exact
-        assert gst["tours"] == ost["tours"]
+    nr_g, nr_o = gsc.eval_states(torch_.from_numpy(gs["x"]).cuda(), False)["nrays"].cpu().numpy(), osc.eval(os_["x"], False)["nrays"]
+    assert gst["rays"] == int(nr_g.sum()) and ost["rays"] == int(nr_o.sum()) and (nr_g[~div] == nr_o[~div]).all()   # closest-hit queries: counted exactly
+    compare_bulk(gch, och, gs, os_, g_last, o_last, div, gst["tours"], ost["tours"])
     worst = rep["frac"]
     # --- teacher-forced steps at several points of a run (Q15)
     for burst in (0, 3, 12):
@@ -175,15 +269,11 @@ def test_teacher_forced_parity(dr, oracle, torch_, method, case):
         gch.step(1)
         och.step(1)
         gs, os_ = gch.download(), och.state()
-        div, rep = compare_states(gs, os_, gch.last_step(), och.last(), stddev)
+        g_last, o_last = gch.last_step(), och.last()
+        div, rep = compare_states(gs, os_, g_last, o_last, stddev)
         worst = max(worst, rep["frac"])
         assert div.mean() < 1e-3, (method, name, burst, rep)
-        if not div.any():
-            assert (gch.queue() == och.queue()).all()
-            assert gch.stats()["tours"] - t0g == och.stats()["tours"] - t0o
-            ga, oa = gch.accum.cpu().numpy().astype(np.float64), och.accum()
-            scale = np.abs(oa).max() + 1e-30
-            assert np.abs(ga - oa).max() <= 2e-5 * scale + 1e-4 * np.abs(oa).max(), (method, name)
+        compare_bulk(gch, och, gs, os_, g_last, o_last, div, gch.stats()["tours"] - t0g, och.stats()["tours"] - t0o)
         assert (gs["x"] >= 0).all() and (gs["x"] < 1).all()
     print(f"{method}/{name}: worst per-step diverged fraction {worst:.2e}")
 
@@ -247,8 +337,10 @@ def test_edge_cases(dr, torch_):
     # resolve before any tour: warning + zero image
     ch = dr.Chains(gsc, "diffusion_restore", 4, seed=1, m=1e9)
     ch.init(0)
-    img, status = ch.resolve()
-    assert status == dr.DR_WARN_NO_TOURS and float(img.abs().max()) == 0.0
+    assert ch.stats()["status"] == dr.DR_OK
+    img, _ = ch.resolve()
+    st = ch.stats()
+    assert st["status"] == dr.DR_WARN_NO_TOURS and st["no_tour_resolves"] == 1 and float(img.abs().max()) == 0.0
     # wrong method in dr_step, invalid configs
     with pytest.raises(dr.DrError):
         dr.binding._check(dr.lib.dr_step(ch.h, 0, 1, None))
@@ -297,6 +389,15 @@ def test_sharded_chains_reproduce_the_unsharded_run(dr, torch_):
 
 # ---- BASELINE.json full sizes, in the launch configuration bench.py times ------------------------------------------------
 FULL = [("cornell", S.cornell, 65536, 2), ("caustic", S.caustic, 262144, 3), ("machines", S.machines, 589824, 4)]
+_SCENES = {}
+
+
+def _full_scene(dr, oracle, name, make):
+    """One scene build per module: the 539 k-triangle BVHs take seconds on either side."""
+    if name not in _SCENES:
+        desc = make()
+        _SCENES[name] = (desc, dr.Scene(desc), oracle.Scene(desc, oracle.F32))
+    return _SCENES[name]
 
 
 @pytest.mark.parametrize("case", FULL, ids=[c[0] for c in FULL])
@@ -304,13 +405,12 @@ def test_full_size_configs(dr, oracle, torch_, case):
     """configs[1..3] at their full chain counts: bit-exact RNG / queue / counters, and sampled states re-evaluated
     one by one by the oracle (the stored (f/p_hat, p, pixel, score, signature) of a chain is the evaluation of its x)."""
     name, make, N, seed = case
-    desc = make()
-    gsc, osc = dr.Scene(desc), oracle.Scene(desc, oracle.F32)
+    desc, gsc, osc = _full_scene(dr, oracle, name, make)
     method = "diffusion_restore"
     gch = dr.Chains(gsc, method, N, seed=seed)
     gch.init(0)
     rng = np.random.default_rng(7)
-    ids = np.unique(np.concatenate([rng.integers(0, N, 3000), [0, 1, 255, 256, N - 257, N - 1]]))
+    ids = np.unique(np.concatenate([rng.integers(0, N, 40000), [0, 1, 255, 256, N - 257, N - 1]]))
     gs = gch.download()
     # init states are the Philox uniforms of (chain, iteration 0, slot, REGEN_U, epoch 0): bit-exact
     for i in ids[:200]:
@@ -324,9 +424,8 @@ def test_full_size_configs(dr, oracle, torch_, case):
         assert (gs["pix"][ids] == e["pix"]).all()                                # splat pixel indices: bit-exact
         ok = gs["sig"][ids] == e["sig"]
         # Whole-path signatures (up to 16 hit triangles and lobes each): a path that grazes a triangle edge within
-        # fp32 rounding continues from the neighbour on one side.  Counted; bound 1e-3 per path, 5e-3 for the
-        # machines scene (14 segments per path over 0.01-0.2 wide facets, specular chains; Q15).
-        assert (~ok).mean() < (5e-3 if name == "machines" else 1e-3), (~ok).sum()
+        # fp32 rounding continues from the neighbour on one side.  Counted; < 1e-3 of the paths (Q15).
+        assert (~ok).mean() < 1e-3, (~ok).sum()
         p, fop = gs["p"][ids][ok].astype(np.float64), gs["fop"][ids][ok].astype(np.float64)
         assert (np.abs(p - e["p"][ok]) <= 1e-4 * np.maximum(e["p"][ok], 1e-8)).all()
         want = e["f"][ok] / (e["p"][ok][:, None] + 1e-8)
@@ -343,56 +442,123 @@ def test_full_size_configs(dr, oracle, torch_, case):
         assert st["mutations"] == N * (it + 1) and st["iteration"] == it and st["nonfinite"] == 0
         assert (gs["x"] >= 0).all() and (gs["x"] < 1).all()
         q = gch.queue()
-        assert (q == np.flatnonzero(gs["killed"])).all()                        # regeneration queue: bit-exact, ascending
+        assert (q == np.flatnonzero(gs["killed"])).all()                        # regeneration queue: ascending killed ids
         kills += len(q)
         assert st["tours"] == kills and st["kills_last_step"] == len(q)
         check_sample(gs)
-    if name != "machines":      # the oracle runs these two in full in seconds: whole-ensemble teacher-forced step
-        och = oracle.Chains(osc, method, N, seed=seed)
-        och.init(0)
-        och.step(2)
-        gch.upload(och.state(), 2)
-        gch.step(1)
-        och.step(1)
-        div, rep = compare_states(gch.download(), och.state(), gch.last_step(), och.last(), float(gch.cfg.stddev))
-        assert div.mean() < 1e-3, rep
-        if not div.any():
-            assert (gch.queue() == och.queue()).all()
+
+
+WHOLE = [("cornell", S.cornell, 65536, 2, m) for m in METHODS] + [("caustic", S.caustic, 262144, 3, m) for m in METHODS] + \
+        [("machines", S.machines, 589824, 4, m) for m in ("metropolis_restore", "diffusion_restore")]
+
+
+@pytest.mark.parametrize("case", WHOLE, ids=[f"{c[0]}-{c[4]}" for c in WHOLE])
+def test_whole_ensemble_teacher_forced_step(dr, oracle, torch_, case):
+    """Every chain of the full-size ensemble, every sampler: the oracle runs init + 2 iterations, its state is uploaded,
+    both sides take one step (through k_wave<GRAD> for the Langevin-based samplers, k_wave<false> for the others), and
+    states, decisions, queue, tourCount and accumulation buffer are compared with the oracle's (Q15)."""
+    name, make, N, seed, method = case
+    desc, gsc, osc = _full_scene(dr, oracle, name, make)
+    gch = dr.Chains(gsc, method, N, seed=seed)
+    och = oracle.Chains(osc, method, N, seed=seed)
+    gch.init(0)
+    och.init(0)
+    och.step(2)
+    gch.upload(och.state(), 2)
+    gch.accum.zero_()
+    och.zero_accum()
+    t0g, t0o = gch.stats()["tours"], och.stats()["tours"]
+    gch.step(1)
+    och.step(1)
+    gs, os_ = gch.download(), och.state()
+    g_last, o_last = gch.last_step(), och.last()
+    div, rep = compare_states(gs, os_, g_last, o_last, float(gch.cfg.stddev))
+    print(f"{name}/{method}: {rep}")
+    assert div.mean() < 1e-3, rep                                               # < 0.1 % of the chains per step (B: north_star)
+    compare_bulk(gch, och, gs, os_, g_last, o_last, div, gch.stats()["tours"] - t0g, och.stats()["tours"] - t0o)
 
 
 # ---- the two forms of the evaluation (k_wave vs per-segment loop) -------------------------------------------------
-_EVAL_SNIPPET = """
+def _same_eval(a, b):
+    for k in ("f", "p", "pix", "nrays", "sig", "g"):
+        if a[k] is None:
+            assert b[k] is None
+            continue
+        x, y = a[k].cpu().numpy(), b[k].cpu().numpy()
+        assert np.array_equal(x.view(np.uint32), y.view(np.uint32)), k
+
+
+WAVE = [("mini_machines", S.mini_machines, 1 << 18), ("ggx_room", S.ggx_room, 1 << 18), ("mini_machines", S.mini_machines, 4999),
+        ("ggx_room", S.ggx_room, 33), ("caustic", S.caustic, 262144), ("machines", S.machines, 589824)]
+
+
+@pytest.mark.parametrize("score", [True, False], ids=["grad", "nograd"])
+@pytest.mark.parametrize("case", WAVE, ids=[f"{c[0]}-{c[2]}" for c in WAVE])
+def test_wave_kernel_equals_segment_loop(dr, oracle, torch_, case, score):
+    """The same states evaluated by k_wave (one persistent kernel, dr_wave.cuh; both instantiations) and by the
+    per-segment loop k_trace / k_shade: both run the same shade_vertex on the same closest hits, so f, p, pixel, rays per
+    path, signature and score must be identical bit for bit -- anything else is a ray lost, duplicated or read before it
+    was written.  Sizes from 33 states (most warps idle) to the bench configuration (machines, one state per pixel)."""
+    name, make, n = case
+    desc, gsc, _ = _full_scene(dr, oracle, name, make) if name in ("caustic", "machines") else (make(), None, None)
+    gsc = gsc or dr.Scene(desc)
+    x = torch_.from_numpy(S.seeded_states(n, desc.dim, 11)).cuda()
+    a = gsc.eval_states(x, score, form=2)
+    b = gsc.eval_states(x, score, form=1)
+    assert int(a["nrays"].sum()) > n                                             # paths do bounce
+    _same_eval(a, b)
+    c = gsc.eval_states(x, score, form=2)                                        # and again: a second launch on fresh memory
+    _same_eval(a, c)
+
+
+def test_chains_run_identically_in_both_forms(dr, torch_):
+    """dr_step through k_wave and through the loop: same states, flags and counters after 6 iterations, for a sampler
+    of each kind (the queue memory is reused by successive evaluations: tags, not clearing, tell them apart)."""
+    desc = S.mini_machines()
+    gsc = dr.Scene(desc)
+    for method in ("metropolis", "mala_restore", "diffusion_restore"):
+        out = []
+        for form in (2, 1):
+            ch = dr.Chains(gsc, method, 20000, seed=5)
+            ch.set_eval_form(form)
+            ch.init(1)
+            ch.step(6)
+            out.append((ch.download(), ch.stats()))
+        (sa, ta), (sb, tb) = out
+        for k in sa:
+            assert np.array_equal(sa[k].view(np.uint8), sb[k].view(np.uint8)), (method, k)
+        assert ta["tours"] == tb["tours"] and ta["rays"] == tb["rays"] and ta["mh_accepts"] == tb["mh_accepts"]
+
+
+_STALL_SNIPPET = """
 import sys, numpy as np, torch
 sys.path.insert(0, {root!r})
 import paper_2605_08916_b200 as dr
 from dr_inputs import scenes as S
-desc = getattr(S, {scene!r})()
+desc = S.mini_machines()
 x = torch.from_numpy(S.seeded_states({n}, desc.dim, 11)).cuda()
-e = dr.Scene(desc).eval_states(x, True)
+e = dr.Scene(desc).eval_states(x, True, form=2)
 torch.cuda.synchronize()
 np.savez({out!r}, **{{k: v.cpu().numpy() for k, v in e.items()}})
 """
 
 
-@pytest.mark.parametrize("scene", ["mini_machines", "ggx_room"])
-def test_wave_kernel_equals_segment_loop(dr, torch_, tmp_path, scene):
-    """2^18 states evaluated by k_wave (one persistent kernel, dr_wave.cuh) and, in a second process with DR_WAVE=0, by
-    the per-segment loop k_trace / k_shade: both run the same shade_vertex on the same closest hits, so f, p, pixel,
-    rays per path, signature and score must be identical bit for bit -- anything else is a ray lost, duplicated or
-    read before it was written in the ring.  (The small parity scenes above never reach k_wave: it starts at 2^18.)"""
+def test_wave_kernel_with_stalled_consumers(dr, torch_, tmp_path):
+    """A build in which every trace warp sleeps 1 ms between claiming queue entries and reading them
+    (-DDR_WAVE_STALL_NS=1000000): the results must not change.  The queue protocol of dr_wave.cuh does not rely on
+    entries being read soon after they were claimed (round 1's ring did, and lost rays under such a stall)."""
     import os
     import subprocess
     import sys
+    from paper_2605_08916_b200 import build
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    n = 1 << 18
-    res = {}
-    for mode in ("1", "0"):
-        out = str(tmp_path / f"eval_{mode}.npz")
-        env = dict(os.environ, DR_WAVE=mode)
-        subprocess.run([sys.executable, "-c", _EVAL_SNIPPET.format(root=root, scene=scene, n=n, out=out)], check=True, env=env,
-                       timeout=600)
-        res[mode] = np.load(out)
-    a, b = res["1"], res["0"]
-    assert int(a["nrays"].sum()) == int(b["nrays"].sum()) and a["nrays"].sum() > n      # paths do bounce
+    lib = build.build_variant("stall", ["-DDR_WAVE_STALL_NS=1000000"])
+    n = 100003
+    out = str(tmp_path / "stall.npz")
+    subprocess.run([sys.executable, "-c", _STALL_SNIPPET.format(root=root, n=n, out=out)], check=True, env=dict(os.environ, DR_LIB=lib),
+                   timeout=900)
+    a = np.load(out)
+    desc = S.mini_machines()
+    b = dr.Scene(desc).eval_states(torch_.from_numpy(S.seeded_states(n, desc.dim, 11)).cuda(), True, form=1)
     for k in ("f", "p", "pix", "nrays", "sig", "g"):
-        assert np.array_equal(a[k].view(np.uint32), b[k].view(np.uint32)), k
+        assert np.array_equal(a[k].view(np.uint32), b[k].cpu().numpy().view(np.uint32)), k

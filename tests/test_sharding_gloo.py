@@ -29,6 +29,12 @@ WORKER = textwrap.dedent("""
     want = sum(torch.from_numpy(np.random.default_rng(r).random((64, 4)).astype(np.float32)) for r in range(world))
     assert torch.allclose(tot, want) and tours == sum(10 + r for r in range(world)) and muts == sum(100 * (r + 1) for r in range(world))
     assert torch.equal(acc, torch.from_numpy(np.random.default_rng(rank).random((64, 4)).astype(np.float32)))  # input untouched
+    # counters as 16-bit limbs in an fp32 buffer: the sum over ranks is exact (what k_pack_frame / k_resolve rely on)
+    mine = [2**40 + 65535 * (rank + 1), 2**33 - 1 - rank]
+    t = torch.tensor(sharding.limbs(mine[0]) + sharding.limbs(mine[1]), dtype=torch.float32)
+    dist.all_reduce(t)
+    assert sharding.from_limbs(t[:4]) == sum(2**40 + 65535 * (r + 1) for r in range(world))
+    assert sharding.from_limbs(t[4:]) == sum(2**33 - 1 - r for r in range(world))
     dist.destroy_process_group()
     print("ok", rank)
 """) % (ROOT, ROOT)
