@@ -186,6 +186,9 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
     if (wave) k_raygen<true><<<g, kShadeBlock, 0, s>>>(dev, ws, io, n);
     else k_raygen<false><<<g, kShadeBlock, 0, s>>>(dev, ws, io, n);
   }
+#if DR_CHECKS
+  if (wave) CUDA_TRY(cudaMemsetAsync(ws.hits, 0, sizeof(uint2) * (size_t)ws.cap, s));   // per-state segment counters of the checks
+#endif
   if (wave) {
     ProfScope ps(prof, DR_PROF_TRACE, s);
     if (grad) k_wave<true><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
@@ -206,6 +209,16 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
   }
   if (grad) { ProfScope ps(prof, DR_PROF_GRAD, s); k_grad<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io); }
   CUDA_TRY(cudaGetLastError());
+#if DR_CHECKS
+  if (wave) {   // checked build: every queue entry that was reserved was consumed, every path finished, no check fired
+    uint32_t h[kCtlWords];
+    CUDA_TRY(cudaMemcpyAsync(h, ws.ctl, sizeof(h), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    if (h[kCtlWaveError] || h[kCtlWaveDone] != n || h[kCtlWaveReserve] > dev.L * ws.cap)
+      return fail(DR_ERR_CUDA, "k_wave protocol check failed: error bits " + std::to_string(h[kCtlWaveError]) + ", finished " +
+                                   std::to_string(h[kCtlWaveDone]) + " of " + std::to_string(n));
+  }
+#endif
   return DR_OK;
 }
 

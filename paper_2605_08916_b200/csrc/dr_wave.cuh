@@ -42,6 +42,16 @@ namespace dr {
 #ifndef DR_WAVE_STALL_NS
 #define DR_WAVE_STALL_NS 0      // test builds: every trace warp sleeps this long after each claim, before it reads the entries
 #endif
+#ifndef DR_CHECKS
+#define DR_CHECKS 0             // test builds (compute-sanitizer is closed on this pool): device-side checks of the queue protocol;
+#endif                          // a violated check sets a bit of ctl[kCtlWaveError], which the evaluation hooks turn into DR_ERR_CUDA
+constexpr int kCtlWaveError = 52;
+enum : uint32_t { kErrIndex = 1u, kErrState = 2u, kErrOwner = 4u, kErrSegment = 8u, kErrHitRing = 16u, kErrCount = 32u };
+#if DR_CHECKS
+#define DR_CHECK(cond, bit) do { if (!(cond)) atomicOr(&ws.ctl[kCtlWaveError], (uint32_t)(bit)); } while (0)
+#else
+#define DR_CHECK(cond, bit) do { } while (0)
+#endif
 constexpr int kWaveShadeWarps = DR_WAVE_SHADE_WARPS;     // sweep 1 / 2 / 3 / 4 / 5 / 6: 9.13 / 5.25 / 4.85 / 5.05 / 5.22 / 5.45 ms per frame
 constexpr int kWaveRefillBelow = DR_WAVE_REFILL_BELOW;   // a trace warp flushes its finished rays and refills below this many busy lanes
 constexpr int kWaveTraceThreads = kTraceBlock - 32 * kWaveShadeWarps;
@@ -95,6 +105,7 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
         if (lane == 0) {
           base = atomicAdd(&wsh->reserve, cnt);
           while ((int)(base + cnt - ld_volatile(&wsh->freed)) > (int)kHitCap) __nanosleep(40);
+          DR_CHECK(base + cnt - ld_volatile(&wsh->head) <= kHitCap, kErrHitRing);   // no unread entry is overwritten
         }
         base = __shfl_sync(kFull, base, 0);
         if (pend) {
@@ -145,6 +156,8 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
         pay = got_pay;
         const float4* e = ws.qa + 4 * (size_t)(pay & kWaveStateMask);
         const float4 o = __ldcg(e), d = __ldcg(e + 1);   // written by another SM during this launch: not through L1
+        DR_CHECK((pay & kWaveStateMask) < ws.cap && (pay >> kWaveKShift) < sc.L, kErrState);
+        DR_CHECK(__float_as_uint(o.w) == (pay & kWaveStateMask), kErrOwner);         // the record is this state's
         trav_setup(L.r, o.x, o.y, o.z, d.x, d.y, d.z, one);
         trav_begin(L.s);
         L.tsp = 0;
@@ -219,6 +232,10 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
     float4* rec = ws.qa + 4 * (size_t)s;
     if (mine) {
       const float4 Q0 = __ldcg(rec), Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2);
+      DR_CHECK(__float_as_uint(Q0.w) == s && k <= sc.L, kErrOwner);
+#if DR_CHECKS
+      DR_CHECK(atomicAdd(&ws.hits[s].x, 1u) == k - 1u, kErrSegment);   // segments of a state are shaded once each, in order
+#endif
       shade_vertex<GRAD>(sc, ws, io, k, Q0, Q1, Q2, h, s, cont, want_grad, bad, n0, n1, n2);
     }
     if (GRAD) {  // reverse-pass list: one atomic per warp
@@ -237,6 +254,7 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
       uint32_t base = 0;
       if (lane == 0) base = atomicAdd(&ws.ctl[kCtlWaveReserve], nc);
       base = __shfl_sync(kFull, base, 0);
+      DR_CHECK(base + nc <= sc.L * ws.cap, kErrIndex);
       if (cont) {
         __stcg(rec, n0); __stcg(rec + 1, n1); __stcg(rec + 2, n2);
         st_release2(ws.ring + base + __popc(b & lt), make_uint2(s | (k << kWaveKShift), ws.tag));   // segment k + 1, stored as k

@@ -562,3 +562,20 @@ def test_wave_kernel_with_stalled_consumers(dr, torch_, tmp_path):
     b = dr.Scene(desc).eval_states(torch_.from_numpy(S.seeded_states(n, desc.dim, 11)).cuda(), True, form=1)
     for k in ("f", "p", "pix", "nrays", "sig", "g"):
         assert np.array_equal(a[k].view(np.uint32), b[k].cpu().numpy().view(np.uint32)), k
+
+
+def test_small_run_under_the_checked_build(dr, tmp_path):
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so the queue protocol of k_wave is checked by
+    a build with device-side assertions instead (-DDR_CHECKS=1, csrc/dr_wave.cuh): indices inside the queue, records owned by
+    the state that the entry names, every segment of a state shaded exactly once and in order, the block's ring never
+    overwriting an unread entry, every path finished.  Run on the stalled-consumer timing as well."""
+    import os
+    import subprocess
+    import sys
+    from paper_2605_08916_b200 import build
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for name, flags in (("checked", ["-DDR_CHECKS=1"]), ("checked_stall", ["-DDR_CHECKS=1", "-DDR_WAVE_STALL_NS=300000"])):
+        lib = build.build_variant(name, flags)
+        r = subprocess.run([sys.executable, os.path.join(root, "tests", "sanitizer", "small_run.py")], env=dict(os.environ, DR_LIB=lib),
+                           capture_output=True, text=True, timeout=900)
+        assert r.returncode == 0 and "small_run ok" in r.stdout, r.stdout + r.stderr
