@@ -159,11 +159,11 @@ void orc_pt_render(void* h_, uint64_t n, uint64_t seed, double* rgb) {
 }
 
 void* orc_chains_create(void* scene_, int method, uint32_t n_chains, double stddev, double c_tilde, double dt, double m,
-                        double large_step_prob, double p_lambda_override, uint64_t seed, uint32_t chain_offset) {
+                        double large_step_prob, double p_lambda_override, uint64_t seed, uint32_t chain_offset, int rao_blackwell) {
   auto* s = (SceneH*)scene_;
   auto* h = new ChainsH();
   h->prec = s->prec;
-  Config c{method, n_chains, stddev, c_tilde, dt, m, large_step_prob, p_lambda_override, seed, chain_offset};
+  Config c{method, n_chains, stddev, c_tilde, dt, m, large_step_prob, p_lambda_override, seed, chain_offset, rao_blackwell};
   if (s->prec == 0) h->f.reset(new Chains<float>(s->f, c)); else h->d.reset(new Chains<double>(s->d, c));
   return h;
 }

@@ -13,7 +13,7 @@ import numpy as np
 from . import build as _build
 
 F32, F64 = 0, 1
-METHODS = {"metropolis": 0, "mala": 1, "metropolis_restore": 2, "mala_restore": 3, "diffusion_restore": 4}
+METHODS = {"metropolis": 0, "mala": 1, "metropolis_restore": 2, "mala_restore": 3, "diffusion_restore": 4, "path_tracing": 5}
 
 _lib = None
 
@@ -37,7 +37,7 @@ def lib():
         L.orc_eval.argtypes = [vp, vp, u32, i32, vp, vp, vp, vp, vp, vp, vp]
         L.orc_pt_render.argtypes = [vp, u64, u64, vp]
         L.orc_chains_create.restype = vp
-        L.orc_chains_create.argtypes = [vp, i32, u32, f64, f64, f64, f64, f64, f64, u64, u32]
+        L.orc_chains_create.argtypes = [vp, i32, u32, f64, f64, f64, f64, f64, f64, u64, u32, i32]
         L.orc_chains_destroy.argtypes = [vp]
         L.orc_chains_init.argtypes = [vp, u32]
         L.orc_chains_step.argtypes = [vp, u32]
@@ -166,7 +166,7 @@ class Chains:
     """Oracle-side chain ensemble: Alg. 1-4 of the paper, one plain loop over chains."""
 
     def __init__(self, scene: Scene, method, n_chains, stddev=None, c_tilde=None, dt=1e-5, m=64.0, large_step_prob=None,
-                 p_lambda_override=0.0, seed=0, chain_offset=0):
+                 p_lambda_override=0.0, seed=0, chain_offset=0, rao_blackwell=False):
         method = METHODS[method] if isinstance(method, str) else int(method)
         if stddev is None:
             stddev = 1e-2 if method in (0, 2) else 5e-3       # PAPER.md L747
@@ -178,7 +178,7 @@ class Chains:
         self.params = dict(stddev=stddev, c_tilde=c_tilde, dt=dt, m=m, large_step_prob=large_step_prob,
                            p_lambda_override=p_lambda_override, seed=seed)
         self.h = lib().orc_chains_create(scene.h, method, self.N, stddev, c_tilde, dt, m, large_step_prob,
-                                         p_lambda_override, int(seed), int(chain_offset))
+                                         p_lambda_override, int(seed), int(chain_offset), int(bool(rao_blackwell)))
 
     def __del__(self):
         if getattr(self, "h", None) and _lib is not None:

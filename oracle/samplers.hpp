@@ -23,7 +23,8 @@
 
 namespace orc {
 
-enum Method : int { METROPOLIS = 0, MALA = 1, METROPOLIS_RESTORE = 2, MALA_RESTORE = 3, DIFFUSION_RESTORE = 4 };
+enum Method : int { METROPOLIS = 0, MALA = 1, METROPOLIS_RESTORE = 2, MALA_RESTORE = 3, DIFFUSION_RESTORE = 4,
+                    PATH_TRACING = 5 };  // 5: ordinary path tracing on the same buffers: the baseline of section 6
 
 struct Config {
   int method;
@@ -36,6 +37,8 @@ struct Config {
   double p_lambda_override; // <= 0: bootstrap from the init states (Q-a0)
   uint64_t seed;
   uint32_t chain_offset;    // global id of chain 0 (chains are keyed by global id: sharding-invariant, section 8e)
+  int rao_blackwell;        // Restore variants: accumulate E[dtau | x] = 1 / (lambda + kappa) instead of the sampled dtau
+                            // (Rao-Blackwellisation of the holding time; DESIGN.md f3)
 };
 
 template <class Real> struct Eval {
@@ -118,7 +121,7 @@ template <class Real> struct Chains {
 
   Chains(const Scene<Real>& s, const Config& c) : sc(s), cfg(c) {
     N = c.n_chains; d = s.dim(); npix = s.W * s.H;
-    restore = c.method >= METROPOLIS_RESTORE;
+    restore = c.method >= METROPOLIS_RESTORE && c.method <= DIFFUSION_RESTORE;
     grad = c.method == MALA || c.method == MALA_RESTORE || c.method == DIFFUSION_RESTORE;
     x.assign((size_t)N * d, 0); g.assign((size_t)N * d, 0); p.assign(N, 0); fop.assign((size_t)N * 3, 0);
     pix.assign(N, 0); sig.assign(N, 0); killed.assign(N, 0); accepted.assign(N, 0); dtau.assign(N, 0);
@@ -149,6 +152,7 @@ template <class Real> struct Chains {
     p[i] = e.p; pix[i] = e.pix; sig[i] = e.sig;
     const Real phat = e.p + Real(kEps);
     for (int c = 0; c < 3; ++c) fop[(size_t)i * 3 + c] = e.f[c] / phat;  // f / p_hat, Alg. 1 L523 with Q9
+    if (cfg.method == PATH_TRACING) for (int c = 0; c < 3; ++c) fop[(size_t)i * 3 + c] = e.f[c];  // independent samples: f itself
   }
 
   // Accumulate, Alg. 1 L506-L526.  The target was evaluated when the state was stored.
@@ -163,13 +167,14 @@ template <class Real> struct Chains {
       const Real dt2 = -std::log(u01_oc<Real>(w[3])) / kappa;  // L512
       if (dt1 < dt2) { weight = dt1; killed[i] = 0; }          // L513-L515
       else { weight = dt2; killed[i] = 1; ++tours; ++kills_last; }  // L516-L519 (tie -> killed, Q16)
+      if (cfg.rao_blackwell) weight = Real(1) / (lambda + kappa);    // E[min(dt1, dt2)]; the kill decision stays the sampled race
     }
     dtau[i] = weight;
     ++mutations;
     if (p[i] > Real(0)) {                                      // L522
       double* a = &accum[(size_t)pix[i] * 4];
       for (int c = 0; c < 3; ++c) a[c] += (double)(weight * fop[(size_t)i * 3 + c]);  // L524
-      a[3] += (double)(weight / phat);                         // ratio-image denominator (Q12)
+      a[3] += cfg.method == PATH_TRACING ? 1.0 : (double)(weight / phat);   // ratio-image denominator (Q12); PT: sample count
     }
   }
 
@@ -240,7 +245,7 @@ template <class Real> struct Chains {
         const Real* gi = &g[(size_t)i * d];
         uint32_t w[4];
         stream_block(cfg.seed, cfg.chain_offset + i, n, 0, DECIDE, epoch, w);
-        if (restore && killed[i]) {                 // Alg. 2: re-initialise from nu
+        if ((restore && killed[i]) || cfg.method == PATH_TRACING) {   // Alg. 2: re-initialise from nu; PT: always
           kind[i] = 1;
           uniform_point(i, n, REGEN_U, y);
         } else if (!restore && u01_co<Real>(w[0]) < (Real)cfg.large_step_prob) {
@@ -295,6 +300,8 @@ template <class Real> struct Chains {
     if (restore) {
       if (tours == 0) { std::fill(rgb, rgb + (size_t)npix * 3, 0.0); return 1; }
       scale = (double)npix * (double)kappa0 / (double)tours;
+    } else if (cfg.method == PATH_TRACING) {
+      scale = (double)npix / (double)mutations;                 // mean of f over the samples, per pixel area
     } else {
       scale = (double)npix * (double)p_lambda / (double)mutations;
     }

@@ -113,10 +113,15 @@ PARAMS = {
 }
 
 
-@pytest.mark.parametrize("method", list(PARAMS))
-def test_finite_state_brute_force(oracle, method):
+RB = [(m, False) for m in PARAMS] + [(m, True) for m in PARAMS if m.endswith("restore")]
+
+
+@pytest.mark.parametrize("method,rb", RB, ids=[m + ("-rao_blackwell" if r else "") for m, r in RB])
+def test_finite_state_brute_force(oracle, method, rb):
+    """rb: Rao-Blackwellised Accumulate (f3): the weight is E[dtau | x] = 1 / (lambda + kappa), which is exactly the
+    `hold` the model propagates, so the same expectations pin it."""
     sc, pts, p, g, pix = grid_model(oracle)
-    kw = dict(PARAMS[method])
+    kw = dict(PARAMS[method], rao_blackwell=rb)
     s, ct = kw["stddev"], kw.get("c_tilde", 0.0)
     m, dt, lsp = kw.get("m", 64.0), kw.get("dt", 1e-5), kw.get("large_step_prob", 0.0)
     p_lambda = 1.0 + EPS
@@ -141,6 +146,69 @@ def test_finite_state_brute_force(oracle, method):
     if method.endswith("restore"):
         t_se = tours.std(ddof=1) / np.sqrt(seeds)
         assert abs(tours.mean() - want_tours) < 5 * t_se + 5e-4 * want_tours, (method, tours.mean(), want_tours)
+
+
+def test_rao_blackwell_weight_is_the_expected_holding_time(oracle):
+    """f3: with the flag every chain accumulates 1 / (lambda + kappa0 / p_hat(x)) -- a closed form of
+    its state -- the kill decisions and hence the states are those of the plain run with the same seed, and the
+    per-pixel spread over seeds of the accumulation buffer shrinks."""
+    sc = oracle.Scene(target(), oracle.F64)
+    kw = dict(PARAMS["diffusion_restore"])
+    N, p_lambda = 20000, 1.0 + EPS
+    spread = {}
+    for rb in (False, True):
+        accs = []
+        for seed in range(6):
+            ch = oracle.Chains(sc, "diffusion_restore", N, seed=300 + seed, p_lambda_override=p_lambda, rao_blackwell=rb, **kw)
+            ch.init(0)
+            ch.step(5)
+            accs.append(ch.accum()[:, 0] / N)
+            if seed == 0:
+                st, (_, w) = ch.state(), ch.last()
+                if rb:
+                    lam, kappa0 = 1.0 / kw["dt"], p_lambda / (kw["m"] * kw["dt"])
+                    assert np.allclose(w, 1.0 / (lam + kappa0 / (st["p"] + EPS)), rtol=1e-13, atol=0)
+                    assert np.array_equal(st["x"], x_plain) and np.array_equal(st["killed"], k_plain)
+                else:
+                    x_plain, k_plain = st["x"], st["killed"]
+        spread[rb] = np.array(accs).std(0, ddof=1).sum()
+    assert spread[True] < 0.85 * spread[False], spread
+
+
+def test_path_tracing_method_is_a_plain_average(oracle):
+    """f2: method 5 draws every chain anew each iteration and accumulates f with unit weight.
+    Recomputed here from the definition: the Philox uniforms of (chain, iteration), the target evaluation (pinned in
+    test_oracle_target.py), a numpy histogram.  And the furnace classes resolve to their closed forms."""
+    desc = S.furnace()
+    sc = oracle.Scene(desc, oracle.F64)
+    N, T, seed = 3000, 3, 11
+    ch = oracle.Chains(sc, "path_tracing", N, seed=seed)
+    ch.init(2)
+    ch.step(T)
+    assert ch.stats()["mutations"] == N * (T + 1) and ch.stats()["tours"] == 0 and len(ch.queue()) == 0
+    want = np.zeros((desc.width * desc.height, 4))
+    for it in range(T + 1):
+        x = np.zeros((N, desc.dim))
+        for i in range(N):
+            for j in range(desc.dim // 4):
+                w = oracle.stream_block(seed, i, it, j, 0, 2)
+                x[i, 4 * j:4 * j + 4] = (w >> 8).astype(np.float64) * 2.0 ** -24
+        e = sc.eval(x, False)
+        np.add.at(want[:, :3], e["pix"], e["f"])
+        np.add.at(want[:, 3], e["pix"], 1.0)
+        if it == T:
+            assert np.array_equal(ch.state()["x"], x)
+    assert np.allclose(ch.accum(), want, rtol=1e-12, atol=0)
+    img, status = ch.resolve()
+    assert status == 0 and np.allclose(img.reshape(-1, 3), want[:, :3] * (desc.width * desc.height / (N * (T + 1.0))), rtol=1e-12)
+    # closed form (tests/golden/furnace.txt): many samples, class means 0.5 / 1.0
+    ch = oracle.Chains(sc, "path_tracing", 100000, seed=1)
+    ch.init(0)
+    ch.step(3)
+    img = ch.resolve()[0][..., 0]
+    yy, xx = np.mgrid[0:64, 0:64]
+    corners = [np.hypot(xx + a - 32, yy + b - 32) for a in (0, 1) for b in (0, 1)]
+    assert abs(img[np.max(corners, axis=0) < 22.65].mean() - 0.5) < 0.01 and abs(img[np.min(corners, axis=0) > 22.75].mean() - 1.0) < 0.01
 
 
 def test_model_identities_tour_length_and_unbiasedness(oracle):
