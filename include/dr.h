@@ -44,7 +44,9 @@ typedef enum {
   DR_MALA = 1,
   DR_METROPOLIS_RESTORE = 2,
   DR_MALA_RESTORE = 3,
-  DR_DIFFUSION_RESTORE = 4
+  DR_DIFFUSION_RESTORE = 4,
+  DR_PATH_TRACING = 5        /* ordinary path tracing on the same buffers, the baseline of its section 6:
+                                every chain is drawn anew each iteration, f accumulated with unit weight */
 } dr_method;
 
 /* pbrt-v4 diffuse / dielectric / conductor + DiffuseAreaLight, simplified as in DESIGN.md Q6-Q7. */
@@ -95,6 +97,8 @@ typedef struct {
   uint64_t seed;             /* Philox key (Q14) */
   uint32_t chain_offset;     /* global id of chain 0: RNG streams are keyed by global chain id, so a run sharded
                                 over several GPUs draws the same numbers as the unsharded run */
+  uint32_t rao_blackwell;    /* Restore variants, 0 / 1: accumulate E[dtau | x] = 1 / (lambda + kappa) instead of the sampled
+                                dtau (Rao-Blackwellised holding time); the kill decision stays the race */
 } dr_config;
 
 typedef struct {
@@ -146,8 +150,8 @@ dr_status dr_chains_init(dr_chains* chains, uint32_t frame_index, void* stream);
  * (DR_ERR_INVALID_ARG otherwise). */
 dr_status dr_step(dr_chains* chains, int32_t method, uint32_t iterations, void* stream);
 
-/* Alg. 3: dev_rgb_out[W*H*3] = N_pix * kappa0 / tourCount * accum (Restore) or N_pix * p_lambda / N_mut * accum
- * (plain MH).  Asynchronous: if tourCount == 0 the kernel writes zeros (no division) and counts the event in
+/* Alg. 3: dev_rgb_out[W*H*3] = N_pix * kappa0 / tourCount * accum (Restore), N_pix * p_lambda / N_mut * accum (plain MH)
+ * or N_pix / N_mut * accum (path tracing).  Asynchronous: if tourCount == 0 the kernel writes zeros (no division) and counts the event in
  * dr_stats.no_tour_resolves; the next dr_chains_stats then returns DR_WARN_NO_TOURS. */
 dr_status dr_resolve_image(dr_chains* chains, float* dev_rgb_out, void* stream);
 

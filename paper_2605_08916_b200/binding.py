@@ -16,8 +16,8 @@ LIB_PATH = os.environ.get("DR_LIB") or os.path.join(HERE, "libdr.so")   # DR_LIB
 
 DR_OK, DR_WARN_NO_TOURS = 0, 1
 DR_ERR_INVALID_ARG, DR_ERR_UNSUPPORTED, DR_ERR_CUDA, DR_ERR_NONFINITE, DR_ERR_OOM = -1, -2, -3, -4, -5
-DR_METROPOLIS, DR_MALA, DR_METROPOLIS_RESTORE, DR_MALA_RESTORE, DR_DIFFUSION_RESTORE = range(5)
-METHODS = {"metropolis": 0, "mala": 1, "metropolis_restore": 2, "mala_restore": 3, "diffusion_restore": 4}
+DR_METROPOLIS, DR_MALA, DR_METROPOLIS_RESTORE, DR_MALA_RESTORE, DR_DIFFUSION_RESTORE, DR_PATH_TRACING = range(6)
+METHODS = {"metropolis": 0, "mala": 1, "metropolis_restore": 2, "mala_restore": 3, "diffusion_restore": 4, "path_tracing": 5}
 
 EXPORTS = [
     "dr_last_error", "dr_scene_create", "dr_scene_create_analytic2d", "dr_scene_destroy", "dr_scene_get_info",
@@ -51,7 +51,7 @@ class dr_analytic2d_desc(C.Structure):
 class dr_config(C.Structure):
     _fields_ = [("method", C.c_int32), ("n_chains", C.c_uint32), ("stddev", C.c_float), ("c_tilde", C.c_float),
                 ("dt", C.c_float), ("m", C.c_float), ("large_step_prob", C.c_float), ("p_lambda_override", C.c_float),
-                ("seed", C.c_uint64), ("chain_offset", C.c_uint32)]
+                ("seed", C.c_uint64), ("chain_offset", C.c_uint32), ("rao_blackwell", C.c_uint32)]
 
 
 class dr_stats(C.Structure):
@@ -215,7 +215,7 @@ class Chains:
     """dr_chains_create over caller-owned torch memory + the per-frame calls."""
 
     def __init__(self, scene: Scene, method, n_chains, stddev=None, c_tilde=None, dt=1e-5, m=64.0, large_step_prob=None,
-                 p_lambda_override=0.0, seed=0, chain_offset=0):
+                 p_lambda_override=0.0, seed=0, chain_offset=0, rao_blackwell=False):
         method = METHODS[method] if isinstance(method, str) else int(method)
         if stddev is None:
             stddev = 1e-2 if method in (0, 2) else 5e-3        # PAPER.md L747
@@ -224,7 +224,8 @@ class Chains:
         if large_step_prob is None:
             large_step_prob = 0.3 if method in (0, 1) else 0.0
         self.scene, self.method, self.N, self.d = scene, method, int(n_chains), scene.dim
-        self.cfg = dr_config(method, self.N, stddev, c_tilde, dt, m, large_step_prob, p_lambda_override, seed, chain_offset)
+        self.cfg = dr_config(method, self.N, stddev, c_tilde, dt, m, large_step_prob, p_lambda_override, seed, chain_offset,
+                             int(bool(rao_blackwell)))
         nbytes = lib.dr_chains_state_bytes(scene.h, C.byref(self.cfg))
         if nbytes == 0:
             raise DrError(DR_ERR_INVALID_ARG, lib.dr_last_error().decode())

@@ -126,7 +126,8 @@ Layout make_layout(uint32_t N, uint32_t planes, uint32_t Lseg, bool grad) {
 
 dr_status check_config(const dr_config* c) {
   if (!c) return fail(DR_ERR_INVALID_ARG, "config is null");
-  if (c->method < 0 || c->method > 4) return fail(DR_ERR_INVALID_ARG, "method out of range");
+  if (c->method < 0 || c->method > DR_PATH_TRACING) return fail(DR_ERR_INVALID_ARG, "method out of range");
+  if (c->rao_blackwell > 1) return fail(DR_ERR_INVALID_ARG, "rao_blackwell must be 0 or 1");
   if (c->n_chains < 1) return fail(DR_ERR_INVALID_ARG, "n_chains must be >= 1");
   if (!(c->stddev > 0.f) || !std::isfinite(c->stddev)) return fail(DR_ERR_INVALID_ARG, "stddev must be > 0");
   if (!(c->c_tilde >= 0.f) || !std::isfinite(c->c_tilde)) return fail(DR_ERR_INVALID_ARG, "c_tilde must be >= 0");
@@ -449,7 +450,8 @@ dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_stat
   dr_chains* h = new dr_chains();
   h->scene = s; h->cfg = *c;
   ChainParams& cp = h->cp;
-  cp.method = c->method; cp.restore = c->method >= DR_METROPOLIS_RESTORE; cp.grad = grad;
+  cp.method = c->method; cp.restore = c->method >= DR_METROPOLIS_RESTORE && c->method <= DR_DIFFUSION_RESTORE; cp.grad = grad;
+  cp.rao_blackwell = cp.restore && c->rao_blackwell;
   cp.N = c->n_chains; cp.d = s->dev.d; cp.planes = s->dev.planes;
   cp.stddev = c->stddev; cp.half_s2 = 0.5f * c->stddev * c->stddev; cp.c_tilde = c->c_tilde; cp.dt = c->dt; cp.m = c->m;
   cp.large_step_prob = cp.restore ? 0.f : c->large_step_prob;

@@ -23,6 +23,7 @@ struct ChainParams {
   int restore, grad;
   uint32_t N, d, planes;
   float stddev, half_s2, c_tilde, dt, m, large_step_prob, p_lambda_override;
+  int rao_blackwell;     // f3: weight = 1 / (lambda + kappa)
   uint64_t seed;
   uint32_t epoch;
   uint32_t chain_offset;  // global id of chain 0 (RNG keying)
@@ -71,7 +72,7 @@ __global__ void __launch_bounds__(kBlock) k_propose(ChainParams cp, ChainState s
   const uint32_t i = blockIdx.x * kBlock + threadIdx.x;
   if (i >= cp.N) return;
   uint32_t kind = 0;
-  if (init || (cp.restore && st.killed[i])) kind = 1;
+  if (init || (cp.restore && st.killed[i]) || cp.method == 5) kind = 1;   // path tracing: a fresh sample every iteration
   else if (!cp.restore) {
     const uint4 w = stream_block(cp.seed, cp.chain_offset + i, n, 0, P_DECIDE, cp.epoch);
     if (u01_co(w.x) < cp.large_step_prob) kind = 2;
@@ -210,6 +211,7 @@ __global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st
       }
       const float ph = fy.w + kEps;
       cur = make_float4(fy.x / ph, fy.y / ph, fy.z / ph, fy.w);   // f / p_hat (Alg. 1, Q9)
+      if (cp.method == 5) cur = fy;                               // path tracing accumulates f itself
       pix = st.pixy[i];
       st.fp[i] = cur;
       st.pix[i] = pix;
@@ -224,12 +226,13 @@ __global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st
       const float dt2 = -logf(u01_oc(w.w)) / kappa;           // L512
       killed = !(dt1 < dt2);                                  // L513 (tie -> killed)
       wgt = killed ? dt2 : dt1;
+      if (cp.rao_blackwell) wgt = 1.0f / (c->lambda + kappa);  // E[min(dt1, dt2)] (f3); the decision stays the race
       st.killed[i] = killed ? 1 : 0;
     }
     st.accepted[i] = take ? 1 : 0;
     st.weight[i] = wgt;
     do_splat = cur.w > 0.f;                                   // L522
-    contrib = make_float4(wgt * cur.x, wgt * cur.y, wgt * cur.z, wgt / phat);  // L524 (+ ratio denominator, Q12)
+    contrib = make_float4(wgt * cur.x, wgt * cur.y, wgt * cur.z, cp.method == 5 ? 1.0f : wgt / phat);  // L524 (+ ratio denominator, Q12; PT: count)
   }
   splat(accum, do_splat, pix, contrib);
   // block-level counts: kills (-> tourCount, regeneration queue) and MH accepts
@@ -313,6 +316,7 @@ __global__ void __launch_bounds__(kBlock) k_resolve(ChainParams cp, Counters* c,
   if (q == 0 && cp.restore && tours == 0) c->no_tour_resolves += 1;   // zero image, no division; reported by dr_chains_stats
   float scale;
   if (cp.restore) scale = tours ? (float)npix * c->kappa0 / (float)tours : 0.f;
+  else if (cp.method == 5) scale = mut ? (float)npix / (float)mut : 0.f;
   else scale = mut ? (float)npix * c->p_lambda / (float)mut : 0.f;
   const float4 a = accum[q];
   rgb[3 * q] = scale * a.x; rgb[3 * q + 1] = scale * a.y; rgb[3 * q + 2] = scale * a.z;

@@ -234,13 +234,28 @@ CASES = [("furnace", S.furnace, 4096), ("mini_machines", S.mini_machines, 5000),
 @pytest.mark.parametrize("method", METHODS)
 @pytest.mark.parametrize("case", CASES, ids=[c[0] for c in CASES])
 def test_teacher_forced_parity(dr, oracle, torch_, method, case):
+    _teacher_forced(dr, oracle, torch_, method, case)
+
+
+EXTRA = [("path_tracing", {}), ("metropolis_restore", dict(rao_blackwell=True)), ("mala_restore", dict(rao_blackwell=True)),
+         ("diffusion_restore", dict(rao_blackwell=True))]
+
+
+@pytest.mark.parametrize("variant", EXTRA, ids=[m + ("-rao_blackwell" if kw else "") for m, kw in EXTRA])
+@pytest.mark.parametrize("case", CASES[:2] + CASES[3:], ids=[c[0] for c in CASES[:2] + CASES[3:]])
+def test_teacher_forced_parity_pt_and_rao_blackwell(dr, oracle, torch_, variant, case):
+    """SURVEY 8f rows f2 (path tracing as a sixth method) and f3 (Rao-Blackwellised Accumulate), same protocol."""
+    _teacher_forced(dr, oracle, torch_, variant[0], case, **variant[1])
+
+
+def _teacher_forced(dr, oracle, torch_, method, case, **kw):
     name, make, N = case
     desc = make()
     seed = 0 if name == "furnace" else 3
     gsc = dr.Scene(desc)
     osc = oracle.Scene(desc, oracle.F32)
-    gch = dr.Chains(gsc, method, N, seed=seed)
-    och = oracle.Chains(osc, method, N, seed=seed)
+    gch = dr.Chains(gsc, method, N, seed=seed, **kw)
+    och = oracle.Chains(osc, method, N, seed=seed, **kw)
     stddev = float(gch.cfg.stddev)
     # --- init (Alg. 1) from the same seed: states are exact uniforms on both sides
     gch.init(2)
