@@ -28,7 +28,8 @@ struct Box {
 struct Node2 {
   Box box;
   uint32_t left = 0, right = 0;   // children (internal)
-  uint32_t first = 0, count = 0;  // leaf range into `order`
+  uint32_t first = 0, count = 0;  // range into `order`; count != 0 marks a BVH2 leaf
+  uint32_t refs = 0;              // references in the subtree = order[first, first + refs)
 };
 
 constexpr int kBins = 32;
@@ -41,6 +42,7 @@ struct Builder {
   const std::vector<float>& cen;  // 3 per triangle
   std::vector<uint32_t> order;
   std::vector<Node2> nodes;
+  uint32_t leaf_max = kMaxLeafTris;   // 1 when the optimal collapse decides the leaves
 
   Builder(const std::vector<Box>& b, const std::vector<float>& c) : tb(b), cen(c) {
     order.resize(b.size());
@@ -59,7 +61,8 @@ struct Builder {
     nodes[me].box = box;
     nodes[me].first = first;
     nodes[me].count = count;
-    if (count <= (uint32_t)kMaxLeafTris) return me;
+    nodes[me].refs = count;
+    if (count <= leaf_max) return me;
     // binned SAH over the three axes
     float best_cost = FLT_MAX;
     int best_axis = -1, best_bin = -1;
@@ -266,7 +269,16 @@ void assign_slots(const std::vector<Node2>& n2, const uint32_t* kids, int nk, in
 }  // namespace
 
 static double g_split_budget = DR_SPLIT_BUDGET;
+#ifndef DR_COLLAPSE_OPTIMAL
+#define DR_COLLAPSE_OPTIMAL 1
+#endif
+static bool g_optimal_collapse = DR_COLLAPSE_OPTIMAL != 0;
+#ifndef DR_COLLAPSE_COST_TRI
+#define DR_COLLAPSE_COST_TRI 0.4
+#endif
+static float kCostNode = 1.0f, kCostTri = (float)(DR_COLLAPSE_COST_TRI);   // relative cost of a BVH8 node test and of a triangle test in the collapse
 void set_split_budget(double extra_refs_per_triangle) { g_split_budget = extra_refs_per_triangle; }
+void set_collapse(bool optimal, float cost_node, float cost_tri) { g_optimal_collapse = optimal; kCostNode = cost_node; kCostTri = cost_tri; }
 
 void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t nt, const uint32_t* tri_mat, BuiltBvh& out) {
   (void)nv;
@@ -303,6 +315,7 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
     return;
   }
   Builder b(tb, cen);
+  b.leaf_max = g_optimal_collapse ? 1u : (uint32_t)kMaxLeafTris;
   b.build(0, nr);
   const std::vector<Node2>& n2 = b.nodes;
 
@@ -317,6 +330,66 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
   };
   out.tris.reserve(nr);
 
+  // ---- which BVH2 subtrees become the children of one BVH8 node
+  // g_optimal_collapse: the cost-optimal cut (dynamic programme over the BVH2, restated from section 3.1 of Ylitie, Karras
+  // and Laine 2017): cost[n][i] = least SAH cost of representing the subtree of n by at most i + 1 roots (leaves of at most
+  // kMaxLeafTris references, or BVH8 nodes), area(n) * kCostNode per node and area * refs * kCostTri per leaf.  The BVH2 is
+  // built down to single references, so the programme also decides what a leaf is.  Otherwise: greedy, open the child of
+  // largest area until there are eight.  Measured on configs[3]: profiles/r02b_bvh_collapse.md.
+  constexpr int kW = 8;
+  const size_t nn2 = n2.size();
+  std::vector<float> cost;          // [n * 7 + i], i = 0..6: at most i + 1 roots
+  std::vector<uint8_t> pick;        // [n * 8 + i]: i < 7: roots given to the left child when n is distributed over i + 1 roots
+                                    //   (0 = not distributed: same as i - 1, or for i = 0 one root: see kind); [n * 8 + 7]: for the 8-way distribution of a node
+  std::vector<uint8_t> kind;        // [n]: 1 = a single root at n is a leaf, 0 = a BVH8 node
+  if (g_optimal_collapse) {
+    cost.assign(nn2 * 7, 0.f); pick.assign(nn2 * 8, 0); kind.assign(nn2, 0);
+    for (size_t n = nn2; n-- > 0;) {   // children have larger indices than their parent (pre-order)
+      const Node2& N = n2[n];
+      const float A = N.box.area();
+      float* c = &cost[n * 7];
+      if (N.count) {                   // BVH2 leaf: one reference
+        for (int i = 0; i < 7; ++i) c[i] = A * kCostTri * (float)N.refs;
+        kind[n] = 1;
+        continue;
+      }
+      const float* cl = &cost[(size_t)N.left * 7];
+      const float* cr = &cost[(size_t)N.right * 7];
+      auto distribute = [&](int roots, uint8_t& k_best) {   // roots >= 2 split between the two children
+        float best = FLT_MAX;
+        for (int k = 1; k < roots; ++k) {
+          if (k > 7 || roots - k > 7) continue;
+          const float v = cl[k - 1] + cr[roots - k - 1];
+          if (v < best) { best = v; k_best = (uint8_t)k; }
+        }
+        return best;
+      };
+      uint8_t k8 = 1;
+      const float as_node = A * kCostNode + distribute(kW, k8);
+      pick[n * 8 + 7] = k8;
+      const float as_leaf = N.refs <= (uint32_t)kMaxLeafTris ? A * kCostTri * (float)N.refs : FLT_MAX;
+      kind[n] = as_leaf <= as_node ? 1 : 0;
+      c[0] = std::min(as_leaf, as_node);
+      for (int i = 1; i < 7; ++i) {
+        uint8_t k = 0;
+        const float d = distribute(i + 1, k);
+        if (d < c[i - 1]) { c[i] = d; pick[n * 8 + i] = k; } else { c[i] = c[i - 1]; pick[n * 8 + i] = 0; }
+      }
+    }
+  }
+  // roots of the subtree of n when it may use `roots` of them
+  struct Expand {
+    const std::vector<Node2>& n2; const std::vector<uint8_t>& pick;
+    void run(uint32_t n, int roots, uint32_t* out, int& cnt) const {
+      while (roots > 1 && pick[(size_t)n * 8 + roots - 1] == 0) --roots;   // fewer roots were as good
+      if (roots == 1 || n2[n].count) { out[cnt++] = n; return; }
+      const int k = pick[(size_t)n * 8 + roots - 1];
+      run(n2[n].left, k, out, cnt);
+      run(n2[n].right, roots - k, out, cnt);
+    }
+  };
+  auto is_leaf = [&](uint32_t n) { return g_optimal_collapse ? kind[n] != 0 : n2[n].count != 0; };
+
   // collapse to BVH8, breadth-first; a node's index is its position in the queue order
   struct Item { uint32_t n2; uint32_t depth; };
   std::queue<Item> q;
@@ -330,18 +403,28 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
     out.depth = std::max(out.depth, it.depth);
     uint32_t kids[8];
     int nk = 0;
-    if (n2[it.n2].count) kids[nk++] = it.n2;  // the root is itself a leaf
-    else { kids[nk++] = n2[it.n2].left; kids[nk++] = n2[it.n2].right; }
-    for (;;) {  // open the internal child with the largest area until 8 children
-      if (nk == 8) break;
-      int pick = -1;
-      float pa = -1.f;
-      for (int i = 0; i < nk; ++i)
-        if (!n2[kids[i]].count && n2[kids[i]].box.area() > pa) { pa = n2[kids[i]].box.area(); pick = i; }
-      if (pick < 0) break;
-      const uint32_t p = kids[pick];
-      kids[pick] = n2[p].left;
-      kids[nk++] = n2[p].right;
+    if (g_optimal_collapse) {
+      if (it.n2 == 0 && n2[0].refs <= (uint32_t)kMaxLeafTris) { kind[0] = 1; kids[nk++] = 0; }   // the whole scene is one leaf
+      else {
+        const int k = pick[(size_t)it.n2 * 8 + 7];
+        const Expand ex{n2, pick};
+        ex.run(n2[it.n2].left, k, kids, nk);
+        ex.run(n2[it.n2].right, kW - k, kids, nk);
+      }
+    } else {
+      if (n2[it.n2].count) kids[nk++] = it.n2;  // the root is itself a leaf
+      else { kids[nk++] = n2[it.n2].left; kids[nk++] = n2[it.n2].right; }
+      for (;;) {  // open the internal child with the largest area until 8 children
+        if (nk == 8) break;
+        int pick_i = -1;
+        float pa = -1.f;
+        for (int i = 0; i < nk; ++i)
+          if (!n2[kids[i]].count && n2[kids[i]].box.area() > pa) { pa = n2[kids[i]].box.area(); pick_i = i; }
+        if (pick_i < 0) break;
+        const uint32_t p = kids[pick_i];
+        kids[pick_i] = n2[p].left;
+        kids[nk++] = n2[p].right;
+      }
     }
     int slot_of[8];
     assign_slots(n2, kids, nk, slot_of);
@@ -389,10 +472,10 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
     for (int s = 0; s < 8; ++s) {
       if (kid_in_slot[s] < 0) continue;
       const Node2& c = n2[kids[kid_in_slot[s]]];
-      if (c.count) {
-        node.trimask |= ((1u << c.count) - 1u) << (3 * s);
-        for (uint32_t k = 0; k < c.count; ++k) emit_tri(refs[b.order[c.first + k]].tri);
-        sah += (double)c.box.area() / root_area * c.count;
+      if (is_leaf(kids[kid_in_slot[s]])) {
+        node.trimask |= ((1u << c.refs) - 1u) << (3 * s);
+        for (uint32_t k = 0; k < c.refs; ++k) emit_tri(refs[b.order[c.first + k]].tri);
+        sah += (double)c.box.area() / root_area * c.refs;
       } else {
         node.imask |= (uint8_t)(1u << s);
         ++next_index;

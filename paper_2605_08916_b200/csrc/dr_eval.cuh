@@ -34,7 +34,7 @@ namespace dr {
 #define DR_TRI_LD __ldg
 #endif
 #ifndef DR_FETCH_CHUNK
-#define DR_FETCH_CHUNK 16
+#define DR_FETCH_CHUNK 32
 #endif
 constexpr int kTraceBlock = DR_TRACE_BLOCK;   // one persistent block per SM
 constexpr int kTriStack = DR_TRI_STACK;      // postponed triangle groups per ray

@@ -74,6 +74,7 @@ struct BuiltBvh {
 
 // Binned-SAH BVH2 -> BVH8 collapse -> slot assignment -> quantisation (host).  verts: 3*nv floats, idx: 3*nt, tri_mat: nt.
 void set_split_budget(double extra_refs_per_triangle);  // tuning hook (default DR_SPLIT_BUDGET)
+void set_collapse(bool optimal, float cost_node, float cost_tri);   // tuning hook: BVH2 -> BVH8 collapse (dr_bvh.cpp)
 void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t nt, const uint32_t* tri_mat, BuiltBvh& out);
 
 }  // namespace dr

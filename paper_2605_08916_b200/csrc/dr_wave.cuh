@@ -55,7 +55,10 @@ enum : uint32_t { kErrIndex = 1u, kErrState = 2u, kErrOwner = 4u, kErrSegment = 
 constexpr int kWaveShadeWarps = DR_WAVE_SHADE_WARPS;     // sweep 1 / 2 / 3 / 4 / 5 / 6: 9.13 / 5.25 / 4.85 / 5.05 / 5.22 / 5.45 ms per frame
 constexpr int kWaveRefillBelow = DR_WAVE_REFILL_BELOW;   // a trace warp flushes its finished rays and refills below this many busy lanes
 constexpr int kWaveTraceThreads = kTraceBlock - 32 * kWaveShadeWarps;
-constexpr uint32_t kHitCap = 1024;   // entries of the block's ring of finished rays (power of two)
+#ifndef DR_WAVE_HIT_CAP
+#define DR_WAVE_HIT_CAP 1024
+#endif
+constexpr uint32_t kHitCap = DR_WAVE_HIT_CAP;   // entries of the block's ring of finished rays (power of two)
 constexpr uint32_t kWaveKShift = 27; // payload = state | (k - 1) << 27
 constexpr uint32_t kWaveStateMask = (1u << kWaveKShift) - 1u;
 

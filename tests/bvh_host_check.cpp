@@ -59,6 +59,7 @@ int main(int argc, char** argv) {
   const uint32_t nt = (uint32_t)(idx.size() / 3), nv = (uint32_t)(v.size() / 3);
 
   set_split_budget(budget);
+  if (argc > 4) set_collapse(atoi(argv[4]) != 0, 1.0f, 0.4f);   // 1 = cost-optimal BVH2 -> BVH8 collapse (the default), 0 = greedy
   BuiltBvh b;
   build_bvh8(v.data(), nv, idx.data(), nt, mat.data(), b);
 

@@ -54,3 +54,13 @@ def test_tiny_and_single_triangle_scenes(exe):
     for n in (1, 2, 9):
         r = run(exe, 1.0, n, 2000)
         assert r["mismatch"] == 0 and r["bad_node"] == 0 and r["referenced"] == r["tris"]
+
+
+def test_optimal_collapse_beats_greedy(exe):
+    """The cost-optimal BVH2 -> BVH8 cut (dr_bvh.cpp) changes no hit and needs fewer nodes, node tests and triangle
+    tests per ray than opening the largest child until there are eight."""
+    a, b = run(exe, 1.0, 6000, 6000, 0), run(exe, 1.0, 6000, 6000, 1)
+    assert a["mismatch"] == 0 and b["mismatch"] == 0 and a["hits"] == b["hits"]
+    assert b["nodes"] < 0.9 * a["nodes"]
+    cost = lambda r: r["nodes_per_ray"] + 0.4 * r["tris_per_ray"]     # the collapse's own weights
+    assert cost(b) < cost(a) and b["tris_per_ray"] < a["tris_per_ray"]

@@ -144,7 +144,7 @@ def test_tie_rule_coincident_triangles(dr, oracle, torch_):
     mism = prim != otri
     assert mism.mean() < 1e-4, mism.sum()
     ok = ~mism & hit
-    assert np.all(np.abs(t[ok] - ot[ok]) <= 2e-6 * np.abs(ot[ok]))
+    assert np.all(np.abs(t[ok] - ot[ok]) <= 1e-5 * np.maximum(np.abs(ot[ok]), 1.0))     # scene extent 4
 
 
 def test_tie_rule_coplanar_box_on_floor(dr, oracle, torch_):
