@@ -235,32 +235,52 @@ def main():
     mutations = n_local * world * args.steps
     value = mutations / (total_ms * 1e-3)
 
-    # ---- end to end: host owns the chain state; every step uploads it, steps, resolves, and reads image + state back
+    # ---- end to end (1): host owns the chain state; every step uploads it from pinned host memory, steps, resolves, and
+    # reads image + state back into pinned host memory (dr_chains_upload / dr_chains_download: DMA + transposition kernels)
     e2e = None
     if rank == 0:
+        names = ("x", "p", "fop", "pix", "killed", "g", "sig")
         st = chains.download()
-        host = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in st.items()}
+        host = {k: torch.from_numpy(np.ascontiguousarray(st[k])).pin_memory() for k in names}
+        views = {k: host[k].numpy() for k in names}
         img_host = torch.empty(desc.height, desc.width, 3, dtype=torch.float32).pin_memory()
-        h2d = sum(host[k].numel() * host[k].element_size() for k in ("x", "p", "fop", "pix", "killed", "g", "sig"))
+        h2d = sum(host[k].numel() * host[k].element_size() for k in names)
         d2h = h2d + img_host.numel() * 4
         it = st1["iteration"]
+        for k in range(2):                                   # warm-up: staging buffers are allocated on first use
+            chains.upload(views, it)
+            chains.download(views)
         torch.cuda.synchronize()
         e0.record(stream)
         for k in range(args.e2e_steps):
-            chains.upload({kk: vv.numpy() for kk, vv in host.items()}, it + k)
+            chains.upload(views, it + k)
             chains.step(1)
             img, _ = chains.resolve()
             img_host.copy_(img, non_blocking=True)
-            st = chains.download()
-            for kk in host:
-                host[kk].copy_(torch.from_numpy(st[kk]))
+            chains.download(views)
         e1.record(stream)
         torch.cuda.synchronize()
         e2e_ms = e0.elapsed_time(e1)
+        # ---- end to end (2): the renderer's own per-frame boundary (chains persist across frames on the device):
+        # dr_step(1) + dr_resolve_image, image read back to pinned host memory every frame
+        e0.record(stream)
+        for k in range(args.e2e_steps):
+            chains.step(1)
+            img, _ = chains.resolve()
+            img_host.copy_(img, non_blocking=True)
+            stream.synchronize()                             # the host has the frame
+        e1.record(stream)
+        torch.cuda.synchronize()
+        res_ms = e0.elapsed_time(e1)
         e2e = {"value": n_local * args.e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / args.e2e_steps, "steps": args.e2e_steps,
                "what": "host-owned chain state: dr_chains_upload (pinned host -> device) + dr_step(1) + dr_resolve_image + "
-                       "image and dr_chains_download back to host, every step, N = 1 GPU"}
+                       "image and dr_chains_download back to pinned host memory, every step, N = 1 GPU",
+               "resident_state_frame": {"value": n_local * args.e2e_steps / (res_ms * 1e-3), "unit": UNIT,
+                                        "ms_per_step": res_ms / args.e2e_steps, "h2d_bytes_per_step": 0,
+                                        "d2h_bytes_per_step": int(img_host.numel() * 4),
+                                        "what": "chain state resident on the device (PAPER.md L482): dr_step(1) + "
+                                                "dr_resolve_image + image to pinned host memory, host waits for every frame"}}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -279,15 +299,17 @@ def main():
     stream_ms = sum(prof[k]["ms"] for k in ("propose", "decide", "scan", "scatter")) / prof_frames
     stream_gbs = stream_bytes_per_mutation(desc.dim, grad) * n_local / (stream_ms * 1e-3) / 1e9
     launches_per_frame = sum(v["launches"] for v in prof.values()) / prof_frames
-    traffic = None
-    # large evaluations run traversal + shading of all segments as one persistent kernel (k_wave, one launch per frame);
-    # small ones, or DR_WAVE=0, the per-segment loop (k_trace + k_shade, L launches each per frame)
+    # evaluations below 2^21 states run traversal + shading of all segments as one persistent kernel (k_wave, one launch per
+    # frame); larger ones the per-segment loop (k_trace + k_shade, L launches each per frame)
     wave = prof["shade"]["launches"] == 0
-    tp = os.path.join(ROOT, "profiles", "trace_traffic.txt")     # from the last ncu --set full capture of that kernel
+    cap = {}                                                      # counters of the last ncu --set full capture of that kernel
+    tp = os.path.join(ROOT, "profiles", "trace_traffic.txt")
     if os.path.exists(tp):
         for line in open(tp):
-            if line.startswith("dram_bytes_per_launch_k_wave" if wave else "dram_bytes_per_launch_k_trace"):
-                traffic = int(line.split()[1])
+            f = line.split()
+            if len(f) == 2 and f[0].endswith("_k_wave" if wave else "_k_trace"):
+                cap[f[0].rsplit("_k_", 1)[0]] = float(f[1])
+    traffic = int(cap["dram_bytes_per_launch"]) if "dram_bytes_per_launch" in cap else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -302,13 +324,18 @@ def main():
         "init_ms": init_ms,
         "workload_stats": {"rays_per_mutation": rays_local / (n_local * args.steps), "nodes_per_ray": nodes_per_ray,
                            "tris_per_ray": tris_per_ray, "kill_fraction_last": st1["kills_last_step"] / n_local,
-                           "tours": st1["tours"], "p_lambda": st1["p_lambda"], "nonfinite": st1["nonfinite"]},
+                           "tours": st1["tours"], "p_lambda": st1["p_lambda"], "nonfinite": st1["nonfinite"],
+                           "zeta_lit_fraction_of_uniform_samples": st1["lit_init"] / n_local,
+                           "mh_acceptance_rate": (st1["mh_accepts"] - st0["mh_accepts"]) / (n_local * args.steps) if args.method in ("metropolis", "mala", "metropolis_restore", "mala_restore") else None,
+                           "grad_list_share_of_evaluations": (st1["grad_states"] - st0["grad_states"]) / (n_local * args.steps)},
         "kernels_ms_per_frame": {k: v["ms"] / prof_frames for k, v in prof.items()},
         "kernel_launches_per_frame": launches_per_frame,
         "gpu_launches": int(round(launches_per_frame * args.steps)),
         "clocks": clocks,
         "roofline": {"kernel": "k_wave" if wave else "k_trace", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                      "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": traffic,
+                     "traffic_source": "ncu --set full capture, profiles/trace_traffic.txt (not measured in this run)",
+                     "ncu_capture": {k: v for k, v in cap.items() if k != "dram_bytes_per_launch"},
                      "peak_source": f"148 SM x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} sm_max_mhz)",
                      "flop_per_ray": flop_per_ray, "rays_per_launch": rays_per_launch, "launch_ms": trace_ms,
                      "grays_per_s_in_kernel": rays_per_launch / (trace_ms * 1e-3) / 1e9},

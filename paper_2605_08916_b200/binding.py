@@ -58,7 +58,7 @@ class dr_stats(C.Structure):
     _fields_ = [("tours", C.c_uint64), ("mutations", C.c_uint64), ("rays", C.c_uint64), ("mh_accepts", C.c_uint64),
                 ("nonfinite", C.c_uint64), ("kills_last_step", C.c_uint32), ("regen_queue_len", C.c_uint32),
                 ("iteration", C.c_uint32), ("p_lambda", C.c_float), ("kappa0", C.c_float), ("lambda_", C.c_float),
-                ("no_tour_resolves", C.c_uint32)]
+                ("no_tour_resolves", C.c_uint32), ("grad_states", C.c_uint64), ("lit_init", C.c_uint64)]
 
 
 class dr_scene_info(C.Structure):
@@ -293,11 +293,14 @@ class Chains:
         d["lambda"] = d.pop("lambda_")
         return d
 
-    def download(self) -> dict:
+    def download(self, out: dict | None = None) -> dict:
+        """Chain state as row-major host arrays.  `out`: arrays to fill (e.g. numpy views of pinned torch tensors, which
+        the copies then reach by DMA); default: fresh numpy arrays."""
         N, d = self.N, self.d
-        s = dict(x=np.zeros((N, d), np.float32), p=np.zeros(N, np.float32), fop=np.zeros((N, 3), np.float32),
-                 pix=np.zeros(N, np.uint32), killed=np.zeros(N, np.uint8), g=np.zeros((N, d), np.float32),
-                 sig=np.zeros(N, np.uint32))
+        s = out if out is not None else dict(
+            x=np.empty((N, d), np.float32), p=np.empty(N, np.float32), fop=np.empty((N, 3), np.float32),
+            pix=np.empty(N, np.uint32), killed=np.empty(N, np.uint8), g=np.empty((N, d), np.float32),
+            sig=np.empty(N, np.uint32))
         _check(lib.dr_chains_download(self.h, _np(s["x"]), _np(s["p"]), _np(s["fop"]), _np(s["pix"]), _np(s["killed"]),
                                       _np(s["g"]), _np(s["sig"]), _stream()))
         return s

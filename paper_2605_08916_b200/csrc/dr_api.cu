@@ -78,7 +78,8 @@ struct dr_chains {
   EvalWs ws{};
   uint32_t eval_tag = 0;           // k_wave: tag of the last evaluation (dr_wave.cuh)
   int eval_form = 0;               // test hook dr_chains_set_eval_form: 0 = default choice, 1 = per-segment loop, 2 = k_wave
-  ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
+  void* hook_scratch = nullptr;    // device staging of dr_chains_download / _upload (row-major copies), allocated on first use
+  ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); cudaFree(hook_scratch); }
 };
 
 namespace {
@@ -239,7 +240,7 @@ EvalIO chain_io(const dr_chains* c, bool use_order) {
   EvalIO io{};
   io.x = c->st.y; io.stride = c->cp.N; io.order = use_order ? c->st.order : nullptr;
   io.g = c->st.gy; io.f = c->st.fy; io.pix = c->st.pixy; io.sig = c->st.sigy; io.nrays = nullptr;
-  io.rays_ctr = &c->st.ctr->rays; io.nonfinite_ctr = &c->st.ctr->nonfinite; io.work = nullptr;
+  io.rays_ctr = &c->st.ctr->rays; io.nonfinite_ctr = &c->st.ctr->nonfinite; io.work = nullptr; io.grad_ctr = &c->st.ctr->grad_states;
   return io;
 }
 
@@ -579,7 +580,7 @@ dr_status dr_chains_work_stats(dr_chains* c, uint64_t* host_out3, void* stream) 
   CUDA_TRY(cudaMemsetAsync(d.p, 0, 24, s));
   // re-evaluates the last proposals (same values are written again) with the counting variant of k_trace
   EvalIO io = chain_io(c, false);
-  io.rays_ctr = d.as<unsigned long long>(); io.nonfinite_ctr = nullptr; io.work = d.as<unsigned long long>() + 1;
+  io.rays_ctr = d.as<unsigned long long>(); io.nonfinite_ctr = nullptr; io.work = d.as<unsigned long long>() + 1; io.grad_ctr = nullptr;
   if (c->cp.grad) CUDA_TRY(cudaMemsetAsync(c->st.gy, 0, sizeof(float4) * (size_t)c->cp.planes * c->cp.N, s));
   const dr_status r = launch_eval(nullptr, c->scene, next_ws(c, s), io, c->cp.N, c->cp.grad != 0, true, 0, s);
   if (r != DR_OK) return r;
@@ -596,39 +597,44 @@ dr_status dr_chains_stats(dr_chains* c, dr_stats* o, void* stream) {
   o->tours = h.tours; o->mutations = h.mutations; o->rays = h.rays; o->mh_accepts = h.mh_accepts; o->nonfinite = h.nonfinite;
   o->kills_last_step = h.kills_last; o->regen_queue_len = h.queue_len; o->iteration = c->iteration;
   o->p_lambda = h.p_lambda; o->kappa0 = h.kappa0; o->lambda = h.lambda; o->no_tour_resolves = h.no_tour_resolves;
+  o->grad_states = h.grad_states; o->lit_init = h.lit_init;
   if (h.no_tour_resolves) { g_err = "a resolve ran before any tour had completed: zero image"; return DR_WARN_NO_TOURS; }
   return DR_OK;
 }
 
 // ---- test hooks ---------------------------------------------------------------------------------------------
+// Staging layout of the two hooks: x rows | score rows | p | f/p_hat   (N * (8 d + 16) bytes, kept for the life of the chains)
+namespace {
+struct HookStage { float *x, *g, *p, *fop; };
+dr_status hook_stage(dr_chains* c, HookStage& st) {
+  const size_t N = c->cp.N, d = c->cp.d;
+  if (!c->hook_scratch) CUDA_TRY(cudaMalloc(&c->hook_scratch, sizeof(float) * N * (2 * d + 4)));
+  st.x = (float*)c->hook_scratch; st.g = st.x + N * d; st.p = st.g + N * d; st.fop = st.p + N;
+  return DR_OK;
+}
+}  // namespace
+
 dr_status dr_chains_download(dr_chains* c, float* hx, float* hp, float* hfop, uint32_t* hpix, uint8_t* hkilled, float* hscore,
                              uint32_t* hsig, void* stream) {
   if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
   cudaStream_t s = (cudaStream_t)stream;
   const uint32_t N = c->cp.N, d = c->cp.d, g = (N + 255) / 256;
-  float* tmp = nullptr;
-  CUDA_TRY(cudaMalloc(&tmp, sizeof(float) * (size_t)N * (d > 4 ? d : 4)));
-  dr_status r = DR_OK;
-  auto rows = [&](const float4* planes, float* host) -> cudaError_t {
-    k_planes_to_rows<<<g, 256, 0, s>>>(planes, tmp, N, d, c->cp.planes);
-    return cudaMemcpyAsync(host, tmp, sizeof(float) * (size_t)N * d, cudaMemcpyDeviceToHost, s);
-  };
-  cudaError_t e = cudaSuccess;
-  if (hx) e = rows(c->st.x, hx);
-  if (e == cudaSuccess && hscore) {
-    if (c->cp.grad) e = rows(c->st.g, hscore);
-    else { e = cudaStreamSynchronize(s); std::memset(hscore, 0, sizeof(float) * (size_t)N * d); }
-  }
-  if (e == cudaSuccess && hp) { k_fp_split<<<g, 256, 0, s>>>(c->st.fp, tmp, nullptr, N); e = cudaMemcpyAsync(hp, tmp, 4 * (size_t)N, cudaMemcpyDeviceToHost, s); }
-  if (e == cudaSuccess && hfop) { k_fp_split<<<g, 256, 0, s>>>(c->st.fp, nullptr, tmp, N); e = cudaMemcpyAsync(hfop, tmp, 12 * (size_t)N, cudaMemcpyDeviceToHost, s); }
-  if (e == cudaSuccess && hpix) e = cudaMemcpyAsync(hpix, c->st.pix, 4 * (size_t)N, cudaMemcpyDeviceToHost, s);
-  if (e == cudaSuccess && hsig) e = cudaMemcpyAsync(hsig, c->st.sig, 4 * (size_t)N, cudaMemcpyDeviceToHost, s);
-  if (e == cudaSuccess && hkilled) e = cudaMemcpyAsync(hkilled, c->st.killed, N, cudaMemcpyDeviceToHost, s);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  if (e == cudaSuccess) e = cudaGetLastError();
-  cudaFree(tmp);
-  if (e != cudaSuccess) r = fail(DR_ERR_CUDA, std::string("download: ") + cudaGetErrorString(e));
-  return r;
+  HookStage st;
+  const dr_status rs = hook_stage(c, st);
+  if (rs != DR_OK) return rs;
+  // every conversion kernel and copy is queued on the stream; one synchronisation at the end (pinned host arrays copy by DMA)
+  if (hx) { k_planes_to_rows<<<g, 256, 0, s>>>(c->st.x, st.x, N, d, c->cp.planes); CUDA_TRY(cudaMemcpyAsync(hx, st.x, sizeof(float) * (size_t)N * d, cudaMemcpyDeviceToHost, s)); }
+  if (hscore && c->cp.grad) { k_planes_to_rows<<<g, 256, 0, s>>>(c->st.g, st.g, N, d, c->cp.planes); CUDA_TRY(cudaMemcpyAsync(hscore, st.g, sizeof(float) * (size_t)N * d, cudaMemcpyDeviceToHost, s)); }
+  if (hp || hfop) k_fp_split<<<g, 256, 0, s>>>(c->st.fp, hp ? st.p : nullptr, hfop ? st.fop : nullptr, N);
+  if (hp) CUDA_TRY(cudaMemcpyAsync(hp, st.p, 4 * (size_t)N, cudaMemcpyDeviceToHost, s));
+  if (hfop) CUDA_TRY(cudaMemcpyAsync(hfop, st.fop, 12 * (size_t)N, cudaMemcpyDeviceToHost, s));
+  if (hpix) CUDA_TRY(cudaMemcpyAsync(hpix, c->st.pix, 4 * (size_t)N, cudaMemcpyDeviceToHost, s));
+  if (hsig) CUDA_TRY(cudaMemcpyAsync(hsig, c->st.sig, 4 * (size_t)N, cudaMemcpyDeviceToHost, s));
+  if (hkilled) CUDA_TRY(cudaMemcpyAsync(hkilled, c->st.killed, N, cudaMemcpyDeviceToHost, s));
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaStreamSynchronize(s));
+  if (hscore && !c->cp.grad) std::memset(hscore, 0, sizeof(float) * (size_t)N * d);
+  return DR_OK;
 }
 
 dr_status dr_chains_upload(dr_chains* c, const float* hx, const float* hp, const float* hfop, const uint32_t* hpix,
@@ -638,30 +644,28 @@ dr_status dr_chains_upload(dr_chains* c, const float* hx, const float* hp, const
   if (!c->initialised) return fail(DR_ERR_INVALID_ARG, "dr_chains_init has not been called");
   cudaStream_t s = (cudaStream_t)stream;
   const uint32_t N = c->cp.N, d = c->cp.d, g = (N + 255) / 256;
-  float *t0 = nullptr, *t1 = nullptr;
-  CUDA_TRY(cudaMalloc(&t0, sizeof(float) * (size_t)N * (d > 4 ? d : 4)));
-  cudaError_t e = cudaMalloc(&t1, sizeof(float) * (size_t)N * 4);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(t0, hx, sizeof(float) * (size_t)N * d, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) k_rows_to_planes<<<g, 256, 0, s>>>(t0, c->st.x, N, d, c->cp.planes);
-  if (e == cudaSuccess && c->cp.grad) {
-    e = cudaMemcpyAsync(t0, hscore, sizeof(float) * (size_t)N * d, cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess) k_rows_to_planes<<<g, 256, 0, s>>>(t0, c->st.g, N, d, c->cp.planes);
+  HookStage st;
+  const dr_status rs = hook_stage(c, st);
+  if (rs != DR_OK) return rs;
+  CUDA_TRY(cudaMemcpyAsync(st.x, hx, sizeof(float) * (size_t)N * d, cudaMemcpyHostToDevice, s));
+  k_rows_to_planes<<<g, 256, 0, s>>>(st.x, c->st.x, N, d, c->cp.planes);
+  if (c->cp.grad) {
+    CUDA_TRY(cudaMemcpyAsync(st.g, hscore, sizeof(float) * (size_t)N * d, cudaMemcpyHostToDevice, s));
+    k_rows_to_planes<<<g, 256, 0, s>>>(st.g, c->st.g, N, d, c->cp.planes);
   }
-  if (e == cudaSuccess) e = cudaMemcpyAsync(t0, hp, 4 * (size_t)N, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(t1, hfop, 12 * (size_t)N, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) k_fp_join<<<g, 256, 0, s>>>(t0, t1, c->st.fp, N);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(c->st.pix, hpix, 4 * (size_t)N, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(c->st.killed, hkilled, N, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess && hsig) e = cudaMemcpyAsync(c->st.sig, hsig, 4 * (size_t)N, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess && c->cp.restore) {
+  CUDA_TRY(cudaMemcpyAsync(st.p, hp, 4 * (size_t)N, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(cudaMemcpyAsync(st.fop, hfop, 12 * (size_t)N, cudaMemcpyHostToDevice, s));
+  k_fp_join<<<g, 256, 0, s>>>(st.p, st.fop, c->st.fp, N);
+  CUDA_TRY(cudaMemcpyAsync(c->st.pix, hpix, 4 * (size_t)N, cudaMemcpyHostToDevice, s));
+  CUDA_TRY(cudaMemcpyAsync(c->st.killed, hkilled, N, cudaMemcpyHostToDevice, s));
+  if (hsig) CUDA_TRY(cudaMemcpyAsync(c->st.sig, hsig, 4 * (size_t)N, cudaMemcpyHostToDevice, s));
+  if (c->cp.restore) {
     k_count_killed<<<c->nblocks, kBlock, 0, s>>>(c->cp, c->st);
     k_scan<<<1, 1024, 0, s>>>(c->st, c->nblocks);
     k_scatter<<<c->nblocks, kBlock, 0, s>>>(c->cp, c->st);
   }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  if (e == cudaSuccess) e = cudaGetLastError();
-  cudaFree(t0); cudaFree(t1);
-  if (e != cudaSuccess) return fail(DR_ERR_CUDA, std::string("upload: ") + cudaGetErrorString(e));
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaStreamSynchronize(s));   // the host arrays may be reused on return
   c->iteration = iteration;
   return DR_OK;
 }

@@ -83,6 +83,7 @@ struct EvalIO {
   unsigned long long* rays_ctr;       // optional: += closest-hit queries
   unsigned long long* nonfinite_ctr;  // optional: += states with non-finite f or score (Q18)
   unsigned long long* work;           // optional (k_trace<true>): work[0] += node visits, work[1] += triangle tests
+  unsigned long long* grad_ctr;       // optional: += states that ran the reverse pass (k_grad)
 };
 
 __device__ __forceinline__ float2 x_pair(const EvalIO& io, uint32_t s, uint32_t k) {  // coordinates (2k, 2k+1)
@@ -472,6 +473,7 @@ __global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, E
 // vertices to the first diffuse vertex or the camera ("Score").  One thread = one listed state.
 __global__ void __launch_bounds__(kGradBlock) k_grad(DevScene sc, EvalWs ws, EvalIO io) {
   const uint32_t idx = blockIdx.x * kGradBlock + threadIdx.x;
+  if (idx == 0 && io.grad_ctr) atomicAdd(io.grad_ctr, (unsigned long long)ws.ctl[kCtlGrad]);
   if (idx >= ws.ctl[kCtlGrad]) return;
   const uint32_t s = ws.gradlist[idx];
   const size_t cap = ws.cap;

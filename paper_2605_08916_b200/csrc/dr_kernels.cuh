@@ -12,7 +12,7 @@ namespace dr {
 constexpr int kBlock = 256;      // streaming kernels
 
 struct Counters {
-  unsigned long long tours, mutations, rays, mh_accepts, nonfinite;
+  unsigned long long tours, mutations, rays, mh_accepts, nonfinite, grad_states, lit_init;
   uint32_t kills_last, queue_len, iteration, no_tour_resolves;
   float p_lambda, kappa0, lambda, pad2;
   double psum;
@@ -175,13 +175,14 @@ __global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st
   const uint32_t i = blockIdx.x * kBlock + threadIdx.x;
   const bool in = i < cp.N;
   const Counters* c = st.ctr;
-  bool killed = false, accepted_mh = false, do_splat = false;
+  bool killed = false, accepted_mh = false, do_splat = false, lit0 = false;
   uint32_t pix = 0;
   float4 contrib = make_float4(0.f, 0.f, 0.f, 0.f);
   if (in) {
     const uint4 w = stream_block(cp.seed, cp.chain_offset + i, n, 0, P_DECIDE, cp.epoch);
     const uint32_t kind = st.kind[i];
     const float4 fy = st.fy[i];
+    lit0 = n == 0 && fy.w > 0.f;   // init pass: uniform samples with a contribution (zeta of SURVEY.md 8d)
     float4 cur = st.fp[i];
     pix = st.pix[i];
     bool take = true;
@@ -236,19 +237,21 @@ __global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st
   }
   splat(accum, do_splat, pix, contrib);
   // block-level counts: kills (-> tourCount, regeneration queue) and MH accepts
-  __shared__ uint32_t s_k, s_a;
-  if (threadIdx.x == 0) { s_k = 0; s_a = 0; }
+  __shared__ uint32_t s_k, s_a, s_l;
+  if (threadIdx.x == 0) { s_k = 0; s_a = 0; s_l = 0; }
   __syncthreads();
-  const unsigned kb = __ballot_sync(0xFFFFFFFFu, killed), ab = __ballot_sync(0xFFFFFFFFu, accepted_mh);
+  const unsigned kb = __ballot_sync(0xFFFFFFFFu, killed), ab = __ballot_sync(0xFFFFFFFFu, accepted_mh), lb = __ballot_sync(0xFFFFFFFFu, lit0);
   if ((threadIdx.x & 31) == 0) {
     if (kb) atomicAdd(&s_k, (uint32_t)__popc(kb));
     if (ab) atomicAdd(&s_a, (uint32_t)__popc(ab));
+    if (lb) atomicAdd(&s_l, (uint32_t)__popc(lb));
   }
   __syncthreads();
   if (threadIdx.x == 0) {
     st.blockcnt[blockIdx.x] = s_k;
     if (s_k) atomicAdd(&st.ctr->tours, (unsigned long long)s_k);
     if (s_a) atomicAdd(&st.ctr->mh_accepts, (unsigned long long)s_a);
+    if (s_l) atomicAdd(&st.ctr->lit_init, (unsigned long long)s_l);
     if (blockIdx.x == 0) {
       atomicAdd(&st.ctr->mutations, (unsigned long long)cp.N);
       st.ctr->iteration = n;

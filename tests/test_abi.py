@@ -29,7 +29,7 @@ def test_binding_lists_the_same_names():
     # struct sizes match the C layout
     assert ctypes.sizeof(binding.dr_material) == 36
     assert ctypes.sizeof(binding.dr_config) == 48
-    assert ctypes.sizeof(binding.dr_stats) == 72
+    assert ctypes.sizeof(binding.dr_stats) == 88
     assert ctypes.sizeof(binding.dr_scene_info) == 32
 
 
