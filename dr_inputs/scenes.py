@@ -33,10 +33,11 @@ class SceneDesc:
     max_path_len: int = 4
     name: str = ""
     meta: dict = field(default_factory=dict)
+    nee: bool = False             # next-event estimation + MIS (Q21): four PSS coordinates per vertex
 
     @property
     def dim(self) -> int:
-        return 2 * self.max_path_len
+        return (4 if self.nee else 2) * self.max_path_len
 
     @property
     def n_tris(self) -> int:

@@ -31,7 +31,7 @@ struct ChainsH {
 template <class Real>
 void fill_scene(Scene<Real>& sc, const float* verts, uint32_t nv, const uint32_t* idx, uint32_t nt, const uint32_t* tri_mat,
                 const double* mats, uint32_t nm, const float* env, const float* cam, float vfov, uint32_t W, uint32_t H,
-                uint32_t L, int use_bvh) {
+                uint32_t L, int use_bvh, int nee) {
   sc.set_geometry(verts, nv, idx, nt);
   sc.tri_mat.assign(tri_mat, tri_mat + nt);
   sc.mats.resize(nm);
@@ -44,6 +44,8 @@ void fill_scene(Scene<Real>& sc, const float* verts, uint32_t nv, const uint32_t
   for (int c = 0; c < 3; ++c) sc.env[c] = (Real)env[c];
   sc.set_camera(cam, cam + 3, cam + 6, vfov, W, H);
   sc.L = L; sc.use_bvh = use_bvh != 0;
+  sc.nee = nee != 0;
+  sc.build_lights();
 }
 
 template <class Real>
@@ -128,10 +130,10 @@ double orc_min_image(double v, int prec) { return prec == 0 ? (double)min_image<
 
 void* orc_scene_create(int prec, const float* verts, uint32_t nv, const uint32_t* idx, uint32_t nt, const uint32_t* tri_mat,
                        const double* mats, uint32_t nm, const float* env, const float* cam, float vfov, uint32_t W, uint32_t H,
-                       uint32_t L, int use_bvh) {
+                       uint32_t L, int use_bvh, int nee) {
   auto* h = new SceneH();
   h->prec = prec;
-  WITH_SCENE(h, S, fill_scene(S, verts, nv, idx, nt, tri_mat, mats, nm, env, cam, vfov, W, H, L, use_bvh));
+  WITH_SCENE(h, S, fill_scene(S, verts, nv, idx, nt, tri_mat, mats, nm, env, cam, vfov, W, H, L, use_bvh, nee));
   return h;
 }
 void* orc_scene_create_analytic2d(int prec, uint32_t nc, const double* w, const double* mx, const double* my, const double* s, uint32_t W, uint32_t H) {

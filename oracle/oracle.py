@@ -25,7 +25,7 @@ def lib():
         L = _lib
         vp, u32, u64, i32, f64, f32 = C.c_void_p, C.c_uint32, C.c_uint64, C.c_int, C.c_double, C.c_float
         L.orc_scene_create.restype = vp
-        L.orc_scene_create.argtypes = [i32, vp, u32, vp, u32, vp, vp, u32, vp, vp, f32, u32, u32, u32, i32]
+        L.orc_scene_create.argtypes = [i32, vp, u32, vp, u32, vp, vp, u32, vp, vp, f32, u32, u32, u32, i32, i32]
         L.orc_scene_create_analytic2d.restype = vp
         L.orc_scene_create_analytic2d.argtypes = [i32, u32, vp, vp, vp, vp, u32, u32]
         L.orc_scene_destroy.argtypes = [vp]
@@ -125,7 +125,8 @@ class Scene:
             cam = np.concatenate([np.asarray(desc.cam_pos, dtype=np.float32), np.asarray(desc.cam_look, dtype=np.float32),
                                   np.asarray(desc.cam_up, dtype=np.float32)])
             self.h = L.orc_scene_create(prec, _p(v), len(v), _p(i), len(i), _p(tm), _p(m), len(m), _p(env), _p(cam),
-                                        float(desc.vfov_deg), desc.width, desc.height, desc.max_path_len, int(use_bvh))
+                                        float(desc.vfov_deg), desc.width, desc.height, desc.max_path_len, int(use_bvh),
+                                        int(bool(getattr(desc, "nee", False))))
         self.dim = int(L.orc_scene_dim(self.h))
         self.npix = desc.width * desc.height
 

@@ -88,7 +88,9 @@ template <class Real> inline void evaluate(const Scene<Real>& sc, const Real* x,
   else if (d <= 8) evaluate_dual<Real, 8>(sc, x, e, g);
   else if (d <= 16) evaluate_dual<Real, 16>(sc, x, e, g);
   else if (d <= 24) evaluate_dual<Real, 24>(sc, x, e, g);
-  else evaluate_dual<Real, 32>(sc, x, e, g);
+  else if (d <= 32) evaluate_dual<Real, 32>(sc, x, e, g);
+  else if (d <= 48) evaluate_dual<Real, 48>(sc, x, e, g);
+  else evaluate_dual<Real, 64>(sc, x, e, g);
   // Q18: a non-finite contribution or score is a zero-contribution state, counted.
   bool bad = !(std::isfinite(e.f[0]) && std::isfinite(e.f[1]) && std::isfinite(e.f[2]) && std::isfinite(e.p));
   if (want_score) for (uint32_t j = 0; j < d; ++j) bad = bad || !std::isfinite(g[j]);

@@ -53,7 +53,24 @@ template <class Real> struct Scene {
   std::vector<uint32_t> order;  // triangle ids in leaf order
   bool use_bvh = true;
 
-  uint32_t dim() const { return analytic ? 2u : 2u * L; }
+  // next-event estimation (Q21): the emitter triangles in index order with their areas and running sums
+  bool nee = false;
+  std::vector<uint32_t> light_tri;
+  std::vector<Real> light_area, light_cdf;  // light_cdf[j] = area_0 + ... + area_j, summed in this order
+  Real light_total = 0;
+
+  void build_lights() {
+    light_tri.clear(); light_area.clear(); light_cdf.clear(); light_total = 0;
+    for (uint32_t t = 0; t < ntris(); ++t) {
+      if (mats[tri_mat[t]].kind != MAT_EMITTER) continue;
+      const V c = cross(e1[t], e2[t]);
+      const Real a = Real(0.5) * std::sqrt(dot(c, c));
+      light_total = light_total + a;
+      light_tri.push_back(t); light_area.push_back(a); light_cdf.push_back(light_total);
+    }
+  }
+
+  uint32_t dim() const { return analytic ? 2u : (nee ? 4u : 2u) * L; }
   uint32_t ntris() const { return (uint32_t)v0.size(); }
 
   // Moeller-Trumbore, no culling, t_min = 0 exclusive (Q8).  Updates `best`
