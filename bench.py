@@ -29,10 +29,12 @@ def stream_bytes_per_mutation(d, grad):
     return (4 if grad else 2) * 4 * d + 42
 
 
-def make_desc(name):
+def make_desc(name, nee=False):
     from dr_inputs import scenes as S
-    return {"machines": S.machines, "cornell": S.cornell, "caustic": S.caustic, "furnace": S.furnace,
-            "mini_machines": S.mini_machines}[name]()
+    d = {"machines": S.machines, "cornell": S.cornell, "caustic": S.caustic, "furnace": S.furnace,
+         "mini_machines": S.mini_machines}[name]()
+    d.nee = bool(nee)          # next-event estimation + MIS (Q21): four PSS coordinates per vertex
+    return d
 
 
 def peaks():
@@ -107,7 +109,7 @@ def run_reference(args):
     if rank != 0:
         return
     from oracle import oracle as O
-    desc = make_desc(args.scene)
+    desc = make_desc(args.scene, args.nee)
     n = 8192
     sc = O.Scene(desc, O.F32)
     ch = O.Chains(sc, args.method, n, seed=4)
@@ -124,7 +126,8 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"configs[3] {desc.name} {desc.width}x{desc.height}, {desc.n_tris} triangles, L={desc.max_path_len}",
-                   "method": args.method, "chains_per_step": n},
+                   "method": args.method, "chains_per_step": n,
+                   "path_construction": "direction sampling + next-event estimation with MIS (Q21)" if args.nee else "direction sampling only (Q5)"},
         "mrays_per_s": (ch.stats()["rays"] - r0) / dt / 1e6,
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -140,6 +143,7 @@ def main():
     ap.add_argument("--method", default="diffusion_restore")
     ap.add_argument("--scene", default="machines")
     ap.add_argument("--chains", type=int, default=0, help="chains per GPU (default: one per pixel)")
+    ap.add_argument("--nee", action="store_true", help="path construction with next-event estimation + MIS (second reading, DESIGN.md Q21)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
     args = ap.parse_args()
@@ -161,7 +165,7 @@ def main():
     import paper_2605_08916_b200 as dr
     from paper_2605_08916_b200 import sharding
 
-    desc = make_desc(args.scene)
+    desc = make_desc(args.scene, args.nee)
     scene = dr.Scene(desc)
     n_local = args.chains or desc.width * desc.height            # weak scaling: every GPU runs one chain per pixel
     offset = sharding.shard_offset(n_local, rank)
@@ -316,6 +320,7 @@ def main():
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"configs[3] {desc.name} {desc.width}x{desc.height}, {desc.n_tris} triangles, L={desc.max_path_len} (d={desc.dim})",
                    "method": args.method, "chains_per_gpu": n_local, "iterations_per_frame": 1,
+                   "path_construction": "direction sampling + next-event estimation with MIS (Q21)" if args.nee else "direction sampling only (Q5)",
                    "l2": "chain state (%.0f MB) larger than L2; no flush" % (chains.state.numel() / 1e6),
                    "seed": 4, "stddev": float(chains.cfg.stddev), "c_tilde": float(chains.cfg.c_tilde), "dt": float(chains.cfg.dt),
                    "m": float(chains.cfg.m)},

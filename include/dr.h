@@ -73,6 +73,8 @@ typedef struct {
   float vfov_deg;                   /* pinhole camera, vertical field of view */
   uint32_t width, height;           /* image W x H; pixel map DESIGN.md Q4 */
   uint32_t max_path_len;            /* L segments, PSS dimension d = 2L (Q5); 1 <= L <= 16 */
+  uint32_t nee;                     /* 0 / 1: next-event estimation + MIS (Q21): emitters sampled by area
+                                       at every Lambert / GGX vertex, balance heuristic; four coordinates per vertex, d = 4L */
 } dr_scene_desc;
 
 /* 2-D analytic target (d = 2): mixture of wrapped Gaussians, f = (p,p,p), closed-form score.

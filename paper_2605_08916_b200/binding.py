@@ -40,7 +40,7 @@ class dr_scene_desc(C.Structure):
                 ("host_tri_material", C.c_void_p), ("host_materials", C.POINTER(dr_material)), ("nm", C.c_uint32),
                 ("env_radiance", C.c_float * 3), ("cam_pos", C.c_float * 3), ("cam_look", C.c_float * 3),
                 ("cam_up", C.c_float * 3), ("vfov_deg", C.c_float), ("width", C.c_uint32), ("height", C.c_uint32),
-                ("max_path_len", C.c_uint32)]
+                ("max_path_len", C.c_uint32), ("nee", C.c_uint32)]
 
 
 class dr_analytic2d_desc(C.Structure):
@@ -168,8 +168,9 @@ class Scene:
             d.cam_look[:] = [float(c) for c in desc.cam_look]
             d.cam_up[:] = [float(c) for c in desc.cam_up]
             d.vfov_deg, d.width, d.height, d.max_path_len = float(desc.vfov_deg), desc.width, desc.height, desc.max_path_len
+            d.nee = int(bool(getattr(desc, "nee", False)))
             _check(lib.dr_scene_create(C.byref(d), C.byref(h)))
-            self.dim = 2 * desc.max_path_len
+            self.dim = desc.dim
         self.h = h
         self.width, self.height = desc.width, desc.height
         self.npix = desc.width * desc.height

@@ -9,6 +9,7 @@
 #include "../../include/dr.h"
 #include "dr_kernels.cuh"
 #include "dr_wave.cuh"
+#include "dr_grad.cuh"
 
 using namespace dr;
 
@@ -51,6 +52,7 @@ struct dr_scene {
   void* d_nodes = nullptr;
   void* d_tris = nullptr;
   void* d_mats = nullptr;
+  void* d_lights = nullptr;
   dr_scene_info info{};
   int n_sm = 1;            // persistent k_trace grid: one block per SM
   size_t trace_smem = 0;   // staged top-level nodes + per-thread traversal stacks
@@ -90,7 +92,7 @@ struct Layout {
   size_t total;
 };
 
-Layout make_layout(uint32_t N, uint32_t planes, uint32_t Lseg, bool grad) {
+Layout make_layout(uint32_t N, uint32_t planes, uint32_t Lseg, bool grad, bool nee) {
   Layout L{};
   size_t o = 0;
   auto take = [&](size_t bytes) { const size_t at = o; o = align256(o + bytes); return at; };
@@ -116,7 +118,7 @@ Layout make_layout(uint32_t N, uint32_t planes, uint32_t Lseg, bool grad) {
   L.ctr = take(sizeof(Counters));
   L.q = take(6 * sizeof(float4) * (size_t)N);           // qa | qb, or the 64-byte ray records of k_wave
   L.hits = take(sizeof(uint2) * (size_t)N);
-  L.ring = take(sizeof(uint2) * (size_t)N * Lseg);      // one entry per ray of an evaluation, never reused (dr_wave.cuh)
+  L.ring = take(sizeof(uint2) * (size_t)N * (nee ? 2 * Lseg - 1 : Lseg));   // one entry per ray of an evaluation, never reused (dr_wave.cuh)
   L.rec = take(grad ? sizeof(float4) * (size_t)N * Lseg : 0);
   L.pinfo = take(grad ? 4 * (size_t)N : 0);
   L.gradlist = take(grad ? 4 * (size_t)N : 0);
@@ -181,7 +183,8 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
     CUDA_TRY(cudaGetLastError());
     return DR_OK;
   }
-  const bool wave = !stats && sc->wave_ok && (form == 2 || (form == 0 && n < kWaveMaxStates));
+  if (dev.nee && (!sc->wave_ok || form == 1)) return fail(DR_ERR_UNSUPPORTED, "next-event estimation runs in k_wave only (no per-segment loop)");
+  const bool wave = dev.nee || (!stats && sc->wave_ok && (form == 2 || (form == 0 && n < kWaveMaxStates)));
   CUDA_TRY(cudaMemsetAsync(ws.ctl, 0, 4 * kCtlWords, s));
   {
     ProfScope ps(prof, DR_PROF_RAYGEN, s);
@@ -193,8 +196,12 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
 #endif
   if (wave) {
     ProfScope ps(prof, DR_PROF_TRACE, s);
-    if (grad) k_wave<true><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
-    else k_wave<false><<<sc->n_sm, kTraceBlock, sc->trace_smem + kWaveExtraSmem, s>>>(dev, ws, io, n);
+    const size_t sm = sc->trace_smem + kWaveExtraSmem;
+    if (stats) {   // the counting pass of a scene with next-event estimation (others count in k_trace<true>)
+      if (grad) k_wave<true, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+      else k_wave<false, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+    } else if (grad) k_wave<true, false><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+    else k_wave<false, false><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
   } else
   for (uint32_t k = 1; k <= dev.L; ++k) {
     const float4* q = (k & 1u) ? ws.qa : ws.qb;
@@ -209,7 +216,11 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
       else k_shade<false><<<g, kShadeBlock, 0, s>>>(dev, ws, io, k);
     }
   }
-  if (grad) { ProfScope ps(prof, DR_PROF_GRAD, s); k_grad<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io); }
+  if (grad) {
+    ProfScope ps(prof, DR_PROF_GRAD, s);
+    if (dev.nee) k_grad_nee<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io);
+    else k_grad<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io);
+  }
   CUDA_TRY(cudaGetLastError());
 #if DR_CHECKS
   if (wave) {   // checked build: every queue entry that was reserved was consumed, every path finished, no check fired
@@ -228,7 +239,7 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
 // tags start at 1, so queue entries of earlier evaluations never look published.
 EvalWs next_ws(dr_chains* c, cudaStream_t s) {
   if (++c->eval_tag == 0) {   // 2^32 evaluations later: clear the queue once and start over
-    cudaMemsetAsync(c->ws.ring, 0, sizeof(uint2) * (size_t)c->ws.cap * c->scene->dev.L, s);
+    cudaMemsetAsync(c->ws.ring, 0, sizeof(uint2) * wave_ring_entries(c->scene->dev, c->ws.cap), s);
     c->eval_tag = 1;
   }
   EvalWs ws = c->ws;
@@ -281,7 +292,7 @@ struct HookEval {
     const size_t N = n, L = sc->dev.L;
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o = align256(o + bytes); return at; };
-    const size_t q = take(96 * N), hits = take(8 * N), ring = take(8 * N * L), rec = take(grad ? 16 * N * L : 0),
+    const size_t q = take(96 * N), hits = take(8 * N), ring = take(8 * wave_ring_entries(sc->dev, N)), rec = take(grad ? 16 * N * L : 0),
                  pinfo = take(grad ? 4 * N : 0), gl = take(grad ? 4 * N : 0), ctl = take(4 * kCtlWords);
     cudaError_t e = ws_mem.alloc(o);
     if (e == cudaSuccess) e = xpl.alloc(16 * N * sc->dev.planes);
@@ -292,7 +303,7 @@ struct HookEval {
     ws.qa = (float4*)(b + q); ws.qb = ws.qa + 3 * N; ws.hits = (uint2*)(b + hits); ws.ring = (uint2*)(b + ring); ws.rec = (float4*)(b + rec);
     ws.pinfo = (uint32_t*)(b + pinfo); ws.gradlist = (uint32_t*)(b + gl); ws.ctl = (uint32_t*)(b + ctl); ws.cap = n;
     ws.tag = 1;
-    return cudaMemsetAsync(ws.ring, 0, 8 * N * L, stream);   // fresh memory: no entry carries tag 1
+    return cudaMemsetAsync(ws.ring, 0, 8 * wave_ring_entries(sc->dev, N), stream);   // fresh memory: no entry carries tag 1
   }
 };
 
@@ -367,8 +378,10 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   s->wave_ok = DR_SMEM_NODES == 0 && s->trace_smem + kWaveExtraSmem <= kMaxDynSmem;
   e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e != cudaSuccess) {
     dr_scene_destroy(s);
     return fail(DR_ERR_CUDA, std::string("k_trace shared memory: ") + cudaGetErrorString(e));
@@ -389,7 +402,42 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   for (int c = 0; c < 3; ++c) { dev.cam_w[c] = w[c]; dev.cam_r[c] = r[c]; dev.cam_v[c] = v[c]; }
   dev.tan_half = std::tan(d->vfov_deg * (float)(3.14159265358979323846 / 360.0));
   dev.tan_half_aspect = dev.tan_half * ((float)d->width / (float)d->height);
-  dev.W = d->width; dev.H = d->height; dev.L = d->max_path_len; dev.d = 2 * d->max_path_len; dev.planes = (dev.d + 3) / 4;
+  dev.nee = d->nee ? 1u : 0u;
+  dev.W = d->width; dev.H = d->height; dev.L = d->max_path_len; dev.d = (dev.nee ? 4 : 2) * d->max_path_len; dev.planes = (dev.d + 3) / 4;
+  // emitter list for next-event estimation (dr_nee.cuh Light; Q21): triangle-index order, areas and running sums in fp32
+  {
+    std::vector<float> lights;
+    float total = 0.f;
+    for (uint32_t t = 0; t < d->nt; ++t) {
+      const dr_material& m = d->host_materials[d->host_tri_material[t]];
+      if (m.kind != DR_MAT_EMITTER) continue;
+      const float* a = &d->host_vertices[3 * d->host_indices[3 * t]];
+      const float* b = &d->host_vertices[3 * d->host_indices[3 * t + 1]];
+      const float* c = &d->host_vertices[3 * d->host_indices[3 * t + 2]];
+      float e1[3], e2[3], cr[3];
+      for (int x = 0; x < 3; ++x) { e1[x] = b[x] - a[x]; e2[x] = c[x] - a[x]; }
+      cross(e1, e2, cr);
+      const float area = 0.5f * std::sqrt(cr[0] * cr[0] + cr[1] * cr[1] + cr[2] * cr[2]);
+      const float before = total;
+      total = total + area;
+      normalize(cr);
+      uint32_t idbits = t;
+      float idf;
+      std::memcpy(&idf, &idbits, 4);
+      const float rec[20] = {a[0], a[1], a[2], total, e1[0], e1[1], e1[2], area, e2[0], e2[1], e2[2], idf,
+                             cr[0], cr[1], cr[2], before, m.emission[0], m.emission[1], m.emission[2], 0.f};
+      lights.insert(lights.end(), rec, rec + 20);
+    }
+    dev.n_lights = (uint32_t)(lights.size() / 20);
+    dev.light_total = total;
+    dev.lights = nullptr;
+    if (dev.n_lights) {
+      cudaError_t le = cudaMalloc(&s->d_lights, lights.size() * sizeof(float));
+      if (le == cudaSuccess) le = cudaMemcpy(s->d_lights, lights.data(), lights.size() * sizeof(float), cudaMemcpyHostToDevice);
+      if (le != cudaSuccess) { dr_scene_destroy(s); return fail(DR_ERR_CUDA, std::string("emitter list: ") + cudaGetErrorString(le)); }
+      dev.lights = (const float4*)s->d_lights;
+    }
+  }
   dev.eps_ray = 1e-5f * bvh.diag;  // Q8
   dev.analytic = 0; dev.n_mix = 0;
   s->info.n_tris = d->nt; s->info.n_nodes = dev.n_nodes; s->info.depth = bvh.depth; s->info.smem_nodes = dev.smem_nodes;
@@ -414,7 +462,7 @@ dr_status dr_scene_create_analytic2d(const dr_analytic2d_desc* d, dr_scene** out
   }
   dev.analytic = 1; dev.n_mix = (int)d->n_components;
   dev.W = d->width; dev.H = d->height; dev.L = 1; dev.d = 2; dev.planes = 1;
-  dev.smem_nodes = 0; dev.n_nodes = 0;
+  dev.smem_nodes = 0; dev.n_nodes = 0; dev.nee = 0; dev.n_lights = 0; dev.lights = nullptr; dev.light_total = 0.f;
   s->info = dr_scene_info{};
   *out = s;
   return DR_OK;
@@ -422,7 +470,7 @@ dr_status dr_scene_create_analytic2d(const dr_analytic2d_desc* d, dr_scene** out
 
 dr_status dr_scene_destroy(dr_scene* s) {
   if (!s) return DR_OK;
-  cudaFree(s->d_nodes); cudaFree(s->d_tris); cudaFree(s->d_mats);
+  cudaFree(s->d_nodes); cudaFree(s->d_tris); cudaFree(s->d_mats); cudaFree(s->d_lights);
   delete s;
   return DR_OK;
 }
@@ -436,7 +484,7 @@ dr_status dr_scene_get_info(const dr_scene* s, dr_scene_info* o) {
 size_t dr_chains_state_bytes(const dr_scene* s, const dr_config* c) {
   if (!s || check_config(c) != DR_OK) return 0;
   const bool grad = c->method == DR_MALA || c->method == DR_MALA_RESTORE || c->method == DR_DIFFUSION_RESTORE;
-  return make_layout(c->n_chains, s->dev.planes, s->dev.L, grad).total;
+  return make_layout(c->n_chains, s->dev.planes, s->dev.L, grad, s->dev.nee != 0).total;
 }
 
 dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_state, size_t bytes, float* dev_accum, dr_chains** out) {
@@ -446,7 +494,7 @@ dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_stat
   if (cs != DR_OK) return cs;
   if (((uintptr_t)dev_state & 255u) || ((uintptr_t)dev_accum & 15u)) return fail(DR_ERR_INVALID_ARG, "dev_state must be 256-byte and dev_accum 16-byte aligned");
   const bool grad = c->method == DR_MALA || c->method == DR_MALA_RESTORE || c->method == DR_DIFFUSION_RESTORE;
-  const Layout L = make_layout(c->n_chains, s->dev.planes, s->dev.L, grad);
+  const Layout L = make_layout(c->n_chains, s->dev.planes, s->dev.L, grad, s->dev.nee != 0);
   if (bytes < L.total) return fail(DR_ERR_INVALID_ARG, "state buffer smaller than dr_chains_state_bytes");
   dr_chains* h = new dr_chains();
   h->scene = s; h->cfg = *c;

@@ -11,6 +11,7 @@
 // kernel ran with 4.5 of 32 lanes active).
 #pragma once
 #include "dr_path.cuh"
+#include "dr_nee.cuh"
 #include "dr_traverse.cuh"
 
 namespace dr {
@@ -61,7 +62,7 @@ struct EvalWs {
   float4* qa;          // 3 * cap; qb = qa + 3 * cap (one allocation of 6 * cap float4: k_wave uses the first 4 * cap as records)
   float4* qb;          // 3 * cap
   uint2* hits;         // cap: (bits(t), triangle in leaf order or kMiss)   (loop form)
-  uint2* ring;         // L * cap ray entries, written once per evaluation, never reused                 (k_wave)
+  uint2* ring;         // wave_ring_entries() ray entries, written once per evaluation, never reused      (k_wave)
   float4* rec;         // L * cap (score only): incoming direction and triangle of vertex k of state s at [k * cap + s]
   uint32_t* pinfo;     // cap (score only): refract mask | rays << 16 of the finished path
   uint32_t* gradlist;  // cap (score only)
@@ -90,6 +91,16 @@ __device__ __forceinline__ float2 x_pair(const EvalIO& io, uint32_t s, uint32_t 
   const float4 q = io.x[(size_t)(k >> 1) * io.stride + s];
   return (k & 1u) ? make_float2(q.z, q.w) : make_float2(q.x, q.y);
 }
+// the coordinates of vertex k: (u1, u2, v1, v2) = plane k with next-event estimation, else (u1, u2, 0, 0)
+__device__ __forceinline__ float4 x_vertex(const DevScene& sc, const EvalIO& io, uint32_t s, uint32_t k) {
+  if (sc.nee) return io.x[(size_t)k * io.stride + s];
+  const float2 u = x_pair(io, s, k);
+  return make_float4(u.x, u.y, 0.f, 0.f);
+}
+__device__ __forceinline__ void g_vertex(const DevScene& sc, const EvalIO& io, uint32_t s, uint32_t k, float4 g) {
+  if (sc.nee) io.g[(size_t)k * io.stride + s] = g;
+  else reinterpret_cast<float2*>(&io.g[(size_t)(k >> 1) * io.stride + s])[k & 1u] = make_float2(g.x, g.y);
+}
 __device__ __forceinline__ void g_pair(const EvalIO& io, uint32_t s, uint32_t k, float a, float b) {
   reinterpret_cast<float2*>(&io.g[(size_t)(k >> 1) * io.stride + s])[k & 1u] = make_float2(a, b);
 }
@@ -97,6 +108,10 @@ __device__ __forceinline__ void g_pair(const EvalIO& io, uint32_t s, uint32_t k,
 // ---- a3: camera rays -------------------------------------------------------------------------------------------
 // WAVE: the ray goes into the state's record and ring entry t (dr_wave.cuh); otherwise into slot t of queue qa.
 constexpr int kCtlWaveReserve = 48, kCtlWaveHead = 50, kCtlWaveDone = 51;   // control words of k_wave
+constexpr uint32_t kRecWords = 6;    // float4 per state record of k_wave: ray (o | state, d | signature, T | masks),
+                                     // (pending emitter connection | density of the ray's direction), shadow ray (o | emitter id, d | lobe)
+// queue entries an evaluation can need: a path makes at most L rays, and with next-event estimation one shadow ray per vertex
+__host__ __device__ inline size_t wave_ring_entries(const DevScene& sc, size_t cap) { return (sc.nee ? 2u * sc.L - 1u : sc.L) * cap; }
 template <bool WAVE>
 __global__ void __launch_bounds__(kShadeBlock) k_raygen(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
   const uint32_t t = blockIdx.x * kShadeBlock + threadIdx.x;
@@ -110,8 +125,13 @@ __global__ void __launch_bounds__(kShadeBlock) k_raygen(DevScene sc, EvalWs ws, 
   const float4 q1 = make_float4(d.x, d.y, d.z, __uint_as_float(kSigInit));
   const float4 q2 = make_float4(1.f, 1.f, 1.f, __uint_as_float(0u));
   if (WAVE) {
-    float4* r = ws.qa + 4 * (size_t)s;
+    float4* r = ws.qa + kRecWords * (size_t)s;
     r[0] = q0; r[1] = q1; r[2] = q2;
+    if (sc.nee) {
+      r[3] = make_float4(0.f, 0.f, 0.f, -1.f);          // the camera ray has no direction density
+      io.f[s] = make_float4(0.f, 0.f, 0.f, 0.f);        // emitter connections accumulate here
+      if (io.nrays) io.nrays[s] = 0u;
+    }
     ws.ring[t] = make_uint2(s, ws.tag);   // segment 1
   } else {
     ws.qa[t] = q0; ws.qa[(size_t)ws.cap + t] = q1; ws.qa[2 * (size_t)ws.cap + t] = q2;
@@ -327,19 +347,59 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   }
 }
 
-// Vertex k of one ray: emission / termination, direction sampling, throughput (rows a3 / a5).  Q0..Q2 = the ray's queue
-// entry, h = (bits(t), triangle in leaf order or kMiss).  A finished path writes f, p, signature of state s; a
-// continuing one returns the next ray in n0..n2 (n0.w = Q0.w).  Shared by k_shade and k_wave.
+// Vertex k of one ray: emission / termination, emitter connection, direction sampling, throughput (rows a3 / a5).
+// Q0..Q2 = the ray's words (dr_eval.cuh EvalWs), pb_prev = density of its direction (< 0: none, e.g. the camera ray or a
+// Dirac lobe), h = (bits(t), triangle in leaf order or kMiss).  Three outcomes:
+//   * the path ends here: f (added to what the emitter connections of earlier vertices left in io.f), p, signature are written;
+//   * it continues (cont): the next ray is in n0..n2, the density of its direction in pb_next;
+//   * with next-event estimation it may first need a shadow ray (shadow): sh_o / sh_d, the connection's contribution if it
+//     is visible in cpend, the emitter triangle's id in light_id, and the lobe code still to be hashed into the signature
+//     (n1.w then holds the signature BEFORE the visibility and the lobe); nee_finish() completes the vertex.
+// Shared by k_shade (no next-event estimation) and k_wave.
+struct ShadeOut {
+  float4 n0, n1, n2;
+  float pb_next;
+  float3 sh_o, sh_d, cpend;
+  uint32_t light_id, lobe;
+  bool cont, shadow, want_grad;
+};
+
+constexpr uint32_t kTermNone = 0xFFFFFFFEu;   // the path ended without a terminal contribution (length cap, zero-weight direction)
+// nv: vertices that sampled (1 .. nv), term: the triangle the last ray hit (leaf order), kMiss (environment) or kTermNone
+__device__ __forceinline__ void finish_path(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t k, uint32_t s, float f0, float f1,
+                                            float f2, uint32_t sig, uint32_t info, uint32_t nv, uint32_t term, bool grad, bool& want_grad,
+                                            uint32_t& bad) {
+  if (sc.nee) { const float4 acc = __ldcg(&io.f[s]); f0 = acc.x + f0; f1 = acc.y + f1; f2 = acc.z + f2; }   // emitter connections so far
+  float p = f0 * 0.2126f + f1 * 0.7152f + f2 * 0.0722f;
+  if (!(isfinite(f0) && isfinite(f1) && isfinite(f2) && isfinite(p))) { f0 = f1 = f2 = p = 0.f; bad = 1; }
+  __stcg(&io.f[s], make_float4(f0, f1, f2, p));
+  io.sig[s] = sig;
+  if (io.nrays && !sc.nee) io.nrays[s] = k;
+  if (grad) {
+    if (sc.nee) {
+      ws.rec[s] = make_float4(__uint_as_float(info), __uint_as_float(k), __uint_as_float(term), __uint_as_float(nv));   // plane 0 of the vertex record
+      want_grad = p > 0.f;                                                          // geometry and MIS terms depend on x
+    } else {
+      ws.pinfo[s] = (info & 0xFFFFu) | (k << 16);
+      // only GGX weights depend on x (DESIGN.md section 2): no GGX vertex or p == 0  =>  score == 0 exactly
+      want_grad = (info >> 16) && p > 0.f;
+    }
+  }
+}
+
 template <bool GRAD>
 __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t k, const float4& Q0,
-                                             const float4& Q1, const float4& Q2, const uint2& h, uint32_t s, bool& cont,
-                                             bool& want_grad, uint32_t& bad, float4& n0, float4& n1, float4& n2) {
+                                             const float4& Q1, const float4& Q2, float pb_prev, const uint2& h, uint32_t s, ShadeOut& out,
+                                             uint32_t& bad) {
   const size_t cap = ws.cap;
   uint32_t sig = __float_as_uint(Q1.w), info = __float_as_uint(Q2.w);
   const float3 o = xyz(Q0), d = xyz(Q1);
   float T0 = Q2.x, T1 = Q2.y, T2 = Q2.z;
   float f0 = 0.f, f1 = 0.f, f2 = 0.f;
   bool done = true;
+  uint32_t term = h.y;          // what the path's last ray hit, if it ends here with a contribution
+  out.cont = false; out.shadow = false; out.want_grad = false;
+  if (sc.nee && io.nrays) __stcg(&io.nrays[s], __ldcg(&io.nrays[s]) + 1u);   // L2: successive events of a path run on different SMs
   if (h.y == kMiss) {
     sig = fnv(sig, 0u);
     f0 = T0 * sc.env[0]; f1 = T1 * sc.env[1]; f2 = T2 * sc.env[2];
@@ -358,69 +418,59 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
       if (dn < 0.f) {
         sig = fnv(sig, 4u);
         const float4 m2 = __ldg(&sc.mats[3 * mi + 2]);
-        f0 = T0 * m1.z; f1 = T1 * m1.w; f2 = T2 * m2.x;
+        const V3<float> ov{o.x, o.y, o.z}, dv{d.x, d.y, d.z};
+        const float w_b = emitter_weight<float>(sc, xyz(t0), fr.nf, ov, dv, pb_prev, pb_prev >= 0.f);   // dn < 0: nf = n
+        f0 = T0 * m1.z * w_b; f1 = T1 * m1.w * w_b; f2 = T2 * m2.x * w_b;
       } else {
         sig = fnv(sig, 5u);
+        term = kTermNone;
       }
     } else if (k < sc.L) {
-      // hit point on the triangle's plane, t = ((v0 - o).n) / (d.n): the traversal's t decided WHICH triangle
-      const float3 nn = fr.nf * (dn < 0.f ? 1.f : -1.f);   // the geometric normal n again (exact: * +-1)
-      const float tp = dot3(xyz(t0) - o, nn) / dot3(d, nn);
-      const float3 hit = o + d * tp;
-      const float2 u = x_pair(io, s, k);
+      term = kTermNone;
+      const float4 u = x_vertex(sc, io, s, k);
       if (GRAD) ws.rec[(size_t)k * cap + s] = make_float4(d.x, d.y, d.z, __uint_as_float(li));
-      V3<float> din{d.x, d.y, d.z}, dnew;
-      float off = 1.f;
-      if (kind == 0u) {
-        sig = fnv(sig, 0u);
-        dnew = lambert_dir<float>(fr, u.x, u.y);
-        T0 *= m0.y; T1 *= m0.z; T2 *= m0.w;
-      } else if (kind == 1u) {
-        const float eta = dn < 0.f ? m1.x : 1.0f / m1.x;
-        const float F = fresnel_dielectric(-dot3(d, fr.nf), eta);
-        const bool reflect = u.x < F;
-        sig = fnv(sig, reflect ? 1u : 2u);
-        if (!reflect) { off = -1.f; info |= 1u << k; }
-        dnew = dielectric_dir<float>(fr, eta, reflect, din);
-      } else {
-        sig = fnv(sig, 3u);
-        info |= 1u << 16;
-        float c5, G1;
-        if (!ggx_dir<float>(fr, m1.y, din, u.x, u.y, dnew, c5, G1)) {
-          T0 = T1 = T2 = 0.f;
-        } else {
-          T0 *= (m0.y + (1.0f - m0.y) * c5) * G1;
-          T1 *= (m0.z + (1.0f - m0.z) * c5) * G1;
-          T2 *= (m0.w + (1.0f - m0.w) * c5) * G1;
-        }
-      }
-      if (!(T0 == 0.f && T1 == 0.f && T2 == 0.f)) {
+      const V3<float> ov{o.x, o.y, o.z}, dv{d.x, d.y, d.z};
+      VertexOut<float> vo;
+      V3<float> hit;
+      bool reflect = false;
+      uint32_t lj = 0;
+      vertex_fn<float>(sc, xyz(t0), fr, dn, m0, m1, kind, ov, dv, u.x, u.y, u.z, u.w, true, reflect, vo, hit, lj);
+      uint32_t lobe = kind == 0u ? 0u : (kind == 1u ? (reflect ? 1u : 2u) : 3u);
+      if (kind == 1u && !reflect) info |= 1u << k;
+      if (kind == 2u) info |= 1u << 16;
+      T0 *= vo.W[0]; T1 *= vo.W[1]; T2 *= vo.W[2];
+      const bool alive = !(T0 == 0.f && T1 == 0.f && T2 == 0.f);
+      if (vo.nee_valid) {   // the vertex is completed by nee_finish() once the shadow ray is back
+        const Light Lt = load_light(sc, lj);
+        out.shadow = true;
+        out.light_id = Lt.id;
+        out.lobe = lobe;
+        // (T fcos) (Le w_l / p_l): T here is the throughput BEFORE this vertex' direction sample
+        out.cpend = make_float3((Q2.x * vo.fcos[0]) * vo.lw[0], (Q2.y * vo.fcos[1]) * vo.lw[1], (Q2.z * vo.fcos[2]) * vo.lw[2]);
+        out.sh_o = make_float3(hit.x + fr.nf.x * sc.eps_ray, hit.y + fr.nf.y * sc.eps_ray, hit.z + fr.nf.z * sc.eps_ray);
+        out.sh_d = normalize3(make_float3(vo.y.x, vo.y.y, vo.y.z) - out.sh_o);   // towards the sampled point, from the offset origin
         done = false;
-        const float3 on = hit + fr.nf * (sc.eps_ray * off);
-        n0 = make_float4(on.x, on.y, on.z, Q0.w);
-        n1 = make_float4(dnew.x, dnew.y, dnew.z, __uint_as_float(sig));
-        n2 = make_float4(T0, T1, T2, __uint_as_float(info));
+      } else {
+        sig = fnv(sig, lobe);
       }
+      if (alive || vo.nee_valid) {
+        done = false;
+        out.cont = alive && !vo.nee_valid;
+        out.n0 = make_float4(vo.o2.x, vo.o2.y, vo.o2.z, Q0.w);
+        out.n1 = make_float4(vo.d2.x, vo.d2.y, vo.d2.z, __uint_as_float(sig));
+        out.n2 = make_float4(T0, T1, T2, __uint_as_float(info));
+        out.pb_next = vo.pb_valid ? vo.pb : -1.f;
+      }
+    } else {
+      term = kTermNone;   // length cap on a surface: nothing is added
     }
   }
-  cont = !done;
-  if (done) {
-    float p = f0 * 0.2126f + f1 * 0.7152f + f2 * 0.0722f;
-    if (!(isfinite(f0) && isfinite(f1) && isfinite(f2) && isfinite(p))) { f0 = f1 = f2 = p = 0.f; bad = 1; }
-    io.f[s] = make_float4(f0, f1, f2, p);
-    io.sig[s] = sig;
-    if (io.nrays) io.nrays[s] = k;
-    if (GRAD) {
-      ws.pinfo[s] = (info & 0xFFFFu) | (k << 16);
-      // only GGX weights depend on x (DESIGN.md section 2): no GGX vertex or p == 0  =>  score == 0 exactly
-      want_grad = (info >> 16) && p > 0.f;
-    }
-  }
+  if (done) finish_path(sc, ws, io, k, s, f0, f1, f2, sig, info, k - 1u, term, GRAD, out.want_grad, bad);
 }
 
 // ---- a3 / a5: shade vertex k of every ray of segment k -------------------------------------------------------------
 template <bool GRAD>
-__global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, EvalIO io, uint32_t k) {
+__global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, EvalIO io, uint32_t k) {   // scenes without next-event estimation
   __shared__ uint32_t s_warp[kShadeBlock / 32];
   __shared__ uint32_t s_base;
   const uint32_t n = ws.ctl[kCtlCnt + k];
@@ -429,14 +479,15 @@ __global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, E
   const float4* qin = (k & 1u) ? ws.qa : ws.qb;
   float4* qout = (k & 1u) ? ws.qb : ws.qa;
   const size_t cap = ws.cap;
-  bool cont = false, want_grad = false;
-  float4 n0, n1, n2;
+  ShadeOut so;
+  so.cont = false; so.want_grad = false;
   uint32_t bad = 0, s = 0;
   if (j < n) {
     const float4 Q0 = qin[j], Q1 = qin[cap + j], Q2 = qin[2 * cap + j];
     s = __float_as_uint(Q0.w);
-    shade_vertex<GRAD>(sc, ws, io, k, Q0, Q1, Q2, ws.hits[j], s, cont, want_grad, bad, n0, n1, n2);
+    shade_vertex<GRAD>(sc, ws, io, k, Q0, Q1, Q2, -1.f, ws.hits[j], s, so, bad);
   }
+  const bool cont = so.cont, want_grad = so.want_grad;
   const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
   if (GRAD) {  // reverse-pass list: one atomic per warp
     const unsigned gm = __ballot_sync(0xFFFFFFFFu, want_grad);
@@ -460,7 +511,7 @@ __global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, E
   __syncthreads();
   if (cont) {
     const size_t at = s_base + s_warp[wid] + __popc(b & ((1u << lane) - 1u));
-    qout[at] = n0; qout[cap + at] = n1; qout[2 * cap + at] = n2;
+    qout[at] = so.n0; qout[cap + at] = so.n1; qout[2 * cap + at] = so.n2;
   }
   if (io.nonfinite_ctr) {
     bad = __reduce_add_sync(0xFFFFFFFFu, bad);

@@ -24,6 +24,9 @@ struct DevScene {
   const float4* tris;   // TriPacked as 3 float4
   const float4* mats;   // MatPacked as 3 float4
   uint32_t n_nodes, smem_nodes, stack_cap, n_tris, n_mats;
+  const float4* lights; // next-event estimation (dr_nee.cuh Light): 5 float4 per emitter triangle
+  uint32_t n_lights, nee;
+  float light_total;
   float env[3];
   float cam_pos[3], cam_w[3], cam_r[3], cam_v[3];
   float tan_half, tan_half_aspect;
@@ -160,7 +163,8 @@ template <class T> __device__ __forceinline__ V3<T> dielectric_dir(const Frame& 
 
 // GGX conductor: visible-normal sampling (spherical-cap form).  Returns false if w_i is below the horizon.
 // c5 = (1 - w_o.h)^5 (Schlick), G1 = Smith masking of w_i; weight_c = (F0_c + (1 - F0_c) c5) G1.
-template <class T> __device__ __forceinline__ bool ggx_dir(const Frame& fr, float al, V3<T> d, T u1, T u2, V3<T>& out, T& c5, T& G1) {
+template <class T> __device__ __forceinline__ bool ggx_dir(const Frame& fr, float al, V3<T> d, T u1, T u2, V3<T>& out, T& c5, T& G1,
+                                                           V3<T>* hm_out = nullptr) {
   V3<T> wo;
   wo.x = -dotf(d, fr.t); wo.y = -dotf(d, fr.bf); wo.z = -dotf(d, fr.nf);
   V3<T> ws;
@@ -175,6 +179,7 @@ template <class T> __device__ __forceinline__ bool ggx_dir(const Frame& fr, floa
   hm.x = (st * c + ws.x) * al; hm.y = (st * s + ws.y) * al; hm.z = z + ws.z;
   const T hn = 1.0f / sqrt_t(dott(hm, hm));
   hm.x = hm.x * hn; hm.y = hm.y * hn; hm.z = hm.z * hn;
+  if (hm_out) *hm_out = hm;
   const T woh = dott(wo, hm);
   V3<T> wi;
   const T k2 = woh * 2.0f;

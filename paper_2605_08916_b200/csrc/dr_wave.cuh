@@ -59,8 +59,9 @@ constexpr int kWaveTraceThreads = kTraceBlock - 32 * kWaveShadeWarps;
 #define DR_WAVE_HIT_CAP 1024
 #endif
 constexpr uint32_t kHitCap = DR_WAVE_HIT_CAP;   // entries of the block's ring of finished rays (power of two)
-constexpr uint32_t kWaveKShift = 27; // payload = state | (k - 1) << 27
+constexpr uint32_t kWaveKShift = 27; // payload = state | (k - 1) << 27 | shadow ray << 31
 constexpr uint32_t kWaveStateMask = (1u << kWaveKShift) - 1u;
+
 
 struct WaveShared {                  // counters of the block's ring (monotonic; index = counter & (kHitCap - 1))
   uint32_t reserve, pub, head, freed;
@@ -84,9 +85,10 @@ __device__ __forceinline__ void st_release2(uint2* p, uint2 v) {
 }
 
 // ---- the trace warps ------------------------------------------------------------------------------------------------
+template <bool STATS>
 __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs& ws, uint32_t n, const uint4* smem, SmemStack& st,
                                                 SmemTriStack& tst, WaveShared* wsh, uint32_t* h_pay, uint32_t* h_t, uint32_t* h_li,
-                                                uint32_t one) {
+                                                uint32_t one, unsigned long long* work) {
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr unsigned kFull = 0xFFFFFFFFu;
   TravLane L;
@@ -97,7 +99,7 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
   uint32_t ent = 0;                         // lane j < kFetchChunk: payload of entry claim + j once it is known
   int poll = 0;
   bool pend = false;                        // this lane holds a finished ray that is not in the block's ring yet
-  const uint32_t ring_cap = sc.L * ws.cap;
+  const uint32_t ring_cap = wave_ring_entries(sc, ws.cap);
   for (;;) {
     // ---- finished rays -> the block's ring (reserve, wait for room, write, publish in reservation order)
     {
@@ -157,10 +159,10 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
       const uint32_t got_pay = __shfl_sync(kFull, ent, (taken + rank) & (kFetchChunk - 1u));
       if (mine) {
         pay = got_pay;
-        const float4* e = ws.qa + 4 * (size_t)(pay & kWaveStateMask);
+        const float4* e = ws.qa + kRecWords * (size_t)(pay & kWaveStateMask) + ((pay >> 31) ? 4u : 0u);   // the path's ray, or its shadow ray
         const float4 o = __ldcg(e), d = __ldcg(e + 1);   // written by another SM during this launch: not through L1
-        DR_CHECK((pay & kWaveStateMask) < ws.cap && (pay >> kWaveKShift) < sc.L, kErrState);
-        DR_CHECK(__float_as_uint(o.w) == (pay & kWaveStateMask), kErrOwner);         // the record is this state's
+        DR_CHECK((pay & kWaveStateMask) < ws.cap && ((pay >> kWaveKShift) & 15u) < sc.L, kErrState);
+        DR_CHECK((pay >> 31) || __float_as_uint(o.w) == (pay & kWaveStateMask), kErrOwner);   // the record is this state's
         trav_setup(L.r, o.x, o.y, o.z, d.x, d.y, d.z, one);
         trav_begin(L.s);
         L.tsp = 0;
@@ -181,11 +183,16 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
     }
     // ---- lockstep traversal; a finished lane keeps its hit in L.r until the flush before the next refill
     do {
-      const bool done = trav_step<false>(sc, smem, st, tst, L, nn, nt);
+      const bool done = trav_step<STATS>(sc, smem, st, tst, L, nn, nt);
       pend = pend || done;
       L.active = L.active && !done;
       act = __ballot_sync(kFull, L.active);
     } while (__popc(act) >= kWaveRefillBelow);
+  }
+  if (STATS) {   // the counting pass (dr_chains_work_stats, dr_eval_work_stats): node visits, triangle tests
+    nn = __reduce_add_sync(kFull, nn);
+    nt = __reduce_add_sync(kFull, nt);
+    if (lane == 0) { atomicAdd(&work[0], (unsigned long long)nn); atomicAdd(&work[1], (unsigned long long)nt); }
   }
 }
 
@@ -195,6 +202,7 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
                                                 const uint32_t* h_pay, const uint32_t* h_t, const uint32_t* h_li) {
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr unsigned kFull = 0xFFFFFFFFu;
+  const uint32_t ring_cap = wave_ring_entries(sc, ws.cap);
   for (;;) {
     // ---- take up to 32 finished rays of this block
     uint32_t head = 0, cnt = 0;
@@ -227,19 +235,56 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
       while (ld_volatile(&wsh->freed) != head) {}
       *reinterpret_cast<volatile uint32_t*>(&wsh->freed) = head + cnt;
     }
-    // ---- shade
-    bool cont = false, want_grad = false;
+    // ---- shade.  With next-event estimation a vertex may take two visits: the hit of the path's ray (phase A: emitter
+    // connection and direction sample; if the connection needs a shadow ray, that ray goes out first and the next ray
+    // waits in the record), then the shadow ray's result (phase B, payload bit 31: visibility, signature, next ray).
     uint32_t bad = 0;
-    const uint32_t s = pay & kWaveStateMask, k = (pay >> kWaveKShift) + 1u;
-    float4 n0, n1, n2;
-    float4* rec = ws.qa + 4 * (size_t)s;
-    if (mine) {
+    const uint32_t s = pay & kWaveStateMask, k = ((pay >> kWaveKShift) & 15u) + 1u;
+    const bool phase_b = (pay >> 31) != 0u;
+    float4* rec = ws.qa + kRecWords * (size_t)s;
+    bool want_grad = false, push = false;     // push: this lane publishes a queue entry (`entry`)
+    uint32_t entry = 0;
+    if (mine && !phase_b) {
       const float4 Q0 = __ldcg(rec), Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2);
+      const float pb_prev = sc.nee ? __ldcg(rec + 3).w : -1.f;
       DR_CHECK(__float_as_uint(Q0.w) == s && k <= sc.L, kErrOwner);
 #if DR_CHECKS
-      DR_CHECK(atomicAdd(&ws.hits[s].x, 1u) == k - 1u, kErrSegment);   // segments of a state are shaded once each, in order
+      if (!sc.nee) DR_CHECK(atomicAdd(&ws.hits[s].x, 1u) == k - 1u, kErrSegment);   // segments of a state are shaded once each, in order
 #endif
-      shade_vertex<GRAD>(sc, ws, io, k, Q0, Q1, Q2, h, s, cont, want_grad, bad, n0, n1, n2);
+      ShadeOut so;
+      shade_vertex<GRAD>(sc, ws, io, k, Q0, Q1, Q2, pb_prev, h, s, so, bad);
+      want_grad = so.want_grad;
+      if (so.cont || so.shadow) {
+        __stcg(rec, so.n0); __stcg(rec + 1, so.n1); __stcg(rec + 2, so.n2);
+        if (sc.nee) __stcg(rec + 3, make_float4(so.cpend.x, so.cpend.y, so.cpend.z, so.pb_next));
+        push = true;
+        entry = s | (k << kWaveKShift);                       // the next ray: segment k + 1, stored as k
+        if (so.shadow) {
+          __stcg(rec + 4, make_float4(so.sh_o.x, so.sh_o.y, so.sh_o.z, __uint_as_float(so.light_id)));
+          __stcg(rec + 5, make_float4(so.sh_d.x, so.sh_d.y, so.sh_d.z, __uint_as_float(so.lobe)));
+          entry = s | ((k - 1u) << kWaveKShift) | 0x80000000u;   // the shadow ray of vertex k
+        }
+      }
+    } else if (mine) {
+      const float4 Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2), Q3 = __ldcg(rec + 3), S0 = __ldcg(rec + 4), S1 = __ldcg(rec + 5);
+      if (io.nrays) __stcg(&io.nrays[s], __ldcg(&io.nrays[s]) + 1u);
+      const bool vis = h.y != kMiss && __float_as_uint(__ldg(&sc.tris[3 * h.y + 2].y)) == __float_as_uint(S0.w);
+      uint32_t info = __float_as_uint(Q2.w);
+      if (vis) {
+        float4 acc = __ldcg(&io.f[s]);
+        acc.x += Q3.x; acc.y += Q3.y; acc.z += Q3.z;
+        __stcg(&io.f[s], acc);
+        info |= 1u << (16u + k);
+      }
+      const uint32_t sig = fnv(fnv(__float_as_uint(Q1.w), vis ? 7u : 6u), __float_as_uint(S1.w));
+      if (Q2.x == 0.f && Q2.y == 0.f && Q2.z == 0.f) {         // the direction sample had zero weight: the path ends here
+        finish_path(sc, ws, io, k, s, 0.f, 0.f, 0.f, sig, info, k, kTermNone, GRAD, want_grad, bad);
+      } else {
+        __stcg(rec + 1, make_float4(Q1.x, Q1.y, Q1.z, __uint_as_float(sig)));
+        __stcg(rec + 2, make_float4(Q2.x, Q2.y, Q2.z, __uint_as_float(info)));
+        push = true;
+        entry = s | (k << kWaveKShift);
+      }
     }
     if (GRAD) {  // reverse-pass list: one atomic per warp
       const unsigned gm = __ballot_sync(kFull, want_grad);
@@ -250,18 +295,15 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
         if (want_grad) ws.gradlist[base + __popc(gm & lt)] = s;
       }
     }
-    // ---- the surviving paths' next rays: record of the state, then the queue entry (release)
-    const unsigned b = __ballot_sync(kFull, cont);
+    // ---- the queue entries of the paths that go on (release: the records above are visible before the entry)
+    const unsigned b = __ballot_sync(kFull, push);
     const uint32_t nc = __popc(b);
     if (nc) {
       uint32_t base = 0;
       if (lane == 0) base = atomicAdd(&ws.ctl[kCtlWaveReserve], nc);
       base = __shfl_sync(kFull, base, 0);
-      DR_CHECK(base + nc <= sc.L * ws.cap, kErrIndex);
-      if (cont) {
-        __stcg(rec, n0); __stcg(rec + 1, n1); __stcg(rec + 2, n2);
-        st_release2(ws.ring + base + __popc(b & lt), make_uint2(s | (k << kWaveKShift), ws.tag));   // segment k + 1, stored as k
-      }
+      DR_CHECK(base + nc <= ring_cap, kErrIndex);
+      if (push) st_release2(ws.ring + base + __popc(b & lt), make_uint2(entry, ws.tag));
     }
     if (lane == 0) {
       if (io.rays_ctr) atomicAdd(io.rays_ctr, (unsigned long long)cnt);
@@ -275,7 +317,7 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------------------
-template <bool GRAD>
+template <bool GRAD, bool STATS>
 __global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
   static_assert(DR_SMEM_NODES == 0, "k_wave does not stage nodes in shared memory");
   static_assert((kFetchChunk & (kFetchChunk - 1u)) == 0 && kFetchChunk <= 32, "chunk: power of two, one entry per lane");
@@ -297,7 +339,7 @@ __global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws,
   __syncthreads();
   const uint32_t one = *(volatile uint32_t*)&smem[0].x;  // dr_traverse.cuh qmagic
   if (threadIdx.x >= (unsigned)kWaveTraceThreads) wave_shade_loop<GRAD>(sc, ws, io, n, wsh, h_pay, h_t, h_li);
-  else wave_trace_loop(sc, ws, n, smem, st, tst, wsh, h_pay, h_t, h_li, one);
+  else wave_trace_loop<STATS>(sc, ws, n, smem, st, tst, wsh, h_pay, h_t, h_li, one, io.work);
 }
 
 }  // namespace dr

@@ -173,10 +173,24 @@ def test_tie_rule_coplanar_box_on_floor(dr, oracle, torch_):
 
 
 # ---- a3, a5, a6: target evaluation --------------------------------------------------------------------------------
-@pytest.mark.parametrize("scene", ["furnace", "cornell", "mini_machines", "ggx_room", "closed_furnace", "mixture3"])
+def _nee(desc):
+    import copy
+    d = copy.copy(desc)
+    d.nee = True
+    d.name = desc.name + "_nee"
+    return d
+
+
+EVAL_SCENES = {"furnace": S.furnace, "cornell": lambda: S.cornell(width=64, height=64), "mini_machines": S.mini_machines,
+               "ggx_room": S.ggx_room, "closed_furnace": S.closed_furnace, "mixture3": S.mixture3,
+               # next-event estimation + MIS (Q21): four coordinates per vertex, shadow rays, position-dependent score
+               "cornell_nee": lambda: _nee(S.cornell(width=64, height=64)), "mini_machines_nee": lambda: _nee(S.mini_machines()),
+               "ggx_room_nee": lambda: _nee(S.ggx_room()), "closed_furnace_nee": lambda: _nee(S.closed_furnace())}
+
+
+@pytest.mark.parametrize("scene", list(EVAL_SCENES))
 def test_eval_matches_oracle(dr, oracle, torch_, scene):
-    desc = {"furnace": S.furnace, "cornell": lambda: S.cornell(width=64, height=64), "mini_machines": S.mini_machines,
-            "ggx_room": S.ggx_room, "closed_furnace": S.closed_furnace, "mixture3": S.mixture3}[scene]()
+    desc = EVAL_SCENES[scene]()
     gsc = dr.Scene(desc)
     osc = oracle.Scene(desc, oracle.F32)
     n = 30011
@@ -189,15 +203,29 @@ def test_eval_matches_oracle(dr, oracle, torch_, scene):
     assert div.mean() < 1e-3, div.sum()                                         # near-threshold decisions: counted
     ok = ~div
     assert (g["nrays"][ok] == e["nrays"][ok]).all()
+    if scene.endswith("_nee"):
+        # a connection that grazes the emitter (cos_l -> 0) or is very short divides by a cancelled quantity: fp32 on either
+        # side then carries a relative error far above its usual 1e-7.  Such states are counted with the diverged ones.
+        ill = np.abs(g["p"] - e["p"]) > 1e-4 * np.maximum(e["p"], 1e-8)
+        assert (div | ill).mean() < 1e-3, (div.sum(), ill.sum())
+        ok &= ~ill
     rel = np.abs(g["p"][ok] - e["p"][ok]) / np.maximum(e["p"][ok], 1e-8)
     assert rel.max() <= 1e-4, rel.max()
     relf = np.abs(g["f"][ok] - e["f"][ok]) / np.maximum(np.abs(e["f"][ok]), 1e-8)
     assert relf.max() <= 1e-4
     stddev = 5e-3
     tol = 1e-4 * np.abs(e["g"][ok]) + 2e-4 / stddev
-    assert (np.abs(g["g"][ok] - e["g"][ok]) <= tol).all()
-    if scene in ("mini_machines", "ggx_room"):
+    bad = np.abs(g["g"][ok] - e["g"][ok]) > tol
+    if scene.endswith("_nee"):      # the same near-singular connections, seen through the derivative of 1 / cos_l and 1 / r^2
+        assert (div.sum() + ill.sum() + bad.any(1).sum()) < 1e-3 * n, (div.sum(), ill.sum(), bad.any(1).sum())
+        rel_g = np.abs(g["g"][ok] - e["g"][ok])[bad] / np.abs(e["g"][ok][bad])
+        assert (rel_g < 5e-2).all(), rel_g                                      # and even there a relative error of per cent
+    else:
+        assert not bad.any(), (int(bad.sum()), float(np.abs(g["g"][ok] - e["g"][ok]).max()))
+    if scene in ("mini_machines", "ggx_room") or scene.endswith("_nee"):
         assert (np.abs(e["g"][ok]).max(1) > 0).sum() > 20                       # the score path is exercised
+    if scene.endswith("_nee"):
+        assert (e["p"] > 0).mean() > 0.2 and (e["nrays"] > desc.max_path_len).any()   # connections are live, shadow rays counted
     # without the score the value outputs are identical
     g2 = gsc.eval_states(torch_.from_numpy(x).cuda(), want_score=False)
     assert np.allclose(g2["p"].cpu().numpy(), g["p"], rtol=1e-6, atol=0) and (g2["sig"].cpu().numpy() == g["sig"]).all()
@@ -237,6 +265,17 @@ def test_teacher_forced_parity(dr, oracle, torch_, method, case):
     _teacher_forced(dr, oracle, torch_, method, case)
 
 
+CASES_NEE = [("cornell_nee", lambda: _nee(S.cornell(width=64, height=64, max_path_len=5)), 6000),
+             ("mini_machines_nee", lambda: _nee(S.mini_machines()), 5000), ("ggx_room_nee", lambda: _nee(S.ggx_room()), 3001)]
+
+
+@pytest.mark.parametrize("method", METHODS + ["path_tracing"])
+@pytest.mark.parametrize("case", CASES_NEE, ids=[c[0] for c in CASES_NEE])
+def test_teacher_forced_parity_with_nee(dr, oracle, torch_, method, case):
+    """every sampler on scenes with next-event estimation + MIS, same protocol."""
+    _teacher_forced(dr, oracle, torch_, method, case)
+
+
 EXTRA = [("path_tracing", {}), ("metropolis_restore", dict(rao_blackwell=True)), ("mala_restore", dict(rao_blackwell=True)),
          ("diffusion_restore", dict(rao_blackwell=True))]
 
@@ -266,7 +305,8 @@ def _teacher_forced(dr, oracle, torch_, method, case, **kw):
     assert np.isclose(gst["p_lambda"], ost["p_lambda"], rtol=2e-6) and np.isclose(gst["kappa0"], ost["kappa0"], rtol=2e-6)
     assert gst["mutations"] == ost["mutations"] == N
     g_last, o_last = gch.last_step(), och.last()
-    div, rep = compare_states(gs, os_, g_last, o_last, stddev)
+    fold = bool(getattr(desc, "nee", False))
+    div, rep = compare_states(gs, os_, g_last, o_last, stddev, fold_outliers=fold)
     assert div.mean() < 1e-3, rep
     nr_g, nr_o = gsc.eval_states(torch_.from_numpy(gs["x"]).cuda(), False)["nrays"].cpu().numpy(), osc.eval(os_["x"], False)["nrays"]
     assert gst["rays"] == int(nr_g.sum()) and ost["rays"] == int(nr_o.sum()) and (nr_g[~div] == nr_o[~div]).all()   # closest-hit queries: counted exactly
@@ -285,7 +325,7 @@ def _teacher_forced(dr, oracle, torch_, method, case, **kw):
         och.step(1)
         gs, os_ = gch.download(), och.state()
         g_last, o_last = gch.last_step(), och.last()
-        div, rep = compare_states(gs, os_, g_last, o_last, stddev)
+        div, rep = compare_states(gs, os_, g_last, o_last, stddev, fold_outliers=fold)
         worst = max(worst, rep["frac"])
         assert div.mean() < 1e-3, (method, name, burst, rep)
         compare_bulk(gch, och, gs, os_, g_last, o_last, div, gch.stats()["tours"] - t0g, och.stats()["tours"] - t0o)
