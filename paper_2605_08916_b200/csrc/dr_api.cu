@@ -197,11 +197,14 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
   if (wave) {
     ProfScope ps(prof, DR_PROF_TRACE, s);
     const size_t sm = sc->trace_smem + kWaveExtraSmem;
-    if (stats) {   // the counting pass of a scene with next-event estimation (others count in k_trace<true>)
-      if (grad) k_wave<true, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
-      else k_wave<false, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
-    } else if (grad) k_wave<true, false><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
-    else k_wave<false, false><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+    if (dev.nee) {
+      if (stats) {   // the counting pass of a scene with next-event estimation (others count in k_trace<true>)
+        if (grad) k_wave<true, true, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+        else k_wave<false, true, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+      } else if (grad) k_wave<true, false, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+      else k_wave<false, false, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+    } else if (grad) k_wave<true, false, false><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+    else k_wave<false, false, false><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
   } else
   for (uint32_t k = 1; k <= dev.L; ++k) {
     const float4* q = (k & 1u) ? ws.qa : ws.qb;
@@ -378,10 +381,10 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   s->wave_ok = DR_SMEM_NODES == 0 && s->trace_smem + kWaveExtraSmem <= kMaxDynSmem;
   e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_wave<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  const void* waves[] = {(const void*)k_wave<false, false, false>, (const void*)k_wave<true, false, false>, (const void*)k_wave<false, false, true>,
+                         (const void*)k_wave<true, false, true>, (const void*)k_wave<false, true, true>, (const void*)k_wave<true, true, true>};
+  for (const void* w : waves)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(w, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e != cudaSuccess) {
     dr_scene_destroy(s);
     return fail(DR_ERR_CUDA, std::string("k_trace shared memory: ") + cudaGetErrorString(e));

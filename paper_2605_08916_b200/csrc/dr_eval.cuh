@@ -366,17 +366,19 @@ struct ShadeOut {
 
 constexpr uint32_t kTermNone = 0xFFFFFFFEu;   // the path ended without a terminal contribution (length cap, zero-weight direction)
 // nv: vertices that sampled (1 .. nv), term: the triangle the last ray hit (leaf order), kMiss (environment) or kTermNone
-__device__ __forceinline__ void finish_path(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t k, uint32_t s, float f0, float f1,
+template <bool NEE>
+__device__ __forceinline__ void finish_path(const DevScene& sc_, const EvalWs& ws, const EvalIO& io, uint32_t k, uint32_t s, float f0, float f1,
                                             float f2, uint32_t sig, uint32_t info, uint32_t nv, uint32_t term, bool grad, bool& want_grad,
                                             uint32_t& bad) {
-  if (sc.nee) { const float4 acc = __ldcg(&io.f[s]); f0 = acc.x + f0; f1 = acc.y + f1; f2 = acc.z + f2; }   // emitter connections so far
+  const bool nee = NEE && sc_.nee;
+  if (nee) { const float4 acc = __ldcg(&io.f[s]); f0 = acc.x + f0; f1 = acc.y + f1; f2 = acc.z + f2; }   // emitter connections so far
   float p = f0 * 0.2126f + f1 * 0.7152f + f2 * 0.0722f;
   if (!(isfinite(f0) && isfinite(f1) && isfinite(f2) && isfinite(p))) { f0 = f1 = f2 = p = 0.f; bad = 1; }
   __stcg(&io.f[s], make_float4(f0, f1, f2, p));
   io.sig[s] = sig;
-  if (io.nrays && !sc.nee) io.nrays[s] = k;
+  if (io.nrays && !nee) io.nrays[s] = k;
   if (grad) {
-    if (sc.nee) {
+    if (nee) {
       ws.rec[s] = make_float4(__uint_as_float(info), __uint_as_float(k), __uint_as_float(term), __uint_as_float(nv));   // plane 0 of the vertex record
       want_grad = p > 0.f;                                                          // geometry and MIS terms depend on x
     } else {
@@ -387,7 +389,7 @@ __device__ __forceinline__ void finish_path(const DevScene& sc, const EvalWs& ws
   }
 }
 
-template <bool GRAD>
+template <bool GRAD, bool NEE>
 __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t k, const float4& Q0,
                                              const float4& Q1, const float4& Q2, float pb_prev, const uint2& h, uint32_t s, ShadeOut& out,
                                              uint32_t& bad) {
@@ -399,7 +401,7 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
   bool done = true;
   uint32_t term = h.y;          // what the path's last ray hit, if it ends here with a contribution
   out.cont = false; out.shadow = false; out.want_grad = false;
-  if (sc.nee && io.nrays) __stcg(&io.nrays[s], __ldcg(&io.nrays[s]) + 1u);   // L2: successive events of a path run on different SMs
+  if (NEE && sc.nee && io.nrays) __stcg(&io.nrays[s], __ldcg(&io.nrays[s]) + 1u);   // L2: successive events of a path run on different SMs
   if (h.y == kMiss) {
     sig = fnv(sig, 0u);
     f0 = T0 * sc.env[0]; f1 = T1 * sc.env[1]; f2 = T2 * sc.env[2];
@@ -419,7 +421,7 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
         sig = fnv(sig, 4u);
         const float4 m2 = __ldg(&sc.mats[3 * mi + 2]);
         const V3<float> ov{o.x, o.y, o.z}, dv{d.x, d.y, d.z};
-        const float w_b = emitter_weight<float>(sc, xyz(t0), fr.nf, ov, dv, pb_prev, pb_prev >= 0.f);   // dn < 0: nf = n
+        const float w_b = emitter_weight<float, NEE>(sc, xyz(t0), fr.nf, ov, dv, pb_prev, pb_prev >= 0.f);   // dn < 0: nf = n
         f0 = T0 * m1.z * w_b; f1 = T1 * m1.w * w_b; f2 = T2 * m2.x * w_b;
       } else {
         sig = fnv(sig, 5u);
@@ -434,13 +436,13 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
       V3<float> hit;
       bool reflect = false;
       uint32_t lj = 0;
-      vertex_fn<float>(sc, xyz(t0), fr, dn, m0, m1, kind, ov, dv, u.x, u.y, u.z, u.w, true, reflect, vo, hit, lj);
+      vertex_fn<float, NEE>(sc, xyz(t0), fr, dn, m0, m1, kind, ov, dv, u.x, u.y, u.z, u.w, true, reflect, vo, hit, lj);
       uint32_t lobe = kind == 0u ? 0u : (kind == 1u ? (reflect ? 1u : 2u) : 3u);
       if (kind == 1u && !reflect) info |= 1u << k;
       if (kind == 2u) info |= 1u << 16;
       T0 *= vo.W[0]; T1 *= vo.W[1]; T2 *= vo.W[2];
       const bool alive = !(T0 == 0.f && T1 == 0.f && T2 == 0.f);
-      if (vo.nee_valid) {   // the vertex is completed by nee_finish() once the shadow ray is back
+      if (NEE && vo.nee_valid) {   // the vertex is completed by nee_finish() once the shadow ray is back
         const Light Lt = load_light(sc, lj);
         out.shadow = true;
         out.light_id = Lt.id;
@@ -453,9 +455,9 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
       } else {
         sig = fnv(sig, lobe);
       }
-      if (alive || vo.nee_valid) {
+      if (alive || (NEE && vo.nee_valid)) {
         done = false;
-        out.cont = alive && !vo.nee_valid;
+        out.cont = alive && !(NEE && vo.nee_valid);
         out.n0 = make_float4(vo.o2.x, vo.o2.y, vo.o2.z, Q0.w);
         out.n1 = make_float4(vo.d2.x, vo.d2.y, vo.d2.z, __uint_as_float(sig));
         out.n2 = make_float4(T0, T1, T2, __uint_as_float(info));
@@ -465,7 +467,7 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
       term = kTermNone;   // length cap on a surface: nothing is added
     }
   }
-  if (done) finish_path(sc, ws, io, k, s, f0, f1, f2, sig, info, k - 1u, term, GRAD, out.want_grad, bad);
+  if (done) finish_path<NEE>(sc, ws, io, k, s, f0, f1, f2, sig, info, k - 1u, term, GRAD, out.want_grad, bad);
 }
 
 // ---- a3 / a5: shade vertex k of every ray of segment k -------------------------------------------------------------
@@ -485,7 +487,7 @@ __global__ void __launch_bounds__(kShadeBlock) k_shade(DevScene sc, EvalWs ws, E
   if (j < n) {
     const float4 Q0 = qin[j], Q1 = qin[cap + j], Q2 = qin[2 * cap + j];
     s = __float_as_uint(Q0.w);
-    shade_vertex<GRAD>(sc, ws, io, k, Q0, Q1, Q2, -1.f, ws.hits[j], s, so, bad);
+    shade_vertex<GRAD, false>(sc, ws, io, k, Q0, Q1, Q2, -1.f, ws.hits[j], s, so, bad);
   }
   const bool cont = so.cont, want_grad = so.want_grad;
   const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;

@@ -81,7 +81,10 @@ __device__ __noinline__ float4 emitter_weight_grad(const DevScene& sc, float3 v0
   return make_float4(w.d[0], w.d[1], w.d[2], w.d[3]);
 }
 
-__global__ void __launch_bounds__(kGradBlock) k_grad_nee(DevScene sc, EvalWs ws, EvalIO io) {
+#ifndef DR_GRAD_MIN_BLOCKS
+#define DR_GRAD_MIN_BLOCKS 6   // 80 registers: 1 / 3 / 4 / 6 blocks per SM: 6.12 / 5.90 / 5.64 / 5.32 ms per frame (configs[3] + NEE)
+#endif
+__global__ void __launch_bounds__(kGradBlock, DR_GRAD_MIN_BLOCKS) k_grad_nee(DevScene sc, EvalWs ws, EvalIO io) {
   const uint32_t idx = blockIdx.x * kGradBlock + threadIdx.x;
   if (idx == 0 && io.grad_ctr) atomicAdd(io.grad_ctr, (unsigned long long)ws.ctl[kCtlGrad]);
   if (idx >= ws.ctl[kCtlGrad]) return;

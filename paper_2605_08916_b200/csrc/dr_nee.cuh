@@ -63,7 +63,7 @@ template <class T> struct VertexOut {
 };
 
 // hit: the point on the triangle's plane.  `decide`: take the lobe decision here (float instantiation) or use `reflect`.
-template <class T>
+template <class T, bool NEE = true>
 __device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const Frame& fr, float dn, float4 m0, float4 m1, uint32_t kind,
                                           V3<T> o, V3<T> d, T u1, T u2, T v1, T v2, bool decide, bool& reflect, VertexOut<T>& out,
                                           V3<T>& hit_out, uint32_t& light_j) {
@@ -77,7 +77,7 @@ __device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const F
   out.nee_valid = false;
   out.fcos[0] = out.fcos[1] = out.fcos[2] = out.lw[0] = out.lw[1] = out.lw[2] = lift_t<T>(0.f);
   // ---- next-event estimation at a Lambert / GGX vertex (Q21)
-  if (sc.nee && kind != 1u && sc.n_lights) {
+  if (NEE && sc.nee && kind != 1u && sc.n_lights) {
     const uint32_t j = pick_light(sc, val(v1));
     light_j = j;
     const Light L = load_light(sc, j);
@@ -144,7 +144,7 @@ __device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const F
       out.d2 = d;
     } else {
       out.W[0] = (m0.y + (1.0f - m0.y) * c5) * G1; out.W[1] = (m0.z + (1.0f - m0.z) * c5) * G1; out.W[2] = (m0.w + (1.0f - m0.w) * c5) * G1;
-      if (sc.nee) {
+      if (NEE && sc.nee) {
         V3<T> wo;
         wo.x = -dotf(d, fr.t); wo.y = -dotf(d, fr.bf); wo.z = -dotf(d, fr.nf);
         out.pb_valid = true;
@@ -157,9 +157,9 @@ __device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const F
 }
 
 // An emitter reached by the direction sample (front face): balance-heuristic weight against next-event estimation.
-template <class T>
+template <class T, bool NEE = true>
 __device__ __forceinline__ T emitter_weight(const DevScene& sc, float3 v0, float3 n, V3<T> o, V3<T> d, T pb, bool pb_valid) {
-  if (!(sc.nee && pb_valid)) return lift_t<T>(1.f);
+  if (!(NEE && sc.nee && pb_valid)) return lift_t<T>(1.f);
   const T te = dotf(vsubf(v0, o), n) / dotf(d, n);
   const T p_l = (te * te) / ((-dotf(d, n)) * sc.light_total);
   return pb / (pb + p_l);

@@ -197,7 +197,7 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
 }
 
 // ---- the shade warps ------------------------------------------------------------------------------------------------
-template <bool GRAD>
+template <bool GRAD, bool NEE>
 __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t n, WaveShared* wsh,
                                                 const uint32_t* h_pay, const uint32_t* h_t, const uint32_t* h_li) {
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
@@ -246,26 +246,26 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
     uint32_t entry = 0;
     if (mine && !phase_b) {
       const float4 Q0 = __ldcg(rec), Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2);
-      const float pb_prev = sc.nee ? __ldcg(rec + 3).w : -1.f;
+      const float pb_prev = NEE ? __ldcg(rec + 3).w : -1.f;
       DR_CHECK(__float_as_uint(Q0.w) == s && k <= sc.L, kErrOwner);
 #if DR_CHECKS
-      if (!sc.nee) DR_CHECK(atomicAdd(&ws.hits[s].x, 1u) == k - 1u, kErrSegment);   // segments of a state are shaded once each, in order
+      if (!NEE) DR_CHECK(atomicAdd(&ws.hits[s].x, 1u) == k - 1u, kErrSegment);   // segments of a state are shaded once each, in order
 #endif
       ShadeOut so;
-      shade_vertex<GRAD>(sc, ws, io, k, Q0, Q1, Q2, pb_prev, h, s, so, bad);
+      shade_vertex<GRAD, NEE>(sc, ws, io, k, Q0, Q1, Q2, pb_prev, h, s, so, bad);
       want_grad = so.want_grad;
       if (so.cont || so.shadow) {
         __stcg(rec, so.n0); __stcg(rec + 1, so.n1); __stcg(rec + 2, so.n2);
-        if (sc.nee) __stcg(rec + 3, make_float4(so.cpend.x, so.cpend.y, so.cpend.z, so.pb_next));
+        if (NEE) __stcg(rec + 3, make_float4(so.cpend.x, so.cpend.y, so.cpend.z, so.pb_next));
         push = true;
         entry = s | (k << kWaveKShift);                       // the next ray: segment k + 1, stored as k
-        if (so.shadow) {
+        if (NEE && so.shadow) {
           __stcg(rec + 4, make_float4(so.sh_o.x, so.sh_o.y, so.sh_o.z, __uint_as_float(so.light_id)));
           __stcg(rec + 5, make_float4(so.sh_d.x, so.sh_d.y, so.sh_d.z, __uint_as_float(so.lobe)));
           entry = s | ((k - 1u) << kWaveKShift) | 0x80000000u;   // the shadow ray of vertex k
         }
       }
-    } else if (mine) {
+    } else if (NEE && mine) {
       const float4 Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2), Q3 = __ldcg(rec + 3), S0 = __ldcg(rec + 4), S1 = __ldcg(rec + 5);
       if (io.nrays) __stcg(&io.nrays[s], __ldcg(&io.nrays[s]) + 1u);
       const bool vis = h.y != kMiss && __float_as_uint(__ldg(&sc.tris[3 * h.y + 2].y)) == __float_as_uint(S0.w);
@@ -278,7 +278,7 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
       }
       const uint32_t sig = fnv(fnv(__float_as_uint(Q1.w), vis ? 7u : 6u), __float_as_uint(S1.w));
       if (Q2.x == 0.f && Q2.y == 0.f && Q2.z == 0.f) {         // the direction sample had zero weight: the path ends here
-        finish_path(sc, ws, io, k, s, 0.f, 0.f, 0.f, sig, info, k, kTermNone, GRAD, want_grad, bad);
+        finish_path<NEE>(sc, ws, io, k, s, 0.f, 0.f, 0.f, sig, info, k, kTermNone, GRAD, want_grad, bad);
       } else {
         __stcg(rec + 1, make_float4(Q1.x, Q1.y, Q1.z, __uint_as_float(sig)));
         __stcg(rec + 2, make_float4(Q2.x, Q2.y, Q2.z, __uint_as_float(info)));
@@ -317,7 +317,8 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
 }
 
 // ---- the kernel -----------------------------------------------------------------------------------------------------
-template <bool GRAD, bool STATS>
+// NEE: the scene uses next-event estimation (two-phase vertices, shadow rays); STATS: the counting pass (NEE scenes only)
+template <bool GRAD, bool STATS, bool NEE>
 __global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
   static_assert(DR_SMEM_NODES == 0, "k_wave does not stage nodes in shared memory");
   static_assert((kFetchChunk & (kFetchChunk - 1u)) == 0 && kFetchChunk <= 32, "chunk: power of two, one entry per lane");
@@ -338,7 +339,7 @@ __global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws,
   }
   __syncthreads();
   const uint32_t one = *(volatile uint32_t*)&smem[0].x;  // dr_traverse.cuh qmagic
-  if (threadIdx.x >= (unsigned)kWaveTraceThreads) wave_shade_loop<GRAD>(sc, ws, io, n, wsh, h_pay, h_t, h_li);
+  if (threadIdx.x >= (unsigned)kWaveTraceThreads) wave_shade_loop<GRAD, NEE>(sc, ws, io, n, wsh, h_pay, h_t, h_li);
   else wave_trace_loop<STATS>(sc, ws, n, smem, st, tst, wsh, h_pay, h_t, h_li, one, io.work);
 }
 

@@ -287,6 +287,50 @@ def test_teacher_forced_parity_pt_and_rao_blackwell(dr, oracle, torch_, variant,
     _teacher_forced(dr, oracle, torch_, variant[0], case, **variant[1])
 
 
+def test_sharded_chains_against_the_oracle(dr, oracle, torch_):
+    """a shard (global chain ids 1000 .. 1999 of a 2000-chain run) against the oracle's shard with the same
+    chain_offset, teacher-forced like everything else: the RNG streams are keyed by global chain id on both sides."""
+    _teacher_forced(dr, oracle, torch_, "diffusion_restore", ("mini_machines", S.mini_machines, 1000), chain_offset=1000, p_lambda_override=0.05)
+    _teacher_forced(dr, oracle, torch_, "metropolis", ("ggx_room", S.ggx_room, 999), chain_offset=12345)
+
+
+def test_scene_change_reinitialises_everything(dr, oracle, torch_):
+    """when the scene changes (camera, geometry) all accumulated samples are invalid and the whole stateBuffer
+    is initialised again (Alg. 1).  As a call sequence: new dr_scene, dr_chains_create on the SAME caller-owned memory,
+    dr_chains_init(frame_index): states are the Philox uniforms of that frame's epoch, buffer and counters start from zero,
+    and the result equals a run that never saw the first scene."""
+    d1, d2 = S.mini_machines(), S.mini_machines(seed=8)                          # "the geometry changed"
+    N = 4096
+    a = dr.Chains(dr.Scene(d1), "diffusion_restore", N, seed=9)
+    a.init(0)
+    a.step(5)
+    a.resolve()
+    assert a.stats()["tours"] > 0 and float(a.accum.abs().sum()) > 0
+    sc2 = dr.Scene(d2)
+    b = dr.Chains(sc2, "diffusion_restore", N, seed=9)
+    b.state, b.accum = a.state, a.accum                                         # reuse the memory of the old ensemble
+    import ctypes as C
+    h = C.c_void_p()
+    dr.binding._check(dr.lib.dr_chains_create(sc2.h, C.byref(b.cfg), C.c_void_p(a.state.data_ptr()), a.state.numel(),
+                                              C.c_void_p(a.accum.data_ptr()), C.byref(h)))
+    dr.lib.dr_chains_destroy(b.h)
+    b.h = h
+    b.init(7)                                                                   # frame 7: a new epoch of every stream
+    fresh = dr.Chains(dr.Scene(d2), "diffusion_restore", N, seed=9)
+    fresh.init(7)
+    sb, sf = b.download(), fresh.download()
+    for k in sb:
+        assert np.array_equal(sb[k].view(np.uint8), sf[k].view(np.uint8)), k
+    stb, stf = b.stats(), fresh.stats()
+    assert stb["mutations"] == stf["mutations"] == N and stb["tours"] == stf["tours"] and stb["iteration"] == 0
+    assert torch_.allclose(b.accum, fresh.accum, rtol=1e-5, atol=1e-9)             # float atomics: order of the addends
+    och = oracle.Chains(oracle.Scene(d2, oracle.F32), "diffusion_restore", N, seed=9)
+    och.init(7)
+    assert (sb["x"].astype(np.float64) == och.state()["x"]).all()                # the epoch-7 uniforms, bit-exact
+    b.step(3); fresh.step(3)
+    assert np.array_equal(b.download()["x"], fresh.download()["x"])
+
+
 def _teacher_forced(dr, oracle, torch_, method, case, **kw):
     name, make, N = case
     desc = make()
