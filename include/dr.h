@@ -220,6 +220,12 @@ dr_status dr_chains_set_eval_form(dr_chains* chains, int32_t form);
 /* Work statistics for n states (device x[n*d], values only): dev_out3[0..2] += {rays, BVH8 node visits, triangle
  * tests}.  bench.py derives the algorithmic FLOPs per ray of its roofline from these. */
 dr_status dr_eval_work_stats(const dr_scene* scene, const float* dev_x, uint32_t n, uint64_t* dev_out3, void* stream);
+/* Appendix C of the paper: the field b = L^* p_hat / p_hat that controls the bias of the
+ * modified killing rate, for the Alg. 4 dynamics (step width stddev, rotation c_tilde, holding rate 1 / dt) on a 2-D analytic
+ * scene.  dev_out[iy * G + ix] (double) = b at the centre of cell (ix, iy) of a G x G grid; the integral over the torus is a
+ * midpoint rule on M x M points, in double (the difference cancels to O(dt)).  Analysis only: not part of dr_step.  Synchronises. */
+dr_status dr_bias_field(const dr_scene* scene, double stddev, double c_tilde, double dt, uint32_t G, uint32_t M, double* dev_out,
+                        void* stream);
 /* Raw Philox blocks for n counters (device arrays ctr[4n] -> out[4n]) under key (seed lo, hi), and the stream
  * transforms of DESIGN.md Q14 for n words pairs: out[4n] = u[0,1), u(0,1], Box-Muller z0, z1. */
 dr_status dr_philox_blocks(uint64_t seed, const uint32_t* dev_ctr, uint32_t n, uint32_t* dev_out, void* stream);

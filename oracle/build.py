@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "liboracle.so")
 SOURCES = ["capi.cpp"]
-HEADERS = ["philox.hpp", "dual.hpp", "scene.hpp", "path.hpp", "analytic2d.hpp", "samplers.hpp"]
+HEADERS = ["philox.hpp", "dual.hpp", "scene.hpp", "path.hpp", "analytic2d.hpp", "samplers.hpp", "bias.hpp"]
 
 
 def stale() -> bool:

@@ -11,6 +11,7 @@
 #include <memory>
 #include <vector>
 
+#include "bias.hpp"
 #include "samplers.hpp"
 
 using namespace orc;
@@ -160,6 +161,13 @@ void orc_pt_render(void* h_, uint64_t n, uint64_t seed, double* rgb) {
   WITH_SCENE(h, S, pt_render(S, n, seed, rgb));
 }
 
+// Appendix-C bias field of the analytic target on a G x G grid (bias.hpp); M x M quadrature points
+void orc_bias_field(void* h_, double stddev, double c_tilde, double dt, uint32_t G, uint32_t M, double* out) {
+  auto* h = (SceneH*)h_;
+  if (h->prec == 0) bias_field<float>(h->f, (float)stddev, (float)c_tilde, (float)dt, G, M, out);
+  else bias_field<double>(h->d, stddev, c_tilde, dt, G, M, out);
+}
+
 void* orc_chains_create(void* scene_, int method, uint32_t n_chains, double stddev, double c_tilde, double dt, double m,
                         double large_step_prob, double p_lambda_override, uint64_t seed, uint32_t chain_offset, int rao_blackwell) {
   auto* s = (SceneH*)scene_;
@@ -170,6 +178,11 @@ void* orc_chains_create(void* scene_, int method, uint32_t n_chains, double stdd
   return h;
 }
 void orc_chains_destroy(void* h) { delete (ChainsH*)h; }
+// f4 (Q24): a_mode and the regeneration density (G x G tile probabilities summing to one; G = 0: uniform); before init
+void orc_chains_set_f4(void* h_, int a_mode, uint32_t G, const double* w) {
+  auto* h = (ChainsH*)h_;
+  WITH_CHAINS(h, C, { C.cfg.a_mode = a_mode; C.cfg.rho_grid = G; C.cfg.rho_w.assign(w, w + (size_t)G * G); });
+}
 void orc_chains_init(void* h_, uint32_t frame) { auto* h = (ChainsH*)h_; WITH_CHAINS(h, C, C.init(frame)); }
 void orc_chains_step(void* h_, uint32_t iters) { auto* h = (ChainsH*)h_; WITH_CHAINS(h, C, C.step(iters)); }
 void orc_chains_get_state(void* h_, double* x, double* p, double* fop, uint32_t* pix, uint8_t* killed, double* g, uint32_t* sig) {

@@ -36,9 +36,11 @@ def lib():
         L.orc_trace.argtypes = [vp, vp, vp, u32, i32, vp, vp]
         L.orc_eval.argtypes = [vp, vp, u32, i32, vp, vp, vp, vp, vp, vp, vp]
         L.orc_pt_render.argtypes = [vp, u64, u64, vp]
+        L.orc_bias_field.argtypes = [vp, f64, f64, f64, u32, u32, vp]
         L.orc_chains_create.restype = vp
         L.orc_chains_create.argtypes = [vp, i32, u32, f64, f64, f64, f64, f64, f64, u64, u32, i32]
         L.orc_chains_destroy.argtypes = [vp]
+        L.orc_chains_set_f4.argtypes = [vp, i32, u32, vp]
         L.orc_chains_init.argtypes = [vp, u32]
         L.orc_chains_step.argtypes = [vp, u32]
         L.orc_chains_get_state.argtypes = [vp] * 8
@@ -157,6 +159,12 @@ class Scene:
                        _p(out["sig"]), _p(out["g"]), _p(out["nonfinite"]))
         return out
 
+    def bias_field(self, stddev: float, c_tilde: float, dt: float, G: int = 64, M: int = 256) -> np.ndarray:
+        """Appendix C: (L^* p_hat / p_hat) of the analytic target on a G x G grid (rows = x1), M x M quadrature points."""
+        out = np.zeros((G, G), dtype=np.float64)
+        lib().orc_bias_field(self.h, float(stddev), float(c_tilde), float(dt), int(G), int(M), _p(out))
+        return out
+
     def pt_render(self, n_samples: int, seed: int = 0) -> np.ndarray:
         rgb = np.zeros((self.npix, 3), dtype=np.float64)
         lib().orc_pt_render(self.h, int(n_samples), int(seed), _p(rgb))
@@ -167,7 +175,7 @@ class Chains:
     """Oracle-side chain ensemble: Alg. 1-4 of the paper, one plain loop over chains."""
 
     def __init__(self, scene: Scene, method, n_chains, stddev=None, c_tilde=None, dt=1e-5, m=64.0, large_step_prob=None,
-                 p_lambda_override=0.0, seed=0, chain_offset=0, rao_blackwell=False):
+                 p_lambda_override=0.0, seed=0, chain_offset=0, rao_blackwell=False, a_mode=0, rho=None):
         method = METHODS[method] if isinstance(method, str) else int(method)
         if stddev is None:
             stddev = 1e-2 if method in (0, 2) else 5e-3       # PAPER.md L747
@@ -180,6 +188,10 @@ class Chains:
                            p_lambda_override=p_lambda_override, seed=seed)
         self.h = lib().orc_chains_create(scene.h, method, self.N, stddev, c_tilde, dt, m, large_step_prob,
                                          p_lambda_override, int(seed), int(chain_offset), int(bool(rao_blackwell)))
+        if a_mode or rho is not None:      # f4: another antisymmetric pattern / a regeneration density on film tiles (float32 weights)
+            w = np.zeros(0) if rho is None else np.ascontiguousarray(rho, dtype=np.float32).astype(np.float64)
+            G = 0 if rho is None else int(round(np.sqrt(w.size)))
+            lib().orc_chains_set_f4(self.h, int(a_mode), G, _p(w.ravel()))
 
     def __del__(self):
         if getattr(self, "h", None) and _lib is not None:

@@ -39,6 +39,14 @@ struct Config {
   uint32_t chain_offset;    // global id of chain 0 (chains are keyed by global id: sharding-invariant, section 8e)
   int rao_blackwell;        // Restore variants: accumulate E[dtau | x] = 1 / (lambda + kappa) instead of the sampled dtau
                             // (Rao-Blackwellisation of the holding time; DESIGN.md f3)
+  int a_mode = 0;           // antisymmetric part of the drift (L567, L687-L692, future work L822): 0 = the paper's
+                            // diag(A_block): coordinate pairs (2i, 2i+1); 1 = pairs (4i, 4i+2), (4i+1, 4i+3): the two
+                            // 2-blocks of a group of four rotate into each other (Q24)
+  // Non-uniform regeneration density rho (L424-L430, L443-L445, future work L824; Q24): piecewise constant on a
+  // rho_grid x rho_grid tiling of the film coordinates (x0, x1), uniform in every other coordinate.  rho_w: tile
+  // probabilities, row-major (tile = ty * G + tx), summing to one, so rho = G^2 w[tile] and rho_lambda = 1.
+  uint32_t rho_grid = 0;
+  std::vector<double> rho_w;
 };
 
 template <class Real> struct Eval {
@@ -137,6 +145,34 @@ template <class Real> struct Chains {
       for (uint32_t c = 0; c < 4 && j + c < d; ++c) y[j + c] = u01_co<Real>(w[c]);
     }
   }
+
+  // ---- regeneration density rho (Q24) ----------------------------------------------------------------------------
+  std::vector<Real> rho_w, rho_cdf;   // tile probabilities and their running sums, in the chains' precision
+  void set_rho() {
+    rho_w.clear(); rho_cdf.clear();
+    Real acc = 0;
+    for (double w : cfg.rho_w) { rho_w.push_back((Real)w); acc = acc + (Real)w; rho_cdf.push_back(acc); }
+  }
+  // x ~ rho from a uniform point: the tile by inversion of the running sums with y0, uniform inside the tile
+  void regeneration_point(Real* y) const {
+    const uint32_t G = cfg.rho_grid;
+    if (!G) return;
+    const Real u0 = y[0], u1 = y[1];
+    uint32_t t = 0;
+    while (t + 1 < G * G && !(u0 < rho_cdf[t])) ++t;
+    const Real before = t ? rho_cdf[t - 1] : Real(0);
+    const Real frac = (u0 - before) / rho_w[t];
+    y[0] = wrap01<Real>((Real(t % G) + frac) / Real(G));
+    y[1] = wrap01<Real>((Real(t / G) + u1) / Real(G));
+  }
+  Real rho_at(const Real* xx) const {   // rho / rho_lambda at a state
+    const uint32_t G = cfg.rho_grid;
+    if (!G) return Real(1);
+    uint32_t tx = (uint32_t)std::floor(xx[0] * Real(G)), ty = (uint32_t)std::floor(xx[1] * Real(G));
+    if (tx > G - 1) tx = G - 1;
+    if (ty > G - 1) ty = G - 1;
+    return Real(G) * Real(G) * rho_w[ty * G + tx];
+  }
   void normals(uint32_t chain, uint32_t iter, Real* xi) const {
     for (uint32_t j = 0; j < d; j += 4) {
       uint32_t w[4];
@@ -164,7 +200,7 @@ template <class Real> struct Chains {
     const Real phat = p[i] + Real(kEps);
     Real weight = Real(1);
     if (restore) {
-      const Real kappa = kappa0 / phat;                       // L445, rho/rho_lambda == 1 (L452)
+      const Real kappa = rho_at(&x[(size_t)i * d]) * kappa0 / phat;   // L445: (rho / rho_lambda) kappa0 / p_hat; uniform rho: 1 (L452)
       const Real dt1 = -std::log(u01_oc<Real>(w[2])) / lambda; // L511
       const Real dt2 = -std::log(u01_oc<Real>(w[3])) / kappa;  // L512
       if (dt1 < dt2) { weight = dt1; killed[i] = 0; }          // L513-L515
@@ -184,7 +220,7 @@ template <class Real> struct Chains {
     if (cfg.p_lambda_override > 0) p_lambda = (Real)cfg.p_lambda_override;
     else {
       double s = 0;
-      for (uint32_t i = 0; i < N; ++i) s += (double)p[i];
+      for (uint32_t i = 0; i < N; ++i) s += (double)(p[i] / rho_at(&x[(size_t)i * d]));   // init states are rho-distributed
       p_lambda = (Real)(s / (double)N + kEps);                 // normalisation of p_hat = p + eps
     }
     const Real dt_eff = cfg.method == DIFFUSION_RESTORE ? (Real)cfg.dt : Real(1);
@@ -195,6 +231,7 @@ template <class Real> struct Chains {
   // Alg. 1: x ~ nu (uniform, L687), evaluate, [bootstrap p_lambda, kappa0], Accumulate.
   void init(uint32_t frame) {
     epoch = frame; iteration = 0;
+    set_rho();
     std::fill(accum.begin(), accum.end(), 0.0);
     tours = mutations = rays = mh_accepts = nonfinite = 0; kills_last = 0;
     std::vector<uint32_t> nr(N); std::vector<uint8_t> nf(N);
@@ -203,6 +240,7 @@ template <class Real> struct Chains {
       const uint32_t i = (uint32_t)ii;
       std::vector<Real> y(d), gy(d);
       uniform_point(i, 0, REGEN_U, y.data());
+      regeneration_point(y.data());                            // x ~ nu = rho (Alg. 1)
       Eval<Real> e;
       evaluate<Real>(sc, y.data(), grad, e, gy.data());
       store(i, y.data(), e, gy.data());
@@ -250,6 +288,7 @@ template <class Real> struct Chains {
         if ((restore && killed[i]) || cfg.method == PATH_TRACING) {   // Alg. 2: re-initialise from nu; PT: always
           kind[i] = 1;
           uniform_point(i, n, REGEN_U, y);
+          if (restore) regeneration_point(y);
         } else if (!restore && u01_co<Real>(w[0]) < (Real)cfg.large_step_prob) {
           kind[i] = 2;                              // large step (plain MH only), L747
           uniform_point(i, n, LARGE_U, y);
@@ -257,7 +296,16 @@ template <class Real> struct Chains {
           kind[i] = 0;
           std::vector<Real> xi(d);
           normals(i, n, xi.data());
-          if (cfg.method == DIFFUSION_RESTORE) {    // Alg. 4
+          if (cfg.method == DIFFUSION_RESTORE && cfg.a_mode == 1) {   // another antisymmetric pattern (Q24): x_j += c~ (A~ g)_j
+            for (uint32_t b = 0; b < d; b += 4) {
+              const bool four = b + 3 < d;                             // a trailing 2-block keeps the paper's rotation
+              const uint32_t p0 = four ? b + 2 : b + 1, p1 = four ? b + 3 : b;
+              Real r[4] = {ct * gi[p0], four ? ct * gi[p1] : -(ct * gi[p1]), Real(0), Real(0)};
+              if (four) { r[2] = -(ct * gi[b]); r[3] = -(ct * gi[b + 1]); }
+              for (uint32_t c = 0; c < (four ? 4u : 2u); ++c)
+                y[b + c] = wrap01<Real>(((xi_[b + c] + h * gi[b + c]) + r[c]) + s * xi[b + c]);
+            }
+          } else if (cfg.method == DIFFUSION_RESTORE) {    // Alg. 4
             for (uint32_t b = 0; b < d; b += 2) {
               const Real r0 = ct * gi[b + 1], r1 = -(ct * gi[b]);     // rotate(v) = c~ (v2, -v1), L720
               y[b] = wrap01<Real>(((xi_[b] + h * gi[b]) + r0) + s * xi[b]);

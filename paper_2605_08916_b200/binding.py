@@ -26,6 +26,7 @@ EXPORTS = [
     "dr_trace_rays", "dr_eval_states", "dr_philox_blocks", "dr_rng_transforms", "dr_resolve_image_sharded",
     "dr_eval_work_stats", "dr_profile_enable", "dr_profile_read", "dr_chains_work_stats", "dr_eval_states_form",
     "dr_chains_set_eval_form", "dr_frame_floats", "dr_pack_frame", "dr_resolve_image_packed",
+    "dr_bias_field",
 ]
 PROF_NAMES = ["propose", "raygen", "trace", "shade", "grad", "decide", "scan", "scatter", "resolve"]
 
@@ -103,6 +104,7 @@ def _load():
     L.dr_frame_floats.argtypes = [vp]
     L.dr_pack_frame.argtypes = [vp, vp, vp]
     L.dr_resolve_image_packed.argtypes = [vp, vp, vp, vp]
+    L.dr_bias_field.argtypes = [vp, C.c_double, C.c_double, C.c_double, u32, u32, vp, vp]
     L.dr_resolve_image_sharded.argtypes = [vp, vp, u64, u64, vp, vp]
     L.dr_eval_work_stats.argtypes = [vp, vp, u32, vp, vp]
     L.dr_profile_enable.argtypes = [vp, i32, vp]
@@ -191,6 +193,11 @@ class Scene:
         prim = torch.empty(n, dtype=torch.int32, device="cuda")
         _check(lib.dr_trace_rays(self.h, _dp(o.contiguous()), _dp(d.contiguous()), n, _dp(t), _dp(prim), _stream()))
         return t, prim
+
+    def bias_field(self, stddev, c_tilde, dt, G=64, M=256) -> torch.Tensor:
+        out = torch.empty(G, G, dtype=torch.float64, device="cuda")
+        _check(lib.dr_bias_field(self.h, float(stddev), float(c_tilde), float(dt), int(G), int(M), _dp(out), _stream()))
+        return out
 
     def eval_work_stats(self, x: torch.Tensor) -> dict:
         out = torch.zeros(3, dtype=torch.int64, device="cuda")

@@ -816,6 +816,20 @@ dr_status dr_eval_work_stats(const dr_scene* sc, const float* x, uint32_t n, uin
   return eval_rows(sc, x, n, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, (unsigned long long*)dev_out3, 0, (cudaStream_t)stream);
 }
 
+dr_status dr_bias_field(const dr_scene* sc, double stddev, double c_tilde, double dt, uint32_t G, uint32_t M, double* dev_out, void* stream) {
+  if (!sc || !dev_out) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (!sc->dev.analytic) return fail(DR_ERR_UNSUPPORTED, "the bias field is defined on the 2-D analytic target");
+  if (!(stddev > 0.0) || !(dt > 0.0) || !std::isfinite(c_tilde) || G < 1 || M < 1 || M > 4096) return fail(DR_ERR_INVALID_ARG, "stddev, dt > 0; 1 <= M <= 4096");
+  cudaStream_t s = (cudaStream_t)stream;
+  DevBuf tab;
+  CUDA_TRY(tab.alloc(3 * sizeof(double) * (size_t)M * M));
+  k_bias_table<<<(M * M + 255) / 256, 256, 0, s>>>(sc->dev, stddev, c_tilde, M, tab.as<double>());
+  k_bias_field<<<G * G, 256, 0, s>>>(sc->dev, stddev, dt, G, M, tab.as<double>(), dev_out);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaStreamSynchronize(s));   // the table is freed on return
+  return DR_OK;
+}
+
 dr_status dr_philox_blocks(uint64_t seed, const uint32_t* ctr, uint32_t n, uint32_t* out, void* stream) {
   if (!ctr || !out) return fail(DR_ERR_INVALID_ARG, "null argument");
   if (!n) return DR_OK;

@@ -336,6 +336,73 @@ __global__ void __launch_bounds__(kBlock) k_pack_frame(const Counters* c, const 
   }
 }
 
+// ---- Appendix C: bias field (L^* p_hat / p_hat) of the Alg. 4 dynamics on the 2-D analytic target ------
+// b(y) = lambda (integral p(x) k(x, y) dx - p(y)) / p(y), lambda = 1 / dt, k = wrapped Gaussian of width s around
+// m(x) = x + (s^2/2) g(x) + c~ (g2, -g1)(x).  Midpoint rule on M x M points; in double: the difference cancels to ~dt.
+__device__ __forceinline__ void analytic_f64(const DevScene& sc, double x0, double x1, double& p, double& g0, double& g1) {
+  double gx = 0.0, gy = 0.0;
+  p = 0.0;
+  for (int k = 0; k < sc.n_mix; ++k) {
+    const double s = sc.mix_s[k], inv = 1.0 / s, norm = 0.3989422804014326779 * inv;
+    double w[2], dw[2];
+    const double dl[2] = {x0 - sc.mix_mx[k], x1 - sc.mix_my[k]};
+    for (int a = 0; a < 2; ++a) {
+      const double dm = dl[a] - floor(dl[a] + 0.5);
+      w[a] = 0.0; dw[a] = 0.0;
+      for (int j = -2; j <= 2; ++j) {
+        const double z = (dm + (double)j) * inv, e = norm * exp(-0.5 * z * z);
+        w[a] += e; dw[a] += -z * inv * e;
+      }
+    }
+    p += sc.mix_w[k] * w[0] * w[1];
+    gx += sc.mix_w[k] * dw[0] * w[1];
+    gy += sc.mix_w[k] * w[0] * dw[1];
+  }
+  g0 = gx / (p + 1e-8);
+  g1 = gy / (p + 1e-8);
+}
+__global__ void k_bias_table(DevScene sc, double s, double c_tilde, uint32_t M, double* tab) {   // tab: p | m0 | m1, M * M each
+  const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= M * M) return;
+  const double x0 = ((double)(k % M) + 0.5) / (double)M, x1 = ((double)(k / M) + 0.5) / (double)M;
+  double p, g0, g1;
+  analytic_f64(sc, x0, x1, p, g0, g1);
+  const double h = 0.5 * s * s;
+  tab[k] = p;
+  tab[(size_t)M * M + k] = x0 + h * g0 + c_tilde * g1;
+  tab[2 * (size_t)M * M + k] = x1 + h * g1 - c_tilde * g0;
+}
+__global__ void __launch_bounds__(256) k_bias_field(DevScene sc, double s, double dt, uint32_t G, uint32_t M, const double* tab, double* out) {
+  __shared__ double sm[256];
+  const uint32_t c = blockIdx.x;
+  const double y0 = ((double)(c % G) + 0.5) / (double)G, y1 = ((double)(c / G) + 0.5) / (double)G;
+  const double norm = 0.3989422804014326779 / s;
+  const size_t MM = (size_t)M * M;
+  double acc = 0.0;
+  for (size_t k = threadIdx.x; k < MM; k += 256) {
+    double d0 = y0 - tab[MM + k], d1 = y1 - tab[2 * MM + k];
+    d0 -= floor(d0 + 0.5); d1 -= floor(d1 + 0.5);
+    double w0 = 0.0, w1 = 0.0;
+    for (int j = -1; j <= 1; ++j) {
+      const double z0 = (d0 + (double)j) / s, z1 = (d1 + (double)j) / s;
+      w0 += norm * exp(-0.5 * z0 * z0);
+      w1 += norm * exp(-0.5 * z1 * z1);
+    }
+    acc += tab[k] * w0 * w1;
+  }
+  sm[threadIdx.x] = acc;
+  __syncthreads();
+  for (int st = 128; st > 0; st >>= 1) {
+    if ((int)threadIdx.x < st) sm[threadIdx.x] += sm[threadIdx.x + st];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    double p, g0, g1;
+    analytic_f64(sc, y0, y1, p, g0, g1);
+    out[c] = (1.0 / dt) * (sm[0] / (double)MM - p) / p;
+  }
+}
+
 // ---- test hooks -------------------------------------------------------------------------------------------
 // dr_trace_rays: user rays -> queue planes (o, d), and hits -> (t, original triangle id).
 __global__ void k_pack_rays(const float* o, const float* d, uint32_t n, float4* q, uint32_t cap, uint32_t* cnt) {

@@ -678,3 +678,18 @@ def test_small_run_under_the_checked_build(dr, tmp_path):
         r = subprocess.run([sys.executable, os.path.join(root, "tests", "sanitizer", "small_run.py")], env=dict(os.environ, DR_LIB=lib),
                            capture_output=True, text=True, timeout=900)
         assert r.returncode == 0 and "small_run ok" in r.stdout, r.stdout + r.stderr
+
+
+def test_bias_field_matches_oracle(dr, oracle, torch_):
+    """Appendix C: the bias field L^* p_hat / p_hat of the Alg. 4 dynamics on the analytic target,
+    dr_bias_field against the oracle's quadrature (both in double), at the paper's dt = 1e-5 and at a coarse one."""
+    desc = S.mixture3()
+    gsc, osc = dr.Scene(desc), oracle.Scene(desc, oracle.F64)
+    for sigma, dt in ((0.5, 1e-5), (0.5, 1e-3), (2.0, 1e-4)):
+        s, ct = sigma * np.sqrt(dt), 0.5 * sigma * sigma * dt
+        g = gsc.bias_field(s, ct, dt, G=24, M=256).cpu().numpy()
+        o = osc.bias_field(s, ct, dt, G=24, M=256)
+        # single-precision mixture parameters on the device side, double arithmetic on both: agreement to rounding of the sums
+        assert np.abs(g - o).max() <= 1e-6 * np.abs(o).max() + 1e-7 / dt * 1e-2, (sigma, dt, np.abs(g - o).max(), np.abs(o).max())
+    with pytest.raises(dr.DrError):
+        dr.Scene(S.furnace()).bias_field(0.01, 0.0, 1e-3)

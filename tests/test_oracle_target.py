@@ -223,3 +223,36 @@ def test_analytic_target(oracle):
         fd = (np.log(sc.eval(xp[None], False)["p"][0] + 1e-8) - np.log(sc.eval(xm[None], False)["p"][0] + 1e-8)) / (2 * h)
         assert np.isclose(got["g"][0, k], fd, rtol=1e-6)
     assert np.isclose(sc.eval(np.array([[0.0, 0.3]]), False)["p"][0], sc.eval(np.array([[1 - 1e-15, 0.3]]), False)["p"][0], rtol=1e-9)
+
+
+def test_bias_field_closed_form_single_gaussian(oracle):
+    """Appendix C: b = L^* p / p for the Alg. 4 dynamics.  For one isotropic Gaussian mode of width tau
+    the Euler-Maruyama step is linear, x' - mu = A (x - mu) + s xi with A = (1 - s^2 / (2 tau^2)) I + (c~ / tau^2) J, so the
+    pushed-forward density is Gaussian with variance v' = tau^2 ((1 - a)^2 + b^2) + s^2 and
+    b(y) = (N(y; mu, v') / N(y; mu, tau^2) - 1) / dt in closed form.  Also: the integral of L^* p vanishes, and at fixed
+    sigma (s^2 = sigma^2 dt) the field shrinks with dt (the vanishing bias the appendix shows)."""
+    tau = 0.05
+    sc = oracle.Scene(S.single_mode(s=tau), oracle.F64)
+    G = 32
+    c = (np.arange(G) + 0.5) / G
+    X, Y = np.meshgrid(c, c)
+    r2 = (X - 0.5) ** 2 + (Y - 0.5) ** 2
+    N = lambda r2, var: np.exp(-r2 / (2 * var)) / (2 * np.pi * var)
+    near = r2 < (3 * tau) ** 2
+    for s, ct, dt in ((0.01, 2e-5, 1e-2), (0.005, 0.0, 1e-3), (0.02, -1e-4, 1.0)):
+        b = sc.bias_field(s, ct, dt, G=G, M=512)
+        a, bb = s * s / (2 * tau * tau), ct / (tau * tau)
+        v = tau * tau * ((1 - a) ** 2 + bb * bb) + s * s
+        want = (N(r2, v) / N(r2, tau * tau) - 1) / dt
+        assert np.abs(b - want)[near].max() <= 1e-5 * np.abs(want[near]).max() + 1e-9, (s, ct, dt)
+        p = sc.eval(np.stack([X.ravel(), Y.ravel()], 1), False)["p"].reshape(G, G)
+        assert abs((b * p).mean()) < 1e-6 * np.abs(b * p).max() * G                # mass is conserved: integral of L^* p = 0
+    # separated modes (the appendix' left panel): the field shrinks like dt at fixed sigma
+    sc3 = oracle.Scene(S.mixture3(), oracle.F64)
+    sigma = 0.5
+    c = (np.arange(24) + 0.5) / 24
+    X, Y = np.meshgrid(c, c)
+    p3 = sc3.eval(np.stack([X.ravel(), Y.ravel()], 1), False)["p"].reshape(24, 24)
+    bulk = p3 > 0.05 * p3.max()                                                     # away from the tails, where 1 / p explodes
+    m = [np.abs(sc3.bias_field(sigma * np.sqrt(dt), 0.5 * sigma ** 2 * dt, dt, G=24, M=384))[bulk].max() for dt in (4e-4, 1e-4)]
+    assert 3.0 < m[0] / m[1] < 5.0, m
