@@ -74,10 +74,18 @@ def local_kernel(method, pts, p, g, s, ct):
     return P
 
 
-def expected_run(method, pts, p, g, pix, s, ct, m, dt, lsp, p_lambda):
+def tile_density(pts, rho):
+    """rho / rho_lambda at the grid points for tile probabilities `rho` (R x R, row = x1 tile): R^2 w[tile]."""
+    R = rho.shape[0]
+    tx, ty = np.minimum((pts[:, 0] * R).astype(int), R - 1), np.minimum((pts[:, 1] * R).astype(int), R - 1)
+    return R * R * rho[ty, tx]
+
+
+def expected_run(method, pts, p, g, pix, s, ct, m, dt, lsp, p_lambda, rho=None):
     n = len(pts)
     ph = p + EPS
-    nu = np.full(n, 1.0 / n)
+    dens = np.ones(n) if rho is None else tile_density(pts, rho)
+    nu = dens / n                                  # regeneration law on the grid (f4: density rho, else uniform)
     P = local_kernel(method, pts, p, g, s, ct)
     restore = method.endswith("restore")
     fop = p / ph                                  # f = (p, p, p)
@@ -87,7 +95,7 @@ def expected_run(method, pts, p, g, pix, s, ct, m, dt, lsp, p_lambda):
     if restore:
         dt_eff = dt if method == "diffusion_restore" else 1.0
         lam = 1.0 / dt_eff                        # PAPER.md L659 / L737
-        kappa = (p_lambda / (m * dt_eff)) / ph    # L752, L445
+        kappa = dens * (p_lambda / (m * dt_eff)) / ph    # L752, L445: (rho / rho_lambda) kappa0 / p_hat
         kill = kappa / (lam + kappa)
         hold = 1.0 / (lam + kappa)                # E[min(Exp(lam), Exp(kappa))]
         for _ in range(T + 1):
@@ -146,6 +154,86 @@ def test_finite_state_brute_force(oracle, method, rb):
     if method.endswith("restore"):
         t_se = tours.std(ddof=1) / np.sqrt(seeds)
         assert abs(tours.mean() - want_tours) < 5 * t_se + 5e-4 * want_tours, (method, tours.mean(), want_tours)
+
+
+def test_nonuniform_regeneration_density(oracle):
+    """f4: regeneration from a density rho that is piecewise constant on film tiles, killing
+    rate (rho / rho_lambda) kappa0 / p_hat.  (i) In the finite-state model the tour estimator stays exact for a reversible
+    kernel: kappa0 nu.h = integral of f with nu = rho; (ii) the model's exact expectations after T iterations pin the oracle's
+    runs with a strongly non-uniform rho; (iii) the init states follow rho."""
+    sc, pts, p, g, pix = grid_model(oracle)
+    rng = np.random.default_rng(8)
+    rho = rng.uniform(0.2, 3.0, size=(4, 4))
+    rho /= rho.sum()
+    rho = rho.astype(np.float32).astype(np.float64)
+    ph, n = p + EPS, len(p)
+    dens = tile_density(pts, rho)
+    nu = dens / n
+    P = local_kernel("metropolis_restore", pts, p, g, 0.1, 0.0)
+    lam, m = 1.0, 5.0
+    kappa0 = ph.mean() * lam / m
+    A = np.diag(lam + dens * kappa0 / ph) - lam * P
+    assert np.isclose(kappa0 * (nu @ np.linalg.solve(A, p / ph)), p.mean(), rtol=1e-9)        # (i)
+    p_lambda = 1.0 + EPS
+    for method in ("metropolis_restore", "diffusion_restore"):
+        kw = dict(PARAMS[method])
+        want_acc, want_tours = expected_run(method, pts, p, g, pix, kw["stddev"], kw.get("c_tilde", 0.0), kw["m"], kw.get("dt", 1e-5),
+                                            0.0, p_lambda, rho=rho)
+        base_acc, _ = expected_run(method, pts, p, g, pix, kw["stddev"], kw.get("c_tilde", 0.0), kw["m"], kw.get("dt", 1e-5), 0.0, p_lambda)
+        assert np.abs(want_acc - base_acc).max() > 0.05 * base_acc.max()                         # rho matters at T = 10
+        seeds, N = 8, 30000
+        accs, tours = [], []
+        for seed in range(seeds):
+            ch = oracle.Chains(sc, method, N, seed=500 + seed, p_lambda_override=p_lambda, rho=rho, **kw)
+            ch.init(0)
+            if seed == 0:                                                                         # (iii)
+                x = ch.state()["x"]
+                hist = np.histogram2d(x[:, 1], x[:, 0], bins=4, range=[[0, 1], [0, 1]])[0] / N
+                assert np.abs(hist - rho).max() < 5 * np.sqrt(rho.max() / N)
+            ch.step(T)
+            accs.append(ch.accum()[:, 0] / N)
+            tours.append(ch.stats()["tours"] / N)
+        accs, tours = np.array(accs), np.array(tours)
+        mean, se = accs.mean(0), accs.std(0, ddof=1) / np.sqrt(seeds)
+        z = np.abs(mean - want_acc) / (se + 2e-3 * want_acc)
+        assert z.max() < 5.0, (method, z.max())
+        t_se = tours.std(ddof=1) / np.sqrt(seeds)
+        assert abs(tours.mean() - want_tours) < 5 * t_se + 5e-4 * want_tours, (method, tours.mean(), want_tours)
+
+
+def test_second_antisymmetric_pattern(oracle):
+    """f4: the drift's antisymmetric part, read off the oracle by teacher forcing.  A state with a
+    chosen score g is set, Diffusion Restore takes one step (always accepted), and y - x - (s^2/2) g - s xi = c~ A~ g with xi
+    recomputed from the chain's Philox stream.  a_mode 0 is the paper's diag(A_block) (rotate(v) = c~ (v2, -v1), L720);
+    a_mode 1 couples coordinates (4i, 4i+2) and (4i+1, 4i+3); both are antisymmetric (g . A~ g = 0, A~^T = -A~)."""
+    desc = S.furnace()                                        # d = 8
+    sc = oracle.Scene(desc, oracle.F64)
+    d, N, s, ct = desc.dim, 64, 1e-3, 0.25
+    want = {0: np.kron(np.eye(4), np.array([[0.0, 1.0], [-1.0, 0.0]])),
+            1: np.kron(np.eye(2), np.array([[0, 0, 1, 0], [0, 0, 0, 1], [-1, 0, 0, 0], [0, -1, 0, 0]], dtype=float))}
+    for mode in (0, 1):
+        ch = oracle.Chains(sc, "diffusion_restore", N, seed=3, stddev=s, c_tilde=ct, a_mode=mode)
+        ch.init(0)
+        st = ch.state()
+        rng = np.random.default_rng(1)
+        st["x"] = rng.uniform(0.3, 0.7, size=(N, d))
+        st["g"] = np.zeros((N, d))
+        st["g"][:d] = np.eye(d) * 0.1                         # chains 0..d-1 probe the columns of A~
+        st["g"][d:] = rng.normal(size=(N - d, d)) * 0.1
+        st["killed"][:] = 0
+        ch.set_state(st, 5)
+        ch.step(1)
+        y = ch.state()["x"]
+        xi = np.zeros((N, d))
+        for i in range(N):
+            for j in range(d // 4):
+                w = oracle.stream_block(3, i, 6, j, 1, 0)    # purpose 1 = PROP_N, iteration 6
+                xi[i, 4 * j:4 * j + 2] = oracle.rng_transforms(int(w[0]), int(w[1]), oracle.F64)[2:]
+                xi[i, 4 * j + 2:4 * j + 4] = oracle.rng_transforms(int(w[2]), int(w[3]), oracle.F64)[2:]
+        Ag = (y - st["x"] - 0.5 * s * s * st["g"] - s * xi) / ct
+        assert np.allclose(Ag, st["g"] @ want[mode].T, atol=1e-12)
+        assert np.allclose(want[mode].T, -want[mode]) and np.abs(np.sum(Ag * st["g"], axis=1)).max() < 1e-12
+    assert not np.allclose(want[0], want[1])
 
 
 def test_rao_blackwell_weight_is_the_expected_holding_time(oracle):
