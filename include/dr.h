@@ -101,6 +101,12 @@ typedef struct {
                                 over several GPUs draws the same numbers as the unsharded run */
   uint32_t rao_blackwell;    /* Restore variants, 0 / 1: accumulate E[dtau | x] = 1 / (lambda + kappa) instead of the sampled
                                 dtau (Rao-Blackwellised holding time); the kill decision stays the race */
+  uint32_t a_mode;           /* antisymmetric part of the Langevin drift (future work L822): 0 = the paper's
+                                diag(A_block), coordinate pairs (2i, 2i+1); 1 = pairs (4i, 4i+2) and (4i+1, 4i+3) (Q24) */
+  uint32_t rho_grid;         /* regeneration density rho (future work L824): 0 = uniform; G in 1..64:
+                                piecewise constant on a G x G tiling of the film coordinates (x0, x1), uniform in the others;
+                                the killing rate becomes (rho / rho_lambda) kappa0 / p_hat */
+  const float* host_rho;     /* G*G tile probabilities, row-major (tile = ty * G + tx), > 0, summing to one (copied) */
 } dr_config;
 
 typedef struct {

@@ -52,7 +52,8 @@ class dr_analytic2d_desc(C.Structure):
 class dr_config(C.Structure):
     _fields_ = [("method", C.c_int32), ("n_chains", C.c_uint32), ("stddev", C.c_float), ("c_tilde", C.c_float),
                 ("dt", C.c_float), ("m", C.c_float), ("large_step_prob", C.c_float), ("p_lambda_override", C.c_float),
-                ("seed", C.c_uint64), ("chain_offset", C.c_uint32), ("rao_blackwell", C.c_uint32)]
+                ("seed", C.c_uint64), ("chain_offset", C.c_uint32), ("rao_blackwell", C.c_uint32), ("a_mode", C.c_uint32),
+                ("rho_grid", C.c_uint32), ("host_rho", C.c_void_p)]
 
 
 class dr_stats(C.Structure):
@@ -223,7 +224,7 @@ class Chains:
     """dr_chains_create over caller-owned torch memory + the per-frame calls."""
 
     def __init__(self, scene: Scene, method, n_chains, stddev=None, c_tilde=None, dt=1e-5, m=64.0, large_step_prob=None,
-                 p_lambda_override=0.0, seed=0, chain_offset=0, rao_blackwell=False):
+                 p_lambda_override=0.0, seed=0, chain_offset=0, rao_blackwell=False, a_mode=0, rho=None):
         method = METHODS[method] if isinstance(method, str) else int(method)
         if stddev is None:
             stddev = 1e-2 if method in (0, 2) else 5e-3        # PAPER.md L747
@@ -232,8 +233,10 @@ class Chains:
         if large_step_prob is None:
             large_step_prob = 0.3 if method in (0, 1) else 0.0
         self.scene, self.method, self.N, self.d = scene, method, int(n_chains), scene.dim
+        rho_arr = None if rho is None else np.ascontiguousarray(rho, dtype=np.float32).ravel()
+        grid = 0 if rho is None else int(round(np.sqrt(rho_arr.size)))
         self.cfg = dr_config(method, self.N, stddev, c_tilde, dt, m, large_step_prob, p_lambda_override, seed, chain_offset,
-                             int(bool(rao_blackwell)))
+                             int(bool(rao_blackwell)), int(a_mode), grid, None if rho is None else _np(rho_arr))
         nbytes = lib.dr_chains_state_bytes(scene.h, C.byref(self.cfg))
         if nbytes == 0:
             raise DrError(DR_ERR_INVALID_ARG, lib.dr_last_error().decode())

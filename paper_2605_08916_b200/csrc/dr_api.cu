@@ -81,7 +81,8 @@ struct dr_chains {
   uint32_t eval_tag = 0;           // k_wave: tag of the last evaluation (dr_wave.cuh)
   int eval_form = 0;               // test hook dr_chains_set_eval_form: 0 = default choice, 1 = per-segment loop, 2 = k_wave
   void* hook_scratch = nullptr;    // device staging of dr_chains_download / _upload (row-major copies), allocated on first use
-  ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); cudaFree(hook_scratch); }
+  void* d_rho = nullptr;           // f4: (probability, running sum) per film tile
+  ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); cudaFree(hook_scratch); cudaFree(d_rho); }
 };
 
 namespace {
@@ -131,6 +132,18 @@ dr_status check_config(const dr_config* c) {
   if (!c) return fail(DR_ERR_INVALID_ARG, "config is null");
   if (c->method < 0 || c->method > DR_PATH_TRACING) return fail(DR_ERR_INVALID_ARG, "method out of range");
   if (c->rao_blackwell > 1) return fail(DR_ERR_INVALID_ARG, "rao_blackwell must be 0 or 1");
+  if (c->a_mode > 1) return fail(DR_ERR_INVALID_ARG, "a_mode must be 0 or 1");
+  if (c->rho_grid > 64) return fail(DR_ERR_INVALID_ARG, "rho_grid must be <= 64");
+  if (c->rho_grid) {
+    if (!c->host_rho) return fail(DR_ERR_INVALID_ARG, "rho_grid > 0 needs host_rho");
+    double sum = 0.0;
+    for (uint32_t t = 0; t < c->rho_grid * c->rho_grid; ++t) {
+      if (!std::isfinite(c->host_rho[t])) return fail(DR_ERR_NONFINITE, "non-finite tile probability");
+      if (!(c->host_rho[t] > 0.f)) return fail(DR_ERR_INVALID_ARG, "tile probabilities must be > 0");
+      sum += c->host_rho[t];
+    }
+    if (std::fabs(sum - 1.0) > 1e-4) return fail(DR_ERR_INVALID_ARG, "tile probabilities must sum to one");
+  }
   if (c->n_chains < 1) return fail(DR_ERR_INVALID_ARG, "n_chains must be >= 1");
   if (!(c->stddev > 0.f) || !std::isfinite(c->stddev)) return fail(DR_ERR_INVALID_ARG, "stddev must be > 0");
   if (!(c->c_tilde >= 0.f) || !std::isfinite(c->c_tilde)) return fail(DR_ERR_INVALID_ARG, "c_tilde must be >= 0");
@@ -504,6 +517,17 @@ dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_stat
   ChainParams& cp = h->cp;
   cp.method = c->method; cp.restore = c->method >= DR_METROPOLIS_RESTORE && c->method <= DR_DIFFUSION_RESTORE; cp.grad = grad;
   cp.rao_blackwell = cp.restore && c->rao_blackwell;
+  cp.a_mode = (int)c->a_mode; cp.rho_grid = c->rho_grid; cp.rho = nullptr;
+  if (c->rho_grid) {   // running sums in fp32, in tile order (what the regeneration inverts)
+    std::vector<float> t2(2 * (size_t)c->rho_grid * c->rho_grid);
+    float acc = 0.f;
+    for (uint32_t t = 0; t < c->rho_grid * c->rho_grid; ++t) { acc = acc + c->host_rho[t]; t2[2 * t] = c->host_rho[t]; t2[2 * t + 1] = acc; }
+    cudaError_t re = cudaMalloc(&h->d_rho, t2.size() * sizeof(float));
+    if (re == cudaSuccess) re = cudaMemcpy(h->d_rho, t2.data(), t2.size() * sizeof(float), cudaMemcpyHostToDevice);
+    if (re != cudaSuccess) { delete h; return fail(DR_ERR_CUDA, std::string("regeneration density: ") + cudaGetErrorString(re)); }
+    cp.rho = (const float2*)h->d_rho;
+    h->cfg.host_rho = nullptr;   // the caller's array is not kept
+  }
   cp.N = c->n_chains; cp.d = s->dev.d; cp.planes = s->dev.planes;
   cp.stddev = c->stddev; cp.half_s2 = 0.5f * c->stddev * c->stddev; cp.c_tilde = c->c_tilde; cp.dt = c->dt; cp.m = c->m;
   cp.large_step_prob = cp.restore ? 0.f : c->large_step_prob;

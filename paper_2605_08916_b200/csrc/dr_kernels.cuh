@@ -24,6 +24,9 @@ struct ChainParams {
   uint32_t N, d, planes;
   float stddev, half_s2, c_tilde, dt, m, large_step_prob, p_lambda_override;
   int rao_blackwell;     // f3: weight = 1 / (lambda + kappa)
+  int a_mode;            // f4: antisymmetric pattern of the drift
+  uint32_t rho_grid;     // f4: regeneration density on G x G film tiles (0: uniform)
+  const float2* rho;     //     (probability, running sum) per tile, row-major
   uint64_t seed;
   uint32_t epoch;
   uint32_t chain_offset;  // global id of chain 0 (RNG keying)
@@ -59,6 +62,26 @@ __device__ __forceinline__ float wrap01(float v) {
   return fminf(w, 0x1.fffffep-1f);  // DESIGN.md Q3
 }
 
+// f4: x ~ rho from a uniform point -- the tile by inversion of the running sums with u0, uniform inside the tile (Q24)
+__device__ __forceinline__ void regeneration_point(const ChainParams& cp, float& x0, float& x1) {
+  const uint32_t G = cp.rho_grid, n = G * G;
+  uint32_t lo = 0, hi = n - 1;                 // first tile t with x0 < cdf[t], else the last one
+  while (lo < hi) {
+    const uint32_t mid = (lo + hi) >> 1;
+    if (x0 < __ldg(&cp.rho[mid]).y) hi = mid; else lo = mid + 1;
+  }
+  const float before = lo ? __ldg(&cp.rho[lo - 1]).y : 0.f;
+  const float frac = (x0 - before) / __ldg(&cp.rho[lo]).x;
+  x0 = wrap01(((float)(lo % G) + frac) / (float)G);
+  x1 = wrap01(((float)(lo / G) + x1) / (float)G);
+}
+__device__ __forceinline__ float rho_at(const ChainParams& cp, float x0, float x1) {   // rho / rho_lambda
+  const uint32_t G = cp.rho_grid;
+  if (!G) return 1.0f;
+  const uint32_t tx = min((uint32_t)floorf(x0 * (float)G), G - 1u), ty = min((uint32_t)floorf(x1 * (float)G), G - 1u);
+  return (float)G * (float)G * __ldg(&cp.rho[ty * G + tx]).x;
+}
+
 __device__ __forceinline__ float4 mask_dims(float4 v, uint32_t plane, uint32_t d) {
   const uint32_t b = 4u * plane;
   if (b + 1 >= d) v.y = 0.f;
@@ -84,10 +107,17 @@ __global__ void __launch_bounds__(kBlock) k_propose(ChainParams cp, ChainState s
     float4 y;
     if (kind) {
       y = uniforms4(stream_block(cp.seed, cp.chain_offset + i, n, j, kind == 1 ? P_REGEN_U : P_LARGE_U, cp.epoch));
+      if (j == 0 && kind == 1 && cp.rho_grid && (init || cp.restore)) regeneration_point(cp, y.x, y.y);   // x ~ nu = rho (Alg. 1, Alg. 2)
     } else {
       const float4 xi = normals4(stream_block(cp.seed, cp.chain_offset + i, n, j, P_PROP_N, cp.epoch));
       const float4 x = st.x[at];
-      if (cp.method == 4) {  // Alg. 4: x += (s^2/2) g + c~ (g2, -g1) + s xi, per 2-block
+      if (cp.method == 4 && cp.a_mode == 1 && 4 * j + 3 < cp.d) {   // f4: the two 2-blocks of the plane rotate into each other
+        const float4 g = st.g[at];
+        y.x = wrap01(((x.x + h * g.x) + ct * g.z) + s * xi.x);
+        y.y = wrap01(((x.y + h * g.y) + ct * g.w) + s * xi.y);
+        y.z = wrap01(((x.z + h * g.z) - ct * g.x) + s * xi.z);
+        y.w = wrap01(((x.w + h * g.w) - ct * g.y) + s * xi.w);
+      } else if (cp.method == 4) {  // Alg. 4: x += (s^2/2) g + c~ (g2, -g1) + s xi, per 2-block
         const float4 g = st.g[at];
         y.x = wrap01(((x.x + h * g.x) + ct * g.y) + s * xi.x);
         y.y = wrap01(((x.y + h * g.y) - ct * g.x) + s * xi.y);
@@ -115,7 +145,12 @@ __global__ void __launch_bounds__(kBlock) k_propose(ChainParams cp, ChainState s
 __global__ void __launch_bounds__(kBlock) k_psum_partial(ChainParams cp, ChainState st) {
   __shared__ double sm[kBlock];
   const uint32_t i = blockIdx.x * kBlock + threadIdx.x;
-  sm[threadIdx.x] = i < cp.N ? (double)st.fy[i].w : 0.0;
+  double pi = 0.0;
+  if (i < cp.N) {
+    const float4 y0 = st.y[i];
+    pi = (double)(st.fy[i].w / rho_at(cp, y0.x, y0.y));   // the init states are rho-distributed (f4); uniform rho: / 1
+  }
+  sm[threadIdx.x] = pi;
   __syncthreads();
   for (int s = kBlock / 2; s > 0; s >>= 1) {
     if ((int)threadIdx.x < s) sm[threadIdx.x] += sm[threadIdx.x + s];
@@ -222,7 +257,9 @@ __global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st
     const float phat = cur.w + kEps;
     float wgt = 1.0f;
     if (cp.restore) {
-      const float kappa = c->kappa0 / phat;                   // L445
+      float rho = 1.0f;
+      if (cp.rho_grid) { const float4 x0 = st.x[i]; rho = rho_at(cp, x0.x, x0.y); }
+      const float kappa = rho * c->kappa0 / phat;             // L445: (rho / rho_lambda) kappa0 / p_hat
       const float dt1 = -logf(u01_oc(w.z)) / c->lambda;       // L511
       const float dt2 = -logf(u01_oc(w.w)) / kappa;           // L512
       killed = !(dt1 < dt2);                                  // L513 (tie -> killed)

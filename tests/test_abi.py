@@ -28,7 +28,7 @@ def test_binding_lists_the_same_names():
     assert sorted(binding.EXPORTS) == declared_symbols()
     # struct sizes match the C layout
     assert ctypes.sizeof(binding.dr_material) == 36
-    assert ctypes.sizeof(binding.dr_config) == 48
+    assert ctypes.sizeof(binding.dr_config) == 64
     assert ctypes.sizeof(binding.dr_stats) == 88
     assert ctypes.sizeof(binding.dr_scene_info) == 32
 

@@ -287,6 +287,24 @@ def test_teacher_forced_parity_pt_and_rao_blackwell(dr, oracle, torch_, variant,
     _teacher_forced(dr, oracle, torch_, variant[0], case, **variant[1])
 
 
+def _rho(grid, seed):
+    w = np.random.default_rng(seed).uniform(0.2, 3.0, size=(grid, grid))
+    return (w / w.sum()).astype(np.float32)
+
+
+F4 = [("diffusion_restore", dict(a_mode=1)), ("diffusion_restore", dict(rho=_rho(4, 1))), ("metropolis_restore", dict(rho=_rho(7, 2))),
+      ("mala_restore", dict(rho=_rho(3, 3), rao_blackwell=True)), ("diffusion_restore", dict(a_mode=1, rho=_rho(16, 4))), ("metropolis", dict(rho=_rho(5, 5)))]
+
+
+@pytest.mark.parametrize("variant", F4, ids=[f"{m}-{'-'.join(sorted(kw))}" for m, kw in F4])
+@pytest.mark.parametrize("case", [CASES[1], CASES[3], CASES_NEE[1]], ids=["mini_machines", "mixture3", "mini_machines_nee"])
+def test_teacher_forced_parity_f4(dr, oracle, torch_, variant, case):
+    """regeneration from a density rho on film tiles with the killing rate (rho / rho_lambda) kappa0 / p_hat
+    (PAPER.md L443-L445), and a second antisymmetric pattern of the Langevin drift (L567, L822); same protocol: bit-exact
+    regenerated states, decisions, queue, tourCount, buffer against the oracle."""
+    _teacher_forced(dr, oracle, torch_, variant[0], case, **variant[1])
+
+
 def test_sharded_chains_against_the_oracle(dr, oracle, torch_):
     """a shard (global chain ids 1000 .. 1999 of a 2000-chain run) against the oracle's shard with the same
     chain_offset, teacher-forced like everything else: the RNG streams are keyed by global chain id on both sides."""
@@ -443,7 +461,8 @@ def test_edge_cases(dr, torch_):
     # wrong method in dr_step, invalid configs
     with pytest.raises(dr.DrError):
         dr.binding._check(dr.lib.dr_step(ch.h, 0, 1, None))
-    for bad in (dict(stddev=0.0), dict(dt=-1.0), dict(m=0.0), dict(large_step_prob=1.5), dict(stddev=float("nan"))):
+    for bad in (dict(stddev=0.0), dict(dt=-1.0), dict(m=0.0), dict(large_step_prob=1.5), dict(stddev=float("nan")), dict(a_mode=2),
+                dict(rho=np.full((3, 3), 0.2, np.float32)), dict(rho=np.array([[0.5, 0.5], [0.0, 0.0]], np.float32))):
         with pytest.raises(dr.DrError):
             dr.Chains(gsc, "metropolis", 16, **bad)
     bad_desc = S.furnace()
