@@ -122,7 +122,7 @@ Layout make_layout(uint32_t N, uint32_t planes, uint32_t Lseg, bool grad, bool n
   L.ring = take(sizeof(uint2) * (size_t)N * (nee ? 2 * Lseg - 1 : Lseg));   // one entry per ray of an evaluation, never reused (dr_wave.cuh)
   L.rec = take(grad ? sizeof(float4) * (size_t)N * Lseg : 0);
   L.pinfo = take(grad ? 4 * (size_t)N : 0);
-  L.gradlist = take(grad ? 4 * (size_t)N : 0);
+  L.gradlist = take(grad ? 4 * (size_t)N * (nee ? 16 : 1) : 0);   // with next-event estimation: 16 bins by path length
   L.ctl = take(4 * kCtlWords);
   L.total = o;
   return L;
@@ -309,7 +309,7 @@ struct HookEval {
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o = align256(o + bytes); return at; };
     const size_t q = take(96 * N), hits = take(8 * N), ring = take(8 * wave_ring_entries(sc->dev, N)), rec = take(grad ? 16 * N * L : 0),
-                 pinfo = take(grad ? 4 * N : 0), gl = take(grad ? 4 * N : 0), ctl = take(4 * kCtlWords);
+                 pinfo = take(grad ? 4 * N : 0), gl = take(grad ? 4 * N * (sc->dev.nee ? 16 : 1) : 0), ctl = take(4 * kCtlWords);
     cudaError_t e = ws_mem.alloc(o);
     if (e == cudaSuccess) e = xpl.alloc(16 * N * sc->dev.planes);
     if (e == cudaSuccess) e = gpl.alloc(grad ? 16 * N * sc->dev.planes : 0);

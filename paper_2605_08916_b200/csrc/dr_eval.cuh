@@ -16,6 +16,9 @@
 
 namespace dr {
 
+#ifndef DR_STREAM_HINTS
+#define DR_STREAM_HINTS 1   // evict-first stores of the vertex record, streaming loads of x in the shading: k_wave 4.33 -> 4.30 ms
+#endif
 #ifndef DR_TRACE_BLOCK
 #define DR_TRACE_BLOCK 640
 #endif
@@ -51,7 +54,8 @@ constexpr uint32_t kMiss = 0xFFFFFFFFu;
 constexpr int kCtlCnt = 0;     // cnt[k], k = 1..L: rays of segment k
 constexpr int kCtlHead = 20;   // head[k]: fetch counter of k_trace for segment k
 constexpr int kCtlGrad = 40;   // states on the reverse-pass list
-constexpr int kCtlWords = 64;
+constexpr int kCtlGradBin = 64; // next-event estimation: states on the reverse-pass list by number of sampling vertices (16 bins)
+constexpr int kCtlWords = 96;
 
 // Workspace for up to `cap` states.  Two forms of the same evaluation use it (same results, state by state):
 //  * per-segment loop (k_trace / k_shade): ray queues qa, qb; an entry is three float4 in planes of `cap` entries,
@@ -65,7 +69,7 @@ struct EvalWs {
   uint2* ring;         // wave_ring_entries() ray entries, written once per evaluation, never reused      (k_wave)
   float4* rec;         // L * cap (score only): incoming direction and triangle of vertex k of state s at [k * cap + s]
   uint32_t* pinfo;     // cap (score only): refract mask | rays << 16 of the finished path
-  uint32_t* gradlist;  // cap (score only)
+  uint32_t* gradlist;  // cap (score only); 16 * cap with next-event estimation: bin b (paths with b sampling vertices) at [b * cap, ...)
   uint32_t* ctl;       // kCtlWords
   uint32_t cap;
   uint32_t tag;        // k_wave: tag of this evaluation, != 0; ring entries of earlier evaluations carry other tags
@@ -88,7 +92,11 @@ struct EvalIO {
 };
 
 __device__ __forceinline__ float2 x_pair(const EvalIO& io, uint32_t s, uint32_t k) {  // coordinates (2k, 2k+1)
+#if DR_STREAM_HINTS
+  const float4 q = __ldcs(&io.x[(size_t)(k >> 1) * io.stride + s]);
+#else
   const float4 q = io.x[(size_t)(k >> 1) * io.stride + s];
+#endif
   return (k & 1u) ? make_float2(q.z, q.w) : make_float2(q.x, q.y);
 }
 // the coordinates of vertex k: (u1, u2, v1, v2) = plane k with next-event estimation, else (u1, u2, 0, 0)
@@ -109,7 +117,7 @@ __device__ __forceinline__ void g_pair(const EvalIO& io, uint32_t s, uint32_t k,
 // WAVE: the ray goes into the state's record and ring entry t (dr_wave.cuh); otherwise into slot t of queue qa.
 constexpr int kCtlWaveReserve = 48, kCtlWaveHead = 50, kCtlWaveDone = 51;   // control words of k_wave
 constexpr uint32_t kRecWords = 6;    // float4 per state record of k_wave: ray (o | state, d | signature, T | masks),
-                                     // (pending emitter connection | density of the ray's direction), shadow ray (o | emitter id, d | lobe)
+                                     // (pending emitter connection | density of the ray's direction), shadow ray (o | emitter id, lobe << 28; d | distance to the sampled point)
 // queue entries an evaluation can need: a path makes at most L rays, and with next-event estimation one shadow ray per vertex
 __host__ __device__ inline size_t wave_ring_entries(const DevScene& sc, size_t cap) { return (sc.nee ? 2u * sc.L - 1u : sc.L) * cap; }
 template <bool WAVE>
@@ -360,7 +368,9 @@ struct ShadeOut {
   float4 n0, n1, n2;
   float pb_next;
   float3 sh_o, sh_d, cpend;
+  float sh_len;          // distance from sh_o to the sampled emitter point
   uint32_t light_id, lobe;
+  uint32_t nv;           // sampling vertices of a path that ended here (bin of the reverse-pass list)
   bool cont, shadow, want_grad;
 };
 
@@ -430,7 +440,11 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
     } else if (k < sc.L) {
       term = kTermNone;
       const float4 u = x_vertex(sc, io, s, k);
+#if DR_STREAM_HINTS
+      if (GRAD) __stcs(&ws.rec[(size_t)k * cap + s], make_float4(d.x, d.y, d.z, __uint_as_float(li)));   // written once, read by k_grad only: evict first
+#else
       if (GRAD) ws.rec[(size_t)k * cap + s] = make_float4(d.x, d.y, d.z, __uint_as_float(li));
+#endif
       const V3<float> ov{o.x, o.y, o.z}, dv{d.x, d.y, d.z};
       VertexOut<float> vo;
       V3<float> hit;
@@ -450,7 +464,9 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
         // (T fcos) (Le w_l / p_l): T here is the throughput BEFORE this vertex' direction sample
         out.cpend = make_float3((Q2.x * vo.fcos[0]) * vo.lw[0], (Q2.y * vo.fcos[1]) * vo.lw[1], (Q2.z * vo.fcos[2]) * vo.lw[2]);
         out.sh_o = make_float3(hit.x + fr.nf.x * sc.eps_ray, hit.y + fr.nf.y * sc.eps_ray, hit.z + fr.nf.z * sc.eps_ray);
-        out.sh_d = normalize3(make_float3(vo.y.x, vo.y.y, vo.y.z) - out.sh_o);   // towards the sampled point, from the offset origin
+        const float3 to_y = make_float3(vo.y.x, vo.y.y, vo.y.z) - out.sh_o;      // towards the sampled point, from the offset origin
+        out.sh_len = sqrtf(dot3(to_y, to_y));
+        out.sh_d = to_y * (1.0f / out.sh_len);                                    // == normalize3(to_y)
         done = false;
       } else {
         sig = fnv(sig, lobe);
@@ -467,6 +483,7 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
       term = kTermNone;   // length cap on a surface: nothing is added
     }
   }
+  out.nv = k - 1u;
   if (done) finish_path<NEE>(sc, ws, io, k, s, f0, f1, f2, sig, info, k - 1u, term, GRAD, out.want_grad, bad);
 }
 

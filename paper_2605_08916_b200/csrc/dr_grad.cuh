@@ -88,8 +88,14 @@ __global__ void __launch_bounds__(kGradBlock, DR_GRAD_MIN_BLOCKS) k_grad_nee(Dev
   const uint32_t idx = blockIdx.x * kGradBlock + threadIdx.x;
   if (idx == 0 && io.grad_ctr) atomicAdd(io.grad_ctr, (unsigned long long)ws.ctl[kCtlGrad]);
   if (idx >= ws.ctl[kCtlGrad]) return;
-  const uint32_t s = ws.gradlist[idx];
   const size_t cap = ws.cap;
+  uint32_t rem = idx, bin = 15;   // the list is binned by the number of sampling vertices; longest paths first
+  for (;; --bin) {
+    const uint32_t c = ws.ctl[kCtlGradBin + bin];
+    if (rem < c || bin == 0) break;
+    rem -= c;
+  }
+  const uint32_t s = ws.gradlist[(size_t)bin * cap + rem];
   const float4 fp = io.f[s];
   const float inv_phat = 1.0f / (fp.w + kEps);
   const float4 hdr = ws.rec[s];

@@ -85,7 +85,11 @@ __device__ __forceinline__ void st_release2(uint2* p, uint2 v) {
 }
 
 // ---- the trace warps ------------------------------------------------------------------------------------------------
-template <bool STATS>
+// NEE: shadow rays (payload bit 31) only ask whether the closest hit is the sampled emitter triangle.  They start with
+// t_max just behind the sampled point and stop at the first other triangle hit clearly in front of it (kShadowBand): the
+// closest hit is then not that emitter either way, so the visibility decision is the one of the full closest-hit query.
+constexpr float kShadowBand = 1e-3f;
+template <bool STATS, bool NEE>
 __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs& ws, uint32_t n, const uint4* smem, SmemStack& st,
                                                 SmemTriStack& tst, WaveShared* wsh, uint32_t* h_pay, uint32_t* h_t, uint32_t* h_li,
                                                 uint32_t one, unsigned long long* work) {
@@ -99,6 +103,8 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
   uint32_t ent = 0;                         // lane j < kFetchChunk: payload of entry claim + j once it is known
   int poll = 0;
   bool pend = false;                        // this lane holds a finished ray that is not in the block's ring yet
+  float sh_lim = -1.f;                      // NEE, shadow ray: an occluder closer than this ends the query (< 0: not a shadow ray)
+  uint32_t sh_id = 0;                       //      the emitter triangle it aims at
   const uint32_t ring_cap = wave_ring_entries(sc, ws.cap);
   for (;;) {
     // ---- finished rays -> the block's ring (reserve, wait for room, write, publish in reservation order)
@@ -167,6 +173,10 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
         trav_begin(L.s);
         L.tsp = 0;
         L.active = true;
+        if (NEE) {
+          sh_lim = -1.f;
+          if (pay >> 31) { L.r.t = d.w * (1.0f + kShadowBand); sh_lim = d.w * (1.0f - kShadowBand); sh_id = __float_as_uint(o.w) & 0x0FFFFFFFu; }
+        }
       }
       const unsigned got = __ballot_sync(kFull, mine);
       taken += __popc(got);
@@ -183,7 +193,13 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
     }
     // ---- lockstep traversal; a finished lane keeps its hit in L.r until the flush before the next refill
     do {
-      const bool done = trav_step<STATS>(sc, smem, st, tst, L, nn, nt);
+      bool done = trav_step<STATS>(sc, smem, st, tst, L, nn, nt);
+      if (NEE && L.active && !done && sh_lim >= 0.f && L.r.id != 0xFFFFFFFFu && L.r.id != sh_id && L.r.t < sh_lim) {
+        done = true;                                   // occluded: drop what is still requested or stacked
+        L.has_node = false;
+#pragma unroll
+        for (int it = 0; it < kTrisPerStep; ++it) L.tri[it].li = kMiss;
+      }
       pend = pend || done;
       L.active = L.active && !done;
       act = __ballot_sync(kFull, L.active);
@@ -243,7 +259,7 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
     const bool phase_b = (pay >> 31) != 0u;
     float4* rec = ws.qa + kRecWords * (size_t)s;
     bool want_grad = false, push = false;     // push: this lane publishes a queue entry (`entry`)
-    uint32_t entry = 0;
+    uint32_t entry = 0, grad_bin = 0;
     if (mine && !phase_b) {
       const float4 Q0 = __ldcg(rec), Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2);
       const float pb_prev = NEE ? __ldcg(rec + 3).w : -1.f;
@@ -254,21 +270,23 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
       ShadeOut so;
       shade_vertex<GRAD, NEE>(sc, ws, io, k, Q0, Q1, Q2, pb_prev, h, s, so, bad);
       want_grad = so.want_grad;
+      grad_bin = so.nv;
       if (so.cont || so.shadow) {
         __stcg(rec, so.n0); __stcg(rec + 1, so.n1); __stcg(rec + 2, so.n2);
         if (NEE) __stcg(rec + 3, make_float4(so.cpend.x, so.cpend.y, so.cpend.z, so.pb_next));
         push = true;
         entry = s | (k << kWaveKShift);                       // the next ray: segment k + 1, stored as k
         if (NEE && so.shadow) {
-          __stcg(rec + 4, make_float4(so.sh_o.x, so.sh_o.y, so.sh_o.z, __uint_as_float(so.light_id)));
-          __stcg(rec + 5, make_float4(so.sh_d.x, so.sh_d.y, so.sh_d.z, __uint_as_float(so.lobe)));
+          __stcg(rec + 4, make_float4(so.sh_o.x, so.sh_o.y, so.sh_o.z, __uint_as_float(so.light_id | (so.lobe << 28))));
+          __stcg(rec + 5, make_float4(so.sh_d.x, so.sh_d.y, so.sh_d.z, so.sh_len));
           entry = s | ((k - 1u) << kWaveKShift) | 0x80000000u;   // the shadow ray of vertex k
         }
       }
     } else if (NEE && mine) {
-      const float4 Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2), Q3 = __ldcg(rec + 3), S0 = __ldcg(rec + 4), S1 = __ldcg(rec + 5);
+      const float4 Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2), Q3 = __ldcg(rec + 3), S0 = __ldcg(rec + 4);
       if (io.nrays) __stcg(&io.nrays[s], __ldcg(&io.nrays[s]) + 1u);
-      const bool vis = h.y != kMiss && __float_as_uint(__ldg(&sc.tris[3 * h.y + 2].y)) == __float_as_uint(S0.w);
+      const uint32_t aim = __float_as_uint(S0.w);                      // emitter triangle | lobe << 28
+      const bool vis = h.y != kMiss && __float_as_uint(__ldg(&sc.tris[3 * h.y + 2].y)) == (aim & 0x0FFFFFFFu);
       uint32_t info = __float_as_uint(Q2.w);
       if (vis) {
         float4 acc = __ldcg(&io.f[s]);
@@ -276,9 +294,10 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
         __stcg(&io.f[s], acc);
         info |= 1u << (16u + k);
       }
-      const uint32_t sig = fnv(fnv(__float_as_uint(Q1.w), vis ? 7u : 6u), __float_as_uint(S1.w));
+      const uint32_t sig = fnv(fnv(__float_as_uint(Q1.w), vis ? 7u : 6u), aim >> 28);
       if (Q2.x == 0.f && Q2.y == 0.f && Q2.z == 0.f) {         // the direction sample had zero weight: the path ends here
         finish_path<NEE>(sc, ws, io, k, s, 0.f, 0.f, 0.f, sig, info, k, kTermNone, GRAD, want_grad, bad);
+        grad_bin = k;
       } else {
         __stcg(rec + 1, make_float4(Q1.x, Q1.y, Q1.z, __uint_as_float(sig)));
         __stcg(rec + 2, make_float4(Q2.x, Q2.y, Q2.z, __uint_as_float(info)));
@@ -286,13 +305,24 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
         entry = s | (k << kWaveKShift);
       }
     }
-    if (GRAD) {  // reverse-pass list: one atomic per warp
+    if (GRAD) {  // reverse-pass list: one atomic per warp (per bin of path length with next-event estimation: k_grad_nee's
+                 // threads then walk paths of equal length side by side)
       const unsigned gm = __ballot_sync(kFull, want_grad);
-      if (gm) {
+      if (gm && !NEE) {
         uint32_t base = 0;
         if (lane == 0) base = atomicAdd(&ws.ctl[kCtlGrad], (uint32_t)__popc(gm));
         base = __shfl_sync(kFull, base, 0);
         if (want_grad) ws.gradlist[base + __popc(gm & lt)] = s;
+      } else if (gm) {
+        if (lane == 0) atomicAdd(&ws.ctl[kCtlGrad], (uint32_t)__popc(gm));
+        if (want_grad) {
+          const unsigned peers = __match_any_sync(gm, grad_bin);
+          const unsigned leader = __ffs(peers) - 1u;
+          uint32_t base = 0;
+          if (lane == leader) base = atomicAdd(&ws.ctl[kCtlGradBin + grad_bin], (uint32_t)__popc(peers));
+          base = __shfl_sync(peers, base, leader);
+          ws.gradlist[(size_t)grad_bin * ws.cap + base + __popc(peers & lt)] = s;
+        }
       }
     }
     // ---- the queue entries of the paths that go on (release: the records above are visible before the entry)
@@ -340,7 +370,7 @@ __global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws,
   __syncthreads();
   const uint32_t one = *(volatile uint32_t*)&smem[0].x;  // dr_traverse.cuh qmagic
   if (threadIdx.x >= (unsigned)kWaveTraceThreads) wave_shade_loop<GRAD, NEE>(sc, ws, io, n, wsh, h_pay, h_t, h_li);
-  else wave_trace_loop<STATS>(sc, ws, n, smem, st, tst, wsh, h_pay, h_t, h_li, one, io.work);
+  else wave_trace_loop<STATS, NEE>(sc, ws, n, smem, st, tst, wsh, h_pay, h_t, h_li, one, io.work);
 }
 
 }  // namespace dr
