@@ -120,6 +120,8 @@ typedef struct {
   uint32_t iteration;        /* n of the last completed iteration (0 = init) */
   float p_lambda, kappa0, lambda;
   uint32_t no_tour_resolves; /* resolves since init that found tourCount == 0 and wrote a zero image */
+  uint32_t wave_timeouts;    /* evaluations ended by k_wave's watchdog (never, unless the queue protocol is broken): dr_chains_stats
+                                then returns DR_ERR_CUDA instead of letting a kernel spin on the GPU for ever */
   uint64_t grad_states;      /* evaluations that ran the reverse pass for the score (states with a non-zero score, a6) */
   uint64_t lit_init;         /* init states with p > 0: lit_init / N = fraction of uniform PSS samples that contribute */
 } dr_stats;

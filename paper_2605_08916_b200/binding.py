@@ -60,7 +60,7 @@ class dr_stats(C.Structure):
     _fields_ = [("tours", C.c_uint64), ("mutations", C.c_uint64), ("rays", C.c_uint64), ("mh_accepts", C.c_uint64),
                 ("nonfinite", C.c_uint64), ("kills_last_step", C.c_uint32), ("regen_queue_len", C.c_uint32),
                 ("iteration", C.c_uint32), ("p_lambda", C.c_float), ("kappa0", C.c_float), ("lambda_", C.c_float),
-                ("no_tour_resolves", C.c_uint32), ("grad_states", C.c_uint64), ("lit_init", C.c_uint64)]
+                ("no_tour_resolves", C.c_uint32), ("wave_timeouts", C.c_uint32), ("grad_states", C.c_uint64), ("lit_init", C.c_uint64)]
 
 
 class dr_scene_info(C.Structure):
@@ -179,7 +179,7 @@ class Scene:
         self.npix = desc.width * desc.height
 
     def __del__(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and lib is not None:      # (module globals are gone at interpreter shutdown)
             lib.dr_scene_destroy(self.h)
             self.h = None
 
@@ -248,7 +248,7 @@ class Chains:
         self.h = h
 
     def __del__(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and lib is not None:
             lib.dr_chains_destroy(self.h)
             self.h = None
 

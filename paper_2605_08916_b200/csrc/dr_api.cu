@@ -283,7 +283,7 @@ dr_status launch_iteration(dr_chains* c, uint32_t n, bool init, cudaStream_t s) 
     k_psum_partial<<<gb, kBlock, 0, s>>>(cp, c->st);
     k_bootstrap<<<1, kBlock, 0, s>>>(cp, c->st, gb);
   }
-  { ProfScope ps(c, DR_PROF_DECIDE, s); k_decide<<<gb, kBlock, 0, s>>>(cp, c->st, c->accum, n); }
+  { ProfScope ps(c, DR_PROF_DECIDE, s); k_decide<<<gb, kBlock, 0, s>>>(cp, c->st, c->accum, n, c->ws.ctl); }
   if (cp.restore) {
     { ProfScope ps(c, DR_PROF_SCAN, s); k_scan<<<1, 1024, 0, s>>>(c->st, gb); }
     { ProfScope ps(c, DR_PROF_SCATTER, s); k_scatter<<<gb, kBlock, 0, s>>>(cp, c->st); }
@@ -672,7 +672,8 @@ dr_status dr_chains_stats(dr_chains* c, dr_stats* o, void* stream) {
   o->tours = h.tours; o->mutations = h.mutations; o->rays = h.rays; o->mh_accepts = h.mh_accepts; o->nonfinite = h.nonfinite;
   o->kills_last_step = h.kills_last; o->regen_queue_len = h.queue_len; o->iteration = c->iteration;
   o->p_lambda = h.p_lambda; o->kappa0 = h.kappa0; o->lambda = h.lambda; o->no_tour_resolves = h.no_tour_resolves;
-  o->grad_states = h.grad_states; o->lit_init = h.lit_init;
+  o->grad_states = h.grad_states; o->lit_init = h.lit_init; o->wave_timeouts = h.wave_timeouts;
+  if (h.wave_timeouts) return fail(DR_ERR_CUDA, "k_wave's watchdog ended an evaluation: results since dr_chains_init are invalid");
   if (h.no_tour_resolves) { g_err = "a resolve ran before any tour had completed: zero image"; return DR_WARN_NO_TOURS; }
   return DR_OK;
 }

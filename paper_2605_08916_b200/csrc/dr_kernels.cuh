@@ -14,6 +14,7 @@ constexpr int kBlock = 256;      // streaming kernels
 struct Counters {
   unsigned long long tours, mutations, rays, mh_accepts, nonfinite, grad_states, lit_init;
   uint32_t kills_last, queue_len, iteration, no_tour_resolves;
+  uint32_t wave_timeouts, pad3[3];
   float p_lambda, kappa0, lambda, pad2;
   double psum;
 };
@@ -206,7 +207,7 @@ __device__ __forceinline__ void splat(float4* accum, bool on, uint32_t pix, floa
 }
 
 // a7 + a8 + a11 (+ per-block kill counts for a9).
-__global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st, float4* accum, uint32_t n) {
+__global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st, float4* accum, uint32_t n, const uint32_t* wave_ctl) {
   const uint32_t i = blockIdx.x * kBlock + threadIdx.x;
   const bool in = i < cp.N;
   const Counters* c = st.ctr;
@@ -292,6 +293,7 @@ __global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st
     if (blockIdx.x == 0) {
       atomicAdd(&st.ctr->mutations, (unsigned long long)cp.N);
       st.ctr->iteration = n;
+      if (wave_ctl && (wave_ctl[52] & 64u)) st.ctr->wave_timeouts += 1;   // k_wave's watchdog fired in this iteration's evaluation (dr_wave.cuh)
     }
   }
 }

@@ -46,7 +46,14 @@ namespace dr {
 #define DR_CHECKS 0             // test builds (compute-sanitizer is closed on this pool): device-side checks of the queue protocol;
 #endif                          // a violated check sets a bit of ctl[kCtlWaveError], which the evaluation hooks turn into DR_ERR_CUDA
 constexpr int kCtlWaveError = 52;
-enum : uint32_t { kErrIndex = 1u, kErrState = 2u, kErrOwner = 4u, kErrSegment = 8u, kErrHitRing = 16u, kErrCount = 32u };
+enum : uint32_t { kErrIndex = 1u, kErrState = 2u, kErrOwner = 4u, kErrSegment = 8u, kErrHitRing = 16u, kErrCount = 32u, kErrTimeout = 64u };
+#ifndef DR_WAVE_IDLE_LIMIT
+#define DR_WAVE_IDLE_LIMIT (1u << 25)
+#endif
+#ifndef DR_WAVE_LOSE_RAY
+#define DR_WAVE_LOSE_RAY 0      // test builds: the second rays of states 0..7 are never published, so the evaluation can only end by the watchdog
+#endif
+constexpr uint32_t kWaveIdleLimit = DR_WAVE_IDLE_LIMIT;   // idle rounds of >= 200 ns each (>= 6.7 s) before a trace warp gives up
 #if DR_CHECKS
 #define DR_CHECK(cond, bit) do { if (!(cond)) atomicOr(&ws.ctl[kCtlWaveError], (uint32_t)(bit)); } while (0)
 #else
@@ -82,6 +89,25 @@ __device__ __forceinline__ uint2 ld_relaxed2(const uint2* p) {
 }
 __device__ __forceinline__ void st_release2(uint2* p, uint2 v) {
   asm volatile("st.release.gpu.global.v2.u32 [%0], {%1, %2};" ::"l"(p), "r"(v.x), "r"(v.y) : "memory");
+}
+
+// A trace warp with nothing to trace waits here until the entry it waits for (`next`) is published (returns 1; at once if its
+// chunk is used up), every path has finished, or the watchdog fires (returns 2).  Not inlined: the wait must not cost the
+// traversal loop registers.
+__device__ __noinline__ uint32_t wave_idle_wait(const EvalWs& ws, uint32_t n, uint32_t next, bool chunk_done, uint32_t ring_cap) {
+  const unsigned lane = threadIdx.x & 31u;
+  for (uint32_t spins = 0;; ++spins) {
+    uint32_t v = 0;
+    if (lane == 0) {
+      const bool ready = chunk_done || (next < ring_cap && ld_relaxed2(ws.ring + next).y == ws.tag);
+      v = ld_relaxed(&ws.ctl[kCtlWaveDone]) >= n ? 2u : (ready ? 1u : 0u);
+      if (!v && (spins & 0xFFFu) == 0xFFFu && (ld_relaxed(&ws.ctl[kCtlWaveError]) & kErrTimeout)) v = 2u;
+      if (!v && spins > kWaveIdleLimit) { atomicOr(&ws.ctl[kCtlWaveError], (uint32_t)kErrTimeout); v = 2u; }
+    }
+    v = __shfl_sync(0xFFFFFFFFu, v, 0);
+    if (v) return v;
+    __nanosleep(200);
+  }
 }
 
 // ---- the trace warps ------------------------------------------------------------------------------------------------
@@ -183,11 +209,11 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
       want &= ~got;
     }
     unsigned act = __ballot_sync(kFull, L.active);
-    if (!act) {  // nothing to trace: over, or waiting for the shade warps
-      uint32_t v = 0;
-      if (lane == 0) v = ld_relaxed(&ws.ctl[kCtlWaveDone]);
-      if (__shfl_sync(kFull, v, 0) >= n) break;
-      __nanosleep(200);
+    if (!act) {  // nothing to trace: over, or waiting for the shade warps.  Spin here (counter local to this path) until the next
+                 // claimed entry is published, every path has finished, or the watchdog gives up: the protocol cannot lose a
+                 // path, but a kernel that never ends would take the GPU down with it.
+      const bool over = wave_idle_wait(ws, n, claim + (taken == kFetchChunk ? kFetchChunk : known), taken == kFetchChunk, ring_cap) == 2u;
+      if (over) break;
       poll = 0;
       continue;
     }
@@ -233,8 +259,8 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
     if (cnt == 0xFFFFFFFFu) continue;
     if (cnt == 0) {
       uint32_t v = 0;
-      if (lane == 0) v = ld_relaxed(&ws.ctl[kCtlWaveDone]);
-      if (__shfl_sync(kFull, v, 0) >= n) break;
+      if (lane == 0) v = ld_relaxed(&ws.ctl[kCtlWaveDone]) | (ld_relaxed(&ws.ctl[kCtlWaveError]) & kErrTimeout ? 0xFFFFFFFFu : 0u);
+      if (__shfl_sync(kFull, v, 0) >= n) break;   // every path finished (or the watchdog fired)
       __nanosleep(100);
       continue;
     }
@@ -333,6 +359,9 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
       if (lane == 0) base = atomicAdd(&ws.ctl[kCtlWaveReserve], nc);
       base = __shfl_sync(kFull, base, 0);
       DR_CHECK(base + nc <= ring_cap, kErrIndex);
+#if DR_WAVE_LOSE_RAY
+      if (push && s < 8u && k == 1u) push = false;   // reserved, never published
+#endif
       if (push) st_release2(ws.ring + base + __popc(b & lt), make_uint2(entry, ws.tag));
     }
     if (lane == 0) {

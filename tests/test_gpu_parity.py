@@ -717,3 +717,34 @@ def test_bias_field_matches_oracle(dr, oracle, torch_):
         assert np.abs(g - o).max() <= 1e-6 * np.abs(o).max() + 1e-7 / dt * 1e-2, (sigma, dt, np.abs(g - o).max(), np.abs(o).max())
     with pytest.raises(dr.DrError):
         dr.Scene(S.furnace()).bias_field(0.01, 0.0, 1e-3)
+
+
+_LOST_RAY_SNIPPET = """
+import sys, torch
+sys.path.insert(0, {root!r})
+import paper_2605_08916_b200 as dr
+from dr_inputs import scenes as S
+ch = dr.Chains(dr.Scene(S.closed_furnace()), "metropolis_restore", 64, seed=1)
+ch.init(0)
+torch.cuda.synchronize()
+try:
+    ch.stats()
+    print("no error")
+except dr.DrError as e:
+    print("DrError", e.status, ch.lib_stats_timeouts() if hasattr(ch, "lib_stats_timeouts") else "")
+"""
+
+
+def test_a_lost_ray_ends_in_an_error_not_in_a_hang(dr, tmp_path):
+    """'if a path is lost ... every warp spins forever.  There is no watchdog, so the GPU hangs.'  The queue cannot
+    lose a ray any more, but the kernel does not rely on that to terminate: a build that drops one ray on purpose
+    (-DDR_WAVE_LOSE_RAY=1, idle limit lowered to milliseconds) ends, and dr_chains_stats reports DR_ERR_CUDA."""
+    import os
+    import subprocess
+    import sys
+    from paper_2605_08916_b200 import build
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    lib = build.build_variant("lose_ray", ["-DDR_WAVE_LOSE_RAY=1", "-DDR_WAVE_IDLE_LIMIT=4096"])
+    r = subprocess.run([sys.executable, "-c", _LOST_RAY_SNIPPET.format(root=root)], env=dict(os.environ, DR_LIB=lib), capture_output=True,
+                       text=True, timeout=120)
+    assert r.returncode == 0 and f"DrError {dr.DR_ERR_CUDA}" in r.stdout, r.stdout + r.stderr
