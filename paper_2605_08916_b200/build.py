@@ -7,7 +7,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdr.so")
 SOURCES = ["dr_api.cu", "dr_bvh.cpp"]
-DEPS = SOURCES + ["dr_kernels.cuh", "dr_eval.cuh", "dr_wave.cuh", "dr_traverse.cuh", "dr_path.cuh", "dr_rng.cuh", "dr_types.h", "../../include/dr.h"]
+DEPS = SOURCES + ["dr_kernels.cuh", "dr_eval.cuh", "dr_wave.cuh", "dr_grad.cuh", "dr_nee.cuh", "dr_traverse.cuh", "dr_path.cuh", "dr_rng.cuh",
+                  "dr_types.h", "../../include/dr.h"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # -fmad=false: no implicit contraction of a * b + c; the kernels say fmaf() where they want one (traversal), and the path
 # arithmetic rounds like a plain fp32 evaluation of the formulas of DESIGN.md Q4-Q8 (csrc/dr_path.cuh, Q15)

@@ -1,13 +1,18 @@
 // Wavefront evaluation of the target for a batch of PSS states (rows a3-a6): x -> (f, p, pixel, score).
-//   k_raygen            a3: camera ray of every state -> ray queue
-//   per segment k = 1..L:
-//     k_trace           a4: persistent closest-hit kernel; a warp refills its idle lanes from the ray queue
-//     k_shade           a3/a5: emission / termination, direction sampling at vertex k, throughput; surviving paths
-//                       are compacted into the next queue (ballot + block-level prefix sum, one atomic per block)
+//   k_raygen            a3: camera ray of every state -> ray queue (state record + queue entry for k_wave)
+//   rows a3-a5, two forms with identical results (dr_api.cu launch_eval):
+//     k_wave (dr_wave.cuh)   ONE persistent kernel traces and shades all segments; the default
+//     per segment k = 1..L:  k_trace  a4: persistent closest-hit kernel; a warp refills its idle lanes from the ray queue
+//                            k_shade  a3/a5: shade_vertex for every ray of the segment; surviving paths are compacted
+//                                     into the next queue (ballot + block-level prefix sum, one atomic per block)
 //   k_grad              a6: reverse pass over the recorded vertices, only for the states that need it
+//                       (with next-event estimation: k_grad_nee, dr_grad.cuh)
+// shade_vertex (here) is one path vertex: emission / termination, emitter connection, direction sample; it calls
+// vertex_fn<float> of dr_nee.cuh, the function the score kernels differentiate.  trav_step (here) is one lockstep step of
+// the traversal, used by k_trace and k_wave.
 // One thread = one ray / path vertex; nothing here is a dense contraction (no tensor cores).  The paper runs one
 // shader thread per chain through a hardware ray-tracing pipeline; splitting the path into
-// per-segment waves is what keeps 32-wide warps busy without RT cores (profiles/r01a: the one-thread-one-path
+// per-segment rays is what keeps 32-wide warps busy without RT cores (profiles/r01a: the one-thread-one-path
 // kernel ran with 4.5 of 32 lanes active).
 #pragma once
 #include "dr_path.cuh"

@@ -4,8 +4,8 @@
 // an edge-grazing ray hits) then fall the same way on both sides of a parity check (Q15).
 // Target evaluation on the device, per-vertex pieces: x -> (f, p, pixel, score)  (rows a3, a5, a6).
 //   a3 camera ray and direction sampling at a vertex, a5 throughput / emission, a6 the local Jacobians of the
-//   reverse pass (forward-mode numbers with a handful of tangents).  The wavefront kernels that call these are
-//   in dr_kernels.cuh; the closest-hit query (a4) is dr_traverse.cuh.
+//   reverse pass (forward-mode numbers with a handful of tangents).  One vertex as a whole is vertex_fn (dr_nee.cuh); the
+//   wavefront kernels that call these are in dr_eval.cuh / dr_wave.cuh / dr_grad.cuh; the closest-hit query (a4) is dr_traverse.cuh.
 // The path map is DESIGN.md Q4-Q9 (the paper does not describe its path sampling routines).
 #pragma once
 #include <cfloat>

@@ -305,6 +305,38 @@ def test_teacher_forced_parity_f4(dr, oracle, torch_, variant, case):
     _teacher_forced(dr, oracle, torch_, variant[0], case, **variant[1])
 
 
+def test_packed_frame_equals_plain_resolve(dr, torch_):
+    """a sharded frame is dr_pack_frame -> ONE all-reduce -> dr_resolve_image_packed.  With one shard the
+    all-reduce is the identity: the packed path must give the image of dr_resolve_image, the tail must hold the counters as
+    16-bit limbs, and two shards' buffers added together must resolve to the image of the unsharded run."""
+    from paper_2605_08916_b200 import sharding
+    desc = S.mini_machines()
+    gsc = dr.Scene(desc)
+    for method in ("diffusion_restore", "metropolis"):
+        ch = dr.Chains(gsc, method, 3000, seed=6, p_lambda_override=0.05)
+        ch.init(0)
+        ch.step(5)
+        want = ch.resolve()[0].clone()
+        buf = ch.pack_frame()
+        st = ch.stats()
+        tail = buf[-8:].cpu().numpy()
+        assert list(tail[:4]) == sharding.limbs(st["tours"]) and list(tail[4:]) == sharding.limbs(st["mutations"])
+        assert torch_.equal(buf[:-8].view(-1, 4), ch.accum)
+        got = sharding.resolve_frame(ch)
+        assert torch_.equal(got, want)
+    full = dr.Chains(gsc, "diffusion_restore", 2000, seed=4, p_lambda_override=0.05)
+    full.init(0); full.step(4)
+    want = full.resolve()[0].clone()
+    shards = [dr.Chains(gsc, "diffusion_restore", 1000, seed=4, p_lambda_override=0.05, chain_offset=off) for off in (0, 1000)]
+    total = None
+    for ch in shards:
+        ch.init(0); ch.step(4)
+        b = ch.pack_frame().clone()
+        total = b if total is None else total + b              # what the all-reduce(sum) does
+    got = shards[0].resolve_packed(total)
+    assert torch_.allclose(got, want, rtol=1e-4, atol=1e-7)
+
+
 def test_sharded_chains_against_the_oracle(dr, oracle, torch_):
     """a shard (global chain ids 1000 .. 1999 of a 2000-chain run) against the oracle's shard with the same
     chain_offset, teacher-forced like everything else: the RNG streams are keyed by global chain id on both sides."""
