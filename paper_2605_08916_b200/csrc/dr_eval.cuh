@@ -25,13 +25,13 @@ namespace dr {
 #define DR_STREAM_HINTS 1   // evict-first stores of the vertex record, streaming loads of x in the shading: k_wave 4.33 -> 4.30 ms
 #endif
 #ifndef DR_TRACE_BLOCK
-#define DR_TRACE_BLOCK 640
+#define DR_TRACE_BLOCK 768   // 24 warps at 80 registers (with one triangle slot per lane): 640 / 704 / 768 / 896 / 1024 threads: profiles/r02f_tuning.md
 #endif
 #ifndef DR_TRI_STACK
 #define DR_TRI_STACK 8
 #endif
 #ifndef DR_TRIS_PER_STEP
-#define DR_TRIS_PER_STEP 2
+#define DR_TRIS_PER_STEP 1   // 2 slots: 11 more registers per thread (20 warps); 1 slot and 24 warps is 2.5 % faster (r02f)
 #endif
 #ifndef DR_REFILL_BELOW
 #define DR_REFILL_BELOW 30

@@ -7,7 +7,7 @@
 // runs dry once, at the end of the evaluation:
 //   * trace warps: the lockstep traversal of k_trace (trav_step); an idle lane takes the next ray of the queue.
 //     A finished ray goes, as (state | segment, t, triangle), into a small ring in the block's shared memory.
-//   * shade warps (kWaveShadeWarps per block): take up to 32 finished rays from the block's ring, run shade_vertex
+//   * shade warps (kWaveShadeWarps<NEE> per block): take up to 32 finished rays from the block's ring, run shade_vertex
 //     (the code of k_shade), write the surviving paths' next rays and count the finished paths.
 // The evaluation is over when every path has finished (ctl[kCtlWaveDone] == n).
 //
@@ -36,6 +36,9 @@ namespace dr {
 #ifndef DR_WAVE_SHADE_WARPS
 #define DR_WAVE_SHADE_WARPS 3
 #endif
+#ifndef DR_WAVE_SHADE_WARPS_NEE
+#define DR_WAVE_SHADE_WARPS_NEE 5   // two visits per vertex and the emitter connection: 3 / 4 / 5 / 6 warps: 9.0 / 7.4 / 6.7 / 6.9 ms (r02f)
+#endif
 #ifndef DR_WAVE_REFILL_BELOW
 #define DR_WAVE_REFILL_BELOW 26
 #endif
@@ -59,9 +62,9 @@ constexpr uint32_t kWaveIdleLimit = DR_WAVE_IDLE_LIMIT;   // idle rounds of >= 2
 #else
 #define DR_CHECK(cond, bit) do { } while (0)
 #endif
-constexpr int kWaveShadeWarps = DR_WAVE_SHADE_WARPS;     // sweep 1 / 2 / 3 / 4 / 5 / 6: 9.13 / 5.25 / 4.85 / 5.05 / 5.22 / 5.45 ms per frame
+template <bool NEE> constexpr int kWaveShadeWarps = NEE ? DR_WAVE_SHADE_WARPS_NEE : DR_WAVE_SHADE_WARPS;   // of the block's warps; the others trace
 constexpr int kWaveRefillBelow = DR_WAVE_REFILL_BELOW;   // a trace warp flushes its finished rays and refills below this many busy lanes
-constexpr int kWaveTraceThreads = kTraceBlock - 32 * kWaveShadeWarps;
+template <bool NEE> constexpr int kWaveTraceThreads = kTraceBlock - 32 * kWaveShadeWarps<NEE>;
 #ifndef DR_WAVE_HIT_CAP
 #define DR_WAVE_HIT_CAP 1024
 #endif
@@ -398,7 +401,7 @@ __global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws,
   }
   __syncthreads();
   const uint32_t one = *(volatile uint32_t*)&smem[0].x;  // dr_traverse.cuh qmagic
-  if (threadIdx.x >= (unsigned)kWaveTraceThreads) wave_shade_loop<GRAD, NEE>(sc, ws, io, n, wsh, h_pay, h_t, h_li);
+  if (threadIdx.x >= (unsigned)kWaveTraceThreads<NEE>) wave_shade_loop<GRAD, NEE>(sc, ws, io, n, wsh, h_pay, h_t, h_li);
   else wave_trace_loop<STATS, NEE>(sc, ws, n, smem, st, tst, wsh, h_pay, h_t, h_li, one, io.work);
 }
 
