@@ -127,7 +127,7 @@ typedef struct {
 } dr_stats;
 
 typedef struct {
-  uint32_t n_tris, n_nodes, depth, smem_nodes; /* BVH8 nodes, tree depth, nodes staged in shared memory */
+  uint32_t n_tris, n_nodes, depth, smem_nodes; /* BVH8 nodes, tree depth; smem_nodes is always 0 (no node staging: the field keeps the layout) */
   float sah_cost;
   float eps_ray;
   size_t device_bytes;

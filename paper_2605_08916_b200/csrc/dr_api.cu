@@ -55,7 +55,7 @@ struct dr_scene {
   void* d_lights = nullptr;
   dr_scene_info info{};
   int n_sm = 1;            // persistent k_trace grid: one block per SM
-  size_t trace_smem = 0;   // staged top-level nodes + per-thread traversal stacks
+  size_t trace_smem = 0;   // per-thread traversal stacks
   bool wave_ok = false;    // k_wave's shared memory (trace_smem + kWaveExtraSmem) fits; otherwise every evaluation uses the loop
 };
 
@@ -385,13 +385,14 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   }
   dev.nodes = (const uint4*)s->d_nodes; dev.tris = (const float4*)s->d_tris; dev.mats = (const float4*)s->d_mats;
   dev.n_nodes = (uint32_t)bvh.nodes.size();
-  dev.smem_nodes = std::min<uint32_t>(dev.n_nodes, (uint32_t)kMaxSmemNodes);
   dev.stack_cap = bvh.depth + 1;  // node groups: at most one per level
   const size_t stack_bytes = ((size_t)(dev.stack_cap + kTriStack) * sizeof(uint2) + (size_t)kTriStack * sizeof(uint32_t)) * kTraceBlock + 16;  // + the constant word of k_trace
-  if (stack_bytes + (size_t)dev.smem_nodes * sizeof(NodeC) > kMaxDynSmem)
-    dev.smem_nodes = (uint32_t)((kMaxDynSmem - stack_bytes) / sizeof(NodeC));
-  s->trace_smem = (size_t)dev.smem_nodes * sizeof(NodeC) + stack_bytes;
-  s->wave_ok = DR_SMEM_NODES == 0 && s->trace_smem + kWaveExtraSmem <= kMaxDynSmem;
+  if (stack_bytes > kMaxDynSmem) {   // (depth + 1) node groups per thread no longer fit the block's shared memory
+    dr_scene_destroy(s);
+    return fail(DR_ERR_UNSUPPORTED, "BVH8 deeper than the traversal stack allows");
+  }
+  s->trace_smem = stack_bytes;
+  s->wave_ok = s->trace_smem + kWaveExtraSmem <= kMaxDynSmem;
   e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   const void* waves[] = {(const void*)k_wave<false, false, false>, (const void*)k_wave<true, false, false>, (const void*)k_wave<false, false, true>,
@@ -456,7 +457,7 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   }
   dev.eps_ray = 1e-5f * bvh.diag;  // Q8
   dev.analytic = 0; dev.n_mix = 0;
-  s->info.n_tris = d->nt; s->info.n_nodes = dev.n_nodes; s->info.depth = bvh.depth; s->info.smem_nodes = dev.smem_nodes;
+  s->info.n_tris = d->nt; s->info.n_nodes = dev.n_nodes; s->info.depth = bvh.depth; s->info.smem_nodes = 0;
   s->info.sah_cost = bvh.sah_cost; s->info.eps_ray = dev.eps_ray; s->info.device_bytes = nb + tb + mb;
   *out = s;
   return DR_OK;
@@ -478,7 +479,7 @@ dr_status dr_scene_create_analytic2d(const dr_analytic2d_desc* d, dr_scene** out
   }
   dev.analytic = 1; dev.n_mix = (int)d->n_components;
   dev.W = d->width; dev.H = d->height; dev.L = 1; dev.d = 2; dev.planes = 1;
-  dev.smem_nodes = 0; dev.n_nodes = 0; dev.nee = 0; dev.n_lights = 0; dev.lights = nullptr; dev.light_total = 0.f;
+  dev.n_nodes = 0; dev.nee = 0; dev.n_lights = 0; dev.lights = nullptr; dev.light_total = 0.f;
   s->info = dr_scene_info{};
   *out = s;
   return DR_OK;

@@ -247,13 +247,8 @@ __device__ __forceinline__ bool trav_step(const DevScene& sc, const uint4* smem,
     const uint32_t node = s.gx + popc32(rest & ~(0xFFFFFFFFu << slot) & 0xFFu);
     s.gy = go ? rest : s.gy;
     if (go) {
-#if DR_SMEM_NODES == 0
       const uint4* np = sc.nodes + 5u * (size_t)node;
       w0 = DR_NODE_LD(np); w1 = DR_NODE_LD(np + 1); w2 = DR_NODE_LD(np + 2); w3 = DR_NODE_LD(np + 3); w4 = DR_NODE_LD(np + 4);
-#else
-      const uint4* np = node < sc.smem_nodes ? smem + 5u * node : sc.nodes + 5u * (size_t)node;
-      w0 = np[0]; w1 = np[1]; w2 = np[2]; w3 = np[3]; w4 = np[4];
-#endif
     }
     has_node = go;
   }
@@ -303,11 +298,10 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   extern __shared__ uint4 smem[];
   const uint32_t n = *cnt;
   if (n == 0) return;
-  for (uint32_t k = threadIdx.x; k < sc.smem_nodes * 5u; k += kTraceBlock) smem[k] = sc.nodes[k];
-  if (threadIdx.x == 0) smem[5u * sc.smem_nodes].x = 0x3F800000u;   // one 16-byte word between the nodes and the stacks
+  if (threadIdx.x == 0) smem[0].x = 0x3F800000u;   // one 16-byte word in front of the stacks
   __syncthreads();
-  const uint32_t one = *(volatile uint32_t*)&smem[5u * sc.smem_nodes].x;  // bits of 1.0f in a register the compiler cannot fold (dr_traverse.cuh qmagic)
-  SmemStack st{reinterpret_cast<uint2*>(smem + 5u * sc.smem_nodes + 1u) + threadIdx.x};
+  const uint32_t one = *(volatile uint32_t*)&smem[0].x;  // bits of 1.0f in a register the compiler cannot fold (dr_traverse.cuh qmagic)
+  SmemStack st{reinterpret_cast<uint2*>(smem + 1u) + threadIdx.x};
   SmemTriStack tst{st.base + (size_t)sc.stack_cap * kTraceBlock, nullptr};
   tst.base3 = reinterpret_cast<uint32_t*>(tst.base + (size_t)kTriStack * kTraceBlock - threadIdx.x) + threadIdx.x;
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;

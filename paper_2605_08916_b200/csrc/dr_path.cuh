@@ -23,7 +23,7 @@ struct DevScene {
   const uint4* nodes;   // NodeC as 5 uint4
   const float4* tris;   // TriPacked as 3 float4
   const float4* mats;   // MatPacked as 3 float4
-  uint32_t n_nodes, smem_nodes, stack_cap, n_tris, n_mats;
+  uint32_t n_nodes, stack_cap, n_tris, n_mats;
   const float4* lights; // next-event estimation (dr_nee.cuh Light): 5 float4 per emitter triangle
   uint32_t n_lights, nee;
   float light_total;

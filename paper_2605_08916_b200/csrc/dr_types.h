@@ -10,12 +10,7 @@ constexpr int kMaxPathLen = 16;        // L <= 16, d = 2L <= 32 (BASELINE.json c
 constexpr int kMaxPlanes = 8;          // d / 4 float4 planes
 constexpr int kMaxMix = 16;
 constexpr int kMaxLeafTris = 3;        // triangles per leaf (three bits per slot in the node's triangle mask)
-#ifndef DR_SMEM_NODES
-#define DR_SMEM_NODES 0
-#endif
-constexpr int kMaxSmemNodes = DR_SMEM_NODES;     // top BVH8 levels staged in shared memory (585 = four levels).  0 (default): none --
-                                                 // the shared memory is worth more as L1 (sweep in DESIGN.md section 6)
-constexpr int kMaxBvhDepth = 30;       // traversal stack entries per ray = depth + 1 (shared memory)
+constexpr int kMaxBvhDepth = 30;       // upper bound; what the traversal stacks in shared memory allow is checked by dr_scene_create
 
 // BVH8 node, 80 bytes = five 16-byte words.  Child boxes are quantised to 8 bits per plane on a per-node
 // grid (origin p, per-axis power-of-two cell 2^(e-127)), rounded outwards, so a node costs five 128-bit loads.

@@ -382,7 +382,6 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
 // NEE: the scene uses next-event estimation (two-phase vertices, shadow rays); STATS: the counting pass (NEE scenes only)
 template <bool GRAD, bool STATS, bool NEE>
 __global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
-  static_assert(DR_SMEM_NODES == 0, "k_wave does not stage nodes in shared memory");
   static_assert((kFetchChunk & (kFetchChunk - 1u)) == 0 && kFetchChunk <= 32, "chunk: power of two, one entry per lane");
   extern __shared__ uint4 smem[];
   if (n == 0) return;
