@@ -59,8 +59,8 @@ constexpr uint32_t kMiss = 0xFFFFFFFFu;
 constexpr int kCtlCnt = 0;     // cnt[k], k = 1..L: rays of segment k
 constexpr int kCtlHead = 20;   // head[k]: fetch counter of k_trace for segment k
 constexpr int kCtlGrad = 40;   // states on the reverse-pass list
-constexpr int kCtlGradBin = 64; // next-event estimation: states on the reverse-pass list by number of sampling vertices (16 bins)
-constexpr int kCtlWords = 96;
+constexpr int kCtlGradKind = 64; // next-event estimation: entries of the reverse sweep's list (vertex index k, material kind) at [3 k + kind]
+constexpr int kCtlWords = 128;
 
 // Workspace for up to `cap` states.  Two forms of the same evaluation use it (same results, state by state):
 //  * per-segment loop (k_trace / k_shade): ray queues qa, qb; an entry is three float4 in planes of `cap` entries,
@@ -73,8 +73,13 @@ struct EvalWs {
   uint2* hits;         // cap: (bits(t), triangle in leaf order or kMiss)   (loop form)
   uint2* ring;         // wave_ring_entries() ray entries, written once per evaluation, never reused      (k_wave)
   float4* rec;         // L * cap (score only): incoming direction and triangle of vertex k of state s at [k * cap + s]
+                       //   next-event estimation: (L + 1) planes, the terminal emitter hit of a path is recorded too, and the
+                       //   vertex' material kind sits in bits 30-31 of the triangle word; plane 0 = (masks, segments, terminal, vertices)
+  float4* rec2;        // (L + 1) * cap, next-event estimation + score: (origin of the ray that reached vertex k, density of its direction)
+  float4* rec3;        // (L + 1) * cap, next-event estimation + score: (throughput before vertex k, 0)
+  float4* adj;         // 3 * cap, next-event estimation + score: adjoints between the steps of the reverse sweep (dr_grad.cuh)
   uint32_t* pinfo;     // cap (score only): refract mask | rays << 16 of the finished path
-  uint32_t* gradlist;  // cap (score only); 16 * cap with next-event estimation: bin b (paths with b sampling vertices) at [b * cap, ...)
+  uint32_t* gradlist;  // cap (score only); 3 * L * cap with next-event estimation: list (vertex index k, material kind) at [(3 k + kind) * cap, ...)
   uint32_t* ctl;       // kCtlWords
   uint32_t cap;
   uint32_t tag;        // k_wave: tag of this evaluation, != 0; ring entries of earlier evaluations carry other tags
@@ -398,6 +403,15 @@ __device__ __forceinline__ void finish_path(const DevScene& sc_, const EvalWs& w
   }
 }
 
+// next-event estimation + score: what the reverse sweep (dr_grad.cuh) needs of the ray that reached vertex k
+__device__ __forceinline__ void record_vertex(const EvalWs& ws, uint32_t k, uint32_t s, float3 o, float3 d, uint32_t li, uint32_t kind,
+                                              float pb_prev, float T0, float T1, float T2) {
+  const size_t at = (size_t)k * ws.cap + s;
+  __stcs(&ws.rec[at], make_float4(d.x, d.y, d.z, __uint_as_float(li | (kind << 30))));
+  __stcs(&ws.rec2[at], make_float4(o.x, o.y, o.z, pb_prev));
+  __stcs(&ws.rec3[at], make_float4(T0, T1, T2, 0.f));
+}
+
 template <bool GRAD, bool NEE>
 __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t k, const float4& Q0,
                                              const float4& Q1, const float4& Q2, float pb_prev, const uint2& h, uint32_t s, ShadeOut& out,
@@ -431,6 +445,7 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
         const float4 m2 = __ldg(&sc.mats[3 * mi + 2]);
         const V3<float> ov{o.x, o.y, o.z}, dv{d.x, d.y, d.z};
         const float w_b = emitter_weight<float, NEE>(sc, xyz(t0), fr.nf, ov, dv, pb_prev, pb_prev >= 0.f);   // dn < 0: nf = n
+        if (GRAD && NEE && sc.nee) record_vertex(ws, k, s, o, d, li, 3u, pb_prev, T0, T1, T2);   // the reverse sweep starts here
         f0 = T0 * m1.z * w_b; f1 = T1 * m1.w * w_b; f2 = T2 * m2.x * w_b;
       } else {
         sig = fnv(sig, 5u);
@@ -439,11 +454,8 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
     } else if (k < sc.L) {
       term = kTermNone;
       const float4 u = x_vertex(sc, io, s, k);
-#if DR_STREAM_HINTS
-      if (GRAD) __stcs(&ws.rec[(size_t)k * cap + s], make_float4(d.x, d.y, d.z, __uint_as_float(li)));   // written once, read by k_grad only: evict first
-#else
-      if (GRAD) ws.rec[(size_t)k * cap + s] = make_float4(d.x, d.y, d.z, __uint_as_float(li));
-#endif
+      if (GRAD && NEE && sc.nee) record_vertex(ws, k, s, o, d, li, kind, pb_prev, T0, T1, T2);
+      else if (GRAD) __stcs(&ws.rec[(size_t)k * cap + s], make_float4(d.x, d.y, d.z, __uint_as_float(li)));   // written once, read by k_grad only: evict first
       const V3<float> ov{o.x, o.y, o.z}, dv{d.x, d.y, d.z};
       VertexOut<float> vo;
       V3<float> hit;

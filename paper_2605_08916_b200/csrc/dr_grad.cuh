@@ -1,14 +1,22 @@
-// Row a6 with next-event estimation: score g = grad p / (p + eps) of a listed state by a reverse sweep over its path.
+// Row a6 with next-event estimation: score g = grad p / (p + eps) of every state with p > 0, by a reverse sweep over its path.
 // With emitter connections the contribution depends on the positions of the vertices, not only on directions (DESIGN.md
 // Q21), so the sweep carries the adjoints of the ray that enters each vertex -- origin, direction and, for the MIS weight of
-// an emitter found by the direction sample, the density of that direction.  The path is first replayed forwards from x and
-// the recorded discrete decisions (triangle per segment, dielectric lobes, visibility bits: ws.rec), with vertex_fn<float>,
-// the function the shading itself uses; then, last vertex first, the gradient of the scalar
+// an emitter found by the direction sample, the density of that direction.  Last vertex first, the gradient of the scalar
 //     Phi_k = sum_c lum_c T_k,c (C_k,c + W_k,c R_k+1,c) + o_bar . o_k+1 + d_bar . d_k+1 + pb_bar pb_k
-// with respect to the vertex' ten inputs (o_k, d_k, u1, u2, v1, v2) is taken by three evaluations of vertex_fn<Du<4>>
-// (T_k: throughput before the vertex, R_k+1: radiance per unit throughput from the later vertices, bars: adjoints of the
-// next ray).  The u-part is the score of the vertex' coordinates, the (o, d)-part the adjoint handed to the vertex before.
-// One thread = one listed state.  The oracle differentiates the same function with forward-mode dual numbers.
+// with respect to the vertex' ten inputs (o_k, d_k, u1, u2, v1, v2) is taken by evaluations of vertex_fn<Du<4>>, the function
+// the shading itself uses with T = float (T_k: throughput before the vertex, R_k+1: radiance per unit throughput from the later
+// vertices, bars: adjoints of the next ray).  The u-part is the score of the vertex' coordinates, the (o, d)-part the adjoint
+// handed to the vertex before.  The oracle differentiates the same function with forward-mode dual numbers.
+//
+// Shape (profiles/r02g_grad_nee.md).  One thread per path ran with 12 of 32 lanes active (material kinds and connection
+// outcomes differ from lane to lane) out of a 99 KB instruction footprint.  Now:
+//   k_grad_nee_init           per state: what the path's last ray found (R and the adjoints of that ray) -> ws.adj; and the path's
+//                             vertices go onto one list per (vertex index k, material kind of vertex k)
+//   k_grad_nee_vertex<KIND>   k = L-1 .. 1, KIND = Lambert / dielectric / GGX: vertex k of every path that has one of that kind;
+//                             every lane of a warp differentiates the same code, compiled for that kind alone
+//   k_grad_nee_finish         Q18
+// What the forward pass knew of the ray that reached a vertex (origin, direction, direction density, throughput) was recorded
+// by the shading (record_vertex, dr_eval.cuh): there is no forward replay.  The adjoints wait in ws.adj between the launches.
 #pragma once
 #include "dr_eval.cuh"
 
@@ -33,7 +41,9 @@ __device__ __forceinline__ void load_vertex(const DevScene& sc, uint32_t li, flo
   tri_frame(e1, e2, d, f.fr, f.dn);
 }
 
-// d Phi / d (four of the inputs).  mode 0: o.xyz, 1: d.xyz, 2: (u1, u2, v1, v2).  Also returns W and the visible C (values).
+// d Phi / d (four of the inputs) at a vertex of material KIND.  mode 0: o.xyz, 1: d.xyz, 2: (u1, u2, v1, v2).  Also returns W and
+// the visible C (values).
+template <int KIND>
 __device__ __noinline__ float4 vertex_phi_grad(const DevScene& sc, const VtxFrozen& f, float3 o, float3 d, float4 u, int mode, float3 lumT,
                                                float3 R, float3 ob, float3 db, float pbb, float3* W_out, float3* C_out) {
   typedef Du<4> D;
@@ -46,7 +56,7 @@ __device__ __noinline__ float4 vertex_phi_grad(const DevScene& sc, const VtxFroz
   V3<D> hit;
   bool reflect = f.reflect;
   uint32_t lj = 0;
-  vertex_fn<D>(sc, f.v0, f.fr, f.dn, f.m0, f.m1, f.kind, O, Dd, U1, U2, V1, V2, false, reflect, vo, hit, lj);
+  vertex_fn<D>(sc, f.v0, f.fr, f.dn, f.m0, f.m1, (uint32_t)KIND, O, Dd, U1, U2, V1, V2, false, reflect, vo, hit, lj);
   const bool conn = vo.nee_valid && f.vis;
   D phi = du_const<4>(0.f);
   const float lt[3] = {lumT.x, lumT.y, lumT.z}, Rr[3] = {R.x, R.y, R.z};
@@ -81,73 +91,64 @@ __device__ __noinline__ float4 emitter_weight_grad(const DevScene& sc, float3 v0
   return make_float4(w.d[0], w.d[1], w.d[2], w.d[3]);
 }
 
-#ifndef DR_GRAD_MIN_BLOCKS
-#define DR_GRAD_MIN_BLOCKS 6   // 80 registers: 1 / 3 / 4 / 6 blocks per SM: 6.12 / 5.90 / 5.64 / 5.32 ms per frame (configs[3] + NEE)
-#endif
-__global__ void __launch_bounds__(kGradBlock, DR_GRAD_MIN_BLOCKS) k_grad_nee(DevScene sc, EvalWs ws, EvalIO io) {
-  const uint32_t idx = blockIdx.x * kGradBlock + threadIdx.x;
-  if (idx == 0 && io.grad_ctr) atomicAdd(io.grad_ctr, (unsigned long long)ws.ctl[kCtlGrad]);
-  if (idx >= ws.ctl[kCtlGrad]) return;
+constexpr int kGradVertexBlock = 128;
+constexpr uint32_t kRecLiMask = 0x3FFFFFFFu;   // ws.rec[k].w = triangle (leaf order) | material kind << 30
+// list of the paths whose vertex k has material `kind`: entries ws.gradlist[(3 k + kind) * cap ...], count ws.ctl[kCtlGradKind + 3 k + kind]
+__device__ __forceinline__ uint32_t grad_list(uint32_t k, uint32_t kind) { return 3u * k + kind; }
+
+// Per state, in index order (the shading wrote f, the header ws.rec[s] and the vertex records of every finished path):
+// what the path's last ray found -- R (radiance per unit throughput) and the adjoints of that ray -- and the path's vertices
+// onto the (k, kind) lists, one atomic per warp, list and vertex index.
+__global__ void __launch_bounds__(kGradBlock) k_grad_nee_init(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
+  const uint32_t s = blockIdx.x * kGradBlock + threadIdx.x;
   const size_t cap = ws.cap;
-  uint32_t rem = idx, bin = 15;   // the list is binned by the number of sampling vertices; longest paths first
-  for (;; --bin) {
-    const uint32_t c = ws.ctl[kCtlGradBin + bin];
-    if (rem < c || bin == 0) break;
-    rem -= c;
+  const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
+  const bool listed = s < n && io.f[s].w > 0.f;   // finish_path: p > 0
+  uint32_t nv = 0, term = kTermNone;
+  if (s < n) ws.pinfo[s] = 0u;   // "score not finite" flag of this evaluation
+  if (listed) {
+    const float4 hdr = ws.rec[s];
+    term = __float_as_uint(hdr.z); nv = __float_as_uint(hdr.w);
   }
-  const uint32_t s = ws.gradlist[(size_t)bin * cap + rem];
-  const float4 fp = io.f[s];
-  const float inv_phat = 1.0f / (fp.w + kEps);
-  const float4 hdr = ws.rec[s];
-  const uint32_t info = __float_as_uint(hdr.x), term = __float_as_uint(hdr.z), nv = __float_as_uint(hdr.w);
-  const float lum[3] = {0.2126f, 0.7152f, 0.0722f};
-  // ---- forward replay: the ray entering every vertex, the throughput before it
-  float3 O[kMaxPathLen + 1], Dv[kMaxPathLen + 1], Tk[kMaxPathLen + 1];
-  float PB[kMaxPathLen + 1];
-  uint32_t LI[kMaxPathLen + 1];
-  const float4 x0 = io.x[s];
   {
-    const V3<float> dc = camera_dir<float>(sc, x0.x, x0.y);
-    O[1] = make_float3(sc.cam_pos[0], sc.cam_pos[1], sc.cam_pos[2]);
-    Dv[1] = make_float3(dc.x, dc.y, dc.z);
-    PB[1] = -1.f;
-    Tk[1] = make_float3(1.f, 1.f, 1.f);
+    const unsigned lm = __ballot_sync(0xFFFFFFFFu, listed);
+    if (lane == 0 && lm && io.grad_ctr) atomicAdd(io.grad_ctr, (unsigned long long)__popc(lm));
   }
-  for (uint32_t k = 1; k <= nv; ++k) {
-    LI[k] = __float_as_uint(ws.rec[(size_t)k * cap + s].w);
-    VtxFrozen f;
-    load_vertex(sc, LI[k], Dv[k], f);
-    const float4 u = io.x[(size_t)k * io.stride + s];
-    const V3<float> ov{O[k].x, O[k].y, O[k].z}, dv{Dv[k].x, Dv[k].y, Dv[k].z};
-    VertexOut<float> vo;
-    V3<float> hit;
-    bool reflect = !((info >> k) & 1u);
-    uint32_t lj = 0;
-    vertex_fn<float>(sc, f.v0, f.fr, f.dn, f.m0, f.m1, f.kind, ov, dv, u.x, u.y, u.z, u.w, false, reflect, vo, hit, lj);
-    O[k + 1] = make_float3(vo.o2.x, vo.o2.y, vo.o2.z);
-    Dv[k + 1] = make_float3(vo.d2.x, vo.d2.y, vo.d2.z);
-    PB[k + 1] = vo.pb_valid ? vo.pb : -1.f;
-    Tk[k + 1] = make_float3(Tk[k].x * vo.W[0], Tk[k].y * vo.W[1], Tk[k].z * vo.W[2]);
+  const uint32_t kmax = __reduce_max_sync(0xFFFFFFFFu, nv);
+  for (uint32_t k = 1; k <= kmax; ++k) {
+    const uint32_t kind = k <= nv ? (__float_as_uint(ws.rec[(size_t)k * cap + s].w) >> 30) : 3u;
+#pragma unroll
+    for (uint32_t q = 0; q < 3; ++q) {
+      const unsigned m = __ballot_sync(0xFFFFFFFFu, kind == q);
+      if (!m) continue;
+      uint32_t base = 0;
+      if (lane == (unsigned)(__ffs(m) - 1)) base = atomicAdd(&ws.ctl[kCtlGradKind + grad_list(k, q)], (uint32_t)__popc(m));
+      base = __shfl_sync(0xFFFFFFFFu, base, __ffs(m) - 1);
+      if (kind == q) ws.gradlist[(size_t)grad_list(k, q) * cap + base + __popc(m & lt)] = s;
+    }
   }
-  // ---- what the path's last ray found
+  if (!listed) return;
   float3 R = make_float3(0.f, 0.f, 0.f), ob = R, db = R;
   float pbb = 0.f;
   if (term == kMiss) {
     R = make_float3(sc.env[0], sc.env[1], sc.env[2]);
   } else if (term != kTermNone) {
+    const size_t at = (size_t)(nv + 1) * cap + s;   // the emitter hit was recorded as vertex nv + 1
+    const float4 rD = ws.rec[at], rO = ws.rec2[at], rT = ws.rec3[at];
     const float4 t0 = __ldg(&sc.tris[3 * term]), t1 = __ldg(&sc.tris[3 * term + 1]), t2 = __ldg(&sc.tris[3 * term + 2]);
     const float3 e1 = make_float3(t0.w, t1.x, t1.y), e2 = make_float3(t1.z, t1.w, t2.x);
     const uint32_t mi = __float_as_uint(t2.z);
     const float4 m1 = __ldg(&sc.mats[3 * mi + 1]), m2 = __ldg(&sc.mats[3 * mi + 2]);
     const float3 le = make_float3(m1.z, m1.w, m2.x);
-    const float3 n = normalize3(cross3(e1, e2));
-    const uint32_t K = nv + 1;
-    if (dot3(Dv[K], n) < 0.f) {   // front face (the forward pass added T Le w_b)
+    const float3 nrm = normalize3(cross3(e1, e2));
+    const float3 o = xyz(rO), d = xyz(rD);
+    const float pb = rO.w;
+    if (dot3(d, nrm) < 0.f) {   // front face (the forward pass added T Le w_b)
       float wb = 1.f;
-      if (PB[K] >= 0.f) {
-        const float sL = lum[0] * Tk[K].x * le.x + lum[1] * Tk[K].y * le.y + lum[2] * Tk[K].z * le.z;
-        const float4 go = emitter_weight_grad(sc, xyz(t0), n, O[K], Dv[K], PB[K], 0, &wb);
-        const float4 gd = emitter_weight_grad(sc, xyz(t0), n, O[K], Dv[K], PB[K], 1, nullptr);
+      if (pb >= 0.f) {
+        const float sL = 0.2126f * rT.x * le.x + 0.7152f * rT.y * le.y + 0.0722f * rT.z * le.z;
+        const float4 go = emitter_weight_grad(sc, xyz(t0), nrm, o, d, pb, 0, &wb);
+        const float4 gd = emitter_weight_grad(sc, xyz(t0), nrm, o, d, pb, 1, nullptr);
         ob = make_float3(sL * go.x, sL * go.y, sL * go.z);
         db = make_float3(sL * gd.x, sL * gd.y, sL * gd.z);
         pbb = sL * go.w;
@@ -155,30 +156,74 @@ __global__ void __launch_bounds__(kGradBlock, DR_GRAD_MIN_BLOCKS) k_grad_nee(Dev
       R = make_float3(le.x * wb, le.y * wb, le.z * wb);
     }
   }
-  // ---- reverse sweep
-  bool bad = false;
-  for (uint32_t k = nv; k >= 1; --k) {
-    VtxFrozen f;
-    load_vertex(sc, LI[k], Dv[k], f);
-    f.reflect = !((info >> k) & 1u);
-    f.vis = ((info >> (16u + k)) & 1u) != 0u;
+  ws.adj[s] = make_float4(R.x, R.y, R.z, ob.x);
+  ws.adj[cap + s] = make_float4(ob.y, ob.z, db.x, db.y);
+  ws.adj[2 * cap + s] = make_float4(db.z, pbb, 0.f, 0.f);
+}
+
+#ifndef DR_GRAD_MIN_BLOCKS
+#define DR_GRAD_MIN_BLOCKS 4
+#endif
+// Vertex k of every path whose vertex k has material KIND (0 Lambert, 1 dielectric, 2 GGX).
+// Phi depends on the ray (o, d) through the hit point h = o + t d on the frozen plane, t = ((v0 - o).n) / (d.n), and -- for a
+// dielectric or GGX vertex only -- on d itself.  With P = I - d n^T / (d.n):  dPhi/do = P^T dPhi/dh,  dPhi/dd = t P^T dPhi/dh
+// + (dPhi/dd at fixed h).  So a Lambert vertex needs no pass over d (dPhi/dd = t dPhi/do), and a dielectric vertex, which makes
+// no connection and has weight one, needs only the Jacobian of its outgoing direction.
+template <int KIND>
+__global__ void __launch_bounds__(kGradVertexBlock, DR_GRAD_MIN_BLOCKS) k_grad_nee_vertex(DevScene sc, EvalWs ws, EvalIO io, uint32_t k) {
+  const uint32_t idx = blockIdx.x * kGradVertexBlock + threadIdx.x;
+  if (idx >= ws.ctl[kCtlGradKind + grad_list(k, KIND)]) return;
+  const size_t cap = ws.cap;
+  const uint32_t s = ws.gradlist[(size_t)grad_list(k, KIND) * cap + idx];
+  const size_t at = (size_t)k * cap + s;
+  const float4 rD = ws.rec[at], rO = ws.rec2[at], rT = ws.rec3[at];
+  const uint32_t info = __float_as_uint(ws.rec[s].x);
+  const float4 a0 = ws.adj[s], a1 = ws.adj[cap + s], a2 = ws.adj[2 * cap + s];
+  float3 R = make_float3(a0.x, a0.y, a0.z), ob = make_float3(a0.w, a1.x, a1.y), db = make_float3(a1.z, a1.w, a2.x);
+  const float pbb = a2.y;
+  const float3 o = xyz(rO), d = xyz(rD);
+  VtxFrozen f;
+  load_vertex(sc, __float_as_uint(rD.w) & kRecLiMask, d, f);
+  f.reflect = !((info >> k) & 1u);
+  f.vis = ((info >> (16u + k)) & 1u) != 0u;
+  const float inv_phat = 1.0f / (io.f[s].w + kEps);
+  const float side = f.dn < 0.f ? 1.f : -1.f;
+  const float3 n = f.fr.nf * side;
+  const float dnn = dot3(d, n);
+  const float tp = dot3(f.v0 - o, n) / dnn;
+  float3 W = make_float3(1.f, 1.f, 1.f), C = make_float3(0.f, 0.f, 0.f);
+  float4 gu = make_float4(0.f, 0.f, 0.f, 0.f), go, gd;
+  if (KIND == 1) {
+    const float c = dot3(d, ob) / dnn;
+    go = make_float4(ob.x - n.x * c, ob.y - n.y * c, ob.z - n.z * c, 0.f);   // P^T o_bar  (o2 = h + const)
+    const float eta = f.dn < 0.f ? f.m1.x : 1.0f / f.m1.x;
+    const V3<Du<3>> di{du_var<3>(d.x, 0), du_var<3>(d.y, 1), du_var<3>(d.z, 2)};
+    const V3<Du<3>> w = dielectric_dir<Du<3>>(f.fr, eta, f.reflect, di);
+    gd = make_float4(tp * go.x + (db.x * w.x.d[0] + db.y * w.y.d[0] + db.z * w.z.d[0]),
+                     tp * go.y + (db.x * w.x.d[1] + db.y * w.y.d[1] + db.z * w.z.d[1]),
+                     tp * go.z + (db.x * w.x.d[2] + db.y * w.y.d[2] + db.z * w.z.d[2]), 0.f);
+  } else {
     const float4 u = io.x[(size_t)k * io.stride + s];
-    const float3 lumT = make_float3(lum[0] * Tk[k].x, lum[1] * Tk[k].y, lum[2] * Tk[k].z);
-    float3 W, C;
-    const float4 gu = vertex_phi_grad(sc, f, O[k], Dv[k], u, 2, lumT, R, ob, db, pbb, &W, &C);
-    const float4 go = vertex_phi_grad(sc, f, O[k], Dv[k], u, 0, lumT, R, ob, db, pbb, nullptr, nullptr);
-    const float4 gd = vertex_phi_grad(sc, f, O[k], Dv[k], u, 1, lumT, R, ob, db, pbb, nullptr, nullptr);
-    const float4 g = make_float4(gu.x * inv_phat, gu.y * inv_phat, gu.z * inv_phat, gu.w * inv_phat);
-    bad = bad || !(isfinite(g.x) && isfinite(g.y) && isfinite(g.z) && isfinite(g.w));
-    io.g[(size_t)k * io.stride + s] = g;
-    R = make_float3(C.x + W.x * R.x, C.y + W.y * R.y, C.z + W.z * R.z);
-    ob = make_float3(go.x, go.y, go.z);
-    db = make_float3(gd.x, gd.y, gd.z);
-    pbb = 0.f;   // a vertex that samples does not use the density of the ray that reached it
+    const float3 lumT = make_float3(0.2126f * rT.x, 0.7152f * rT.y, 0.0722f * rT.z);
+    gu = vertex_phi_grad<KIND>(sc, f, o, d, u, 2, lumT, R, ob, db, pbb, &W, &C);
+    go = vertex_phi_grad<KIND>(sc, f, o, d, u, 0, lumT, R, ob, db, pbb, nullptr, nullptr);
+    if (KIND == 0) gd = make_float4(tp * go.x, tp * go.y, tp * go.z, 0.f);
+    else gd = vertex_phi_grad<KIND>(sc, f, o, d, u, 1, lumT, R, ob, db, pbb, nullptr, nullptr);
   }
-  {
+  const float4 g = make_float4(gu.x * inv_phat, gu.y * inv_phat, gu.z * inv_phat, gu.w * inv_phat);
+  bool bad = !(isfinite(g.x) && isfinite(g.y) && isfinite(g.z) && isfinite(g.w));
+  io.g[(size_t)k * io.stride + s] = g;
+  R = make_float3(C.x + W.x * R.x, C.y + W.y * R.y, C.z + W.z * R.z);
+  ob = make_float3(go.x, go.y, go.z);
+  db = make_float3(gd.x, gd.y, gd.z);
+  if (k > 1u) {   // a vertex that samples does not use the density of the ray that reached it: pb_bar = 0
+    ws.adj[s] = make_float4(R.x, R.y, R.z, ob.x);
+    ws.adj[cap + s] = make_float4(ob.y, ob.z, db.x, db.y);
+    ws.adj[2 * cap + s] = make_float4(db.z, 0.f, 0.f, 0.f);
+  } else {        // the camera: its position is fixed, only the direction depends on the film point
     float ga = 0.f, gb = 0.f;
-    if (db.x != 0.f || db.y != 0.f || db.z != 0.f) {   // the camera position is fixed: only the direction depends on the film point
+    if (db.x != 0.f || db.y != 0.f || db.z != 0.f) {
+      const float4 x0 = io.x[s];
       const V3<Du<2>> w = camera_dir<Du<2>>(sc, du_var<2>(x0.x, 0), du_var<2>(x0.y, 1));
       ga = (db.x * w.x.d[0] + db.y * w.y.d[0] + db.z * w.z.d[0]) * inv_phat;
       gb = (db.x * w.x.d[1] + db.y * w.y.d[1] + db.z * w.z.d[1]) * inv_phat;
@@ -186,11 +231,17 @@ __global__ void __launch_bounds__(kGradBlock, DR_GRAD_MIN_BLOCKS) k_grad_nee(Dev
     bad = bad || !(isfinite(ga) && isfinite(gb));
     io.g[s] = make_float4(ga, gb, 0.f, 0.f);
   }
-  if (bad) {  // Q18: a non-finite score makes the state a zero-contribution state
-    io.f[s] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (uint32_t k = 0; k <= nv; ++k) io.g[(size_t)k * io.stride + s] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (io.nonfinite_ctr) atomicAdd(io.nonfinite_ctr, 1ull);
-  }
+  if (bad) ws.pinfo[s] = 1u;
+}
+
+// Q18: a non-finite score makes the state a zero-contribution state
+__global__ void __launch_bounds__(kGradBlock) k_grad_nee_finish(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
+  const uint32_t s = blockIdx.x * kGradBlock + threadIdx.x;
+  if (s >= n || !ws.pinfo[s]) return;
+  const uint32_t nv = __float_as_uint(ws.rec[s].w);
+  io.f[s] = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (uint32_t k = 0; k <= nv; ++k) io.g[(size_t)k * io.stride + s] = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (io.nonfinite_ctr) atomicAdd(io.nonfinite_ctr, 1ull);
 }
 
 }  // namespace dr

@@ -334,24 +334,13 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
         entry = s | (k << kWaveKShift);
       }
     }
-    if (GRAD) {  // reverse-pass list: one atomic per warp (per bin of path length with next-event estimation: k_grad_nee's
-                 // threads then walk paths of equal length side by side)
+    if (GRAD && !NEE) {  // reverse-pass list: one atomic per warp (with next-event estimation the sweep makes its own lists: dr_grad.cuh)
       const unsigned gm = __ballot_sync(kFull, want_grad);
-      if (gm && !NEE) {
+      if (gm) {
         uint32_t base = 0;
         if (lane == 0) base = atomicAdd(&ws.ctl[kCtlGrad], (uint32_t)__popc(gm));
         base = __shfl_sync(kFull, base, 0);
         if (want_grad) ws.gradlist[base + __popc(gm & lt)] = s;
-      } else if (gm) {
-        if (lane == 0) atomicAdd(&ws.ctl[kCtlGrad], (uint32_t)__popc(gm));
-        if (want_grad) {
-          const unsigned peers = __match_any_sync(gm, grad_bin);
-          const unsigned leader = __ffs(peers) - 1u;
-          uint32_t base = 0;
-          if (lane == leader) base = atomicAdd(&ws.ctl[kCtlGradBin + grad_bin], (uint32_t)__popc(peers));
-          base = __shfl_sync(peers, base, leader);
-          ws.gradlist[(size_t)grad_bin * ws.cap + base + __popc(peers & lt)] = s;
-        }
       }
     }
     // ---- the queue entries of the paths that go on (release: the records above are visible before the entry)
