@@ -239,12 +239,8 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
     ProfScope ps(prof, DR_PROF_GRAD, s);
     if (dev.nee) {   // one launch per vertex index and material kind, last vertex first (dr_grad.cuh)
       k_grad_nee_init<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io, n);
-      const uint32_t gv = (n + kGradVertexBlock - 1) / kGradVertexBlock;   // the lists' lengths are known on the device only: blocks past the end leave at once
-      for (uint32_t k = dev.L - 1; k >= 1; --k) {
-        k_grad_nee_vertex<0><<<gv, kGradVertexBlock, 0, s>>>(dev, ws, io, k);
-        k_grad_nee_vertex<1><<<gv, kGradVertexBlock, 0, s>>>(dev, ws, io, k);
-        k_grad_nee_vertex<2><<<gv, kGradVertexBlock, 0, s>>>(dev, ws, io, k);
-      }
+      const uint32_t gv = (n + kGradVertexBlock - 1) / kGradVertexBlock + 3;   // three lists, each rounded up to whole blocks
+      for (uint32_t k = dev.L - 1; k >= 1; --k) k_grad_nee_vertex<<<gv, kGradVertexBlock, 0, s>>>(dev, ws, io, k);
       k_grad_nee_finish<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io, n);
     }
     else k_grad<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io);

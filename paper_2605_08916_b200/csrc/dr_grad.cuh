@@ -44,7 +44,7 @@ __device__ __forceinline__ void load_vertex(const DevScene& sc, uint32_t li, flo
 // d Phi / d (four of the inputs) at a vertex of material KIND.  mode 0: o.xyz, 1: d.xyz, 2: (u1, u2, v1, v2).  Also returns W and
 // the visible C (values).
 template <int KIND>
-__device__ __noinline__ float4 vertex_phi_grad(const DevScene& sc, const VtxFrozen& f, float3 o, float3 d, float4 u, int mode, float3 lumT,
+__device__ __forceinline__ float4 vertex_phi_grad(const DevScene& sc, const VtxFrozen& f, float3 o, float3 d, float4 u, int mode, float3 lumT,
                                                float3 R, float3 ob, float3 db, float pbb, float3* W_out, float3* C_out) {
   typedef Du<4> D;
   V3<D> O{du_const<4>(o.x), du_const<4>(o.y), du_const<4>(o.z)}, Dd{du_const<4>(d.x), du_const<4>(d.y), du_const<4>(d.z)};
@@ -170,9 +170,7 @@ __global__ void __launch_bounds__(kGradBlock) k_grad_nee_init(DevScene sc, EvalW
 // + (dPhi/dd at fixed h).  So a Lambert vertex needs no pass over d (dPhi/dd = t dPhi/do), and a dielectric vertex, which makes
 // no connection and has weight one, needs only the Jacobian of its outgoing direction.
 template <int KIND>
-__global__ void __launch_bounds__(kGradVertexBlock, DR_GRAD_MIN_BLOCKS) k_grad_nee_vertex(DevScene sc, EvalWs ws, EvalIO io, uint32_t k) {
-  const uint32_t idx = blockIdx.x * kGradVertexBlock + threadIdx.x;
-  if (idx >= ws.ctl[kCtlGradKind + grad_list(k, KIND)]) return;
+__device__ __forceinline__ void grad_vertex(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t k, uint32_t idx) {
   const size_t cap = ws.cap;
   const uint32_t s = ws.gradlist[(size_t)grad_list(k, KIND) * cap + idx];
   const size_t at = (size_t)k * cap + s;
@@ -205,10 +203,16 @@ __global__ void __launch_bounds__(kGradVertexBlock, DR_GRAD_MIN_BLOCKS) k_grad_n
   } else {
     const float4 u = io.x[(size_t)k * io.stride + s];
     const float3 lumT = make_float3(0.2126f * rT.x, 0.7152f * rT.y, 0.0722f * rT.z);
-    gu = vertex_phi_grad<KIND>(sc, f, o, d, u, 2, lumT, R, ob, db, pbb, &W, &C);
-    go = vertex_phi_grad<KIND>(sc, f, o, d, u, 0, lumT, R, ob, db, pbb, nullptr, nullptr);
+    // one copy of the differentiated vertex in the code, run two (Lambert) or three times: everything stays in registers
+#pragma unroll 1
+    for (int pass = 0; pass < (KIND == 0 ? 2 : 3); ++pass) {
+      float3 Wp, Cp;
+      const float4 r = vertex_phi_grad<KIND>(sc, f, o, d, u, pass == 0 ? 2 : pass - 1, lumT, R, ob, db, pbb, &Wp, &Cp);
+      if (pass == 0) { gu = r; W = Wp; C = Cp; }
+      else if (pass == 1) go = r;
+      else gd = r;
+    }
     if (KIND == 0) gd = make_float4(tp * go.x, tp * go.y, tp * go.z, 0.f);
-    else gd = vertex_phi_grad<KIND>(sc, f, o, d, u, 1, lumT, R, ob, db, pbb, nullptr, nullptr);
   }
   const float4 g = make_float4(gu.x * inv_phat, gu.y * inv_phat, gu.z * inv_phat, gu.w * inv_phat);
   bool bad = !(isfinite(g.x) && isfinite(g.y) && isfinite(g.z) && isfinite(g.w));
@@ -232,6 +236,21 @@ __global__ void __launch_bounds__(kGradVertexBlock, DR_GRAD_MIN_BLOCKS) k_grad_n
     io.g[s] = make_float4(ga, gb, 0.f, 0.f);
   }
   if (bad) ws.pinfo[s] = 1u;
+}
+
+// One launch per vertex index: the blocks are dealt to the three lists of that index in turn (list lengths are known on the
+// device only: the grid covers the worst case and the blocks past the end leave at once).
+__global__ void __launch_bounds__(kGradVertexBlock, DR_GRAD_MIN_BLOCKS) k_grad_nee_vertex(DevScene sc, EvalWs ws, EvalIO io, uint32_t k) {
+  const uint32_t c0 = ws.ctl[kCtlGradKind + grad_list(k, 0)], c1 = ws.ctl[kCtlGradKind + grad_list(k, 1)], c2 = ws.ctl[kCtlGradKind + grad_list(k, 2)];
+  const uint32_t nb0 = (c0 + kGradVertexBlock - 1) / kGradVertexBlock, nb2 = (c2 + kGradVertexBlock - 1) / kGradVertexBlock;
+  uint32_t b = blockIdx.x;
+  // GGX first (the longest blocks), then Lambert, then dielectric
+  if (b < nb2) { const uint32_t idx = b * kGradVertexBlock + threadIdx.x; if (idx < c2) grad_vertex<2>(sc, ws, io, k, idx); return; }
+  b -= nb2;
+  if (b < nb0) { const uint32_t idx = b * kGradVertexBlock + threadIdx.x; if (idx < c0) grad_vertex<0>(sc, ws, io, k, idx); return; }
+  b -= nb0;
+  const uint32_t idx = b * kGradVertexBlock + threadIdx.x;
+  if (idx < c1) grad_vertex<1>(sc, ws, io, k, idx);
 }
 
 // Q18: a non-finite score makes the state a zero-contribution state
