@@ -89,7 +89,7 @@ namespace {
 
 struct Layout {
   size_t x, g, fp, pix, sig, killed, y, gy, fy, pixy, sigy, kind, accepted, weight, order, blockcnt, blockoff, partial, ctr;
-  size_t q, hits, ring, rec, rec2, rec3, adj, pinfo, gradlist, ctl;   // evaluation workspace (dr_eval.cuh EvalWs)
+  size_t q, hits, ring, rec, vrec, adj, pinfo, gradlist, ctl;   // evaluation workspace (dr_eval.cuh EvalWs)
   size_t total;
 };
 
@@ -120,9 +120,8 @@ Layout make_layout(uint32_t N, uint32_t planes, uint32_t Lseg, bool grad, bool n
   L.q = take(6 * sizeof(float4) * (size_t)N);           // qa | qb, or the 64-byte ray records of k_wave
   L.hits = take(sizeof(uint2) * (size_t)N);
   L.ring = take(sizeof(uint2) * (size_t)N * (nee ? 2 * Lseg - 1 : Lseg));   // one entry per ray of an evaluation, never reused (dr_wave.cuh)
-  L.rec = take(grad ? sizeof(float4) * (size_t)N * (Lseg + (nee ? 1 : 0)) : 0);
-  L.rec2 = take(grad && nee ? sizeof(float4) * (size_t)N * (Lseg + 1) : 0);
-  L.rec3 = take(grad && nee ? sizeof(float4) * (size_t)N * (Lseg + 1) : 0);
+  L.rec = take(grad ? sizeof(float4) * (size_t)N * (nee ? 1 : Lseg) : 0);
+  L.vrec = take(grad && nee ? 3 * sizeof(float4) * (size_t)N * Lseg : 0);
   L.adj = take(grad && nee ? sizeof(float4) * (size_t)N * 3 : 0);
   L.pinfo = take(grad ? 4 * (size_t)N : 0);
   L.gradlist = take(grad ? 4 * (size_t)N * (nee ? 3 * Lseg : 1) : 0);   // with next-event estimation: one list per (vertex index, material kind)
@@ -238,7 +237,7 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
   if (grad) {
     ProfScope ps(prof, DR_PROF_GRAD, s);
     if (dev.nee) {   // one launch per vertex index and material kind, last vertex first (dr_grad.cuh)
-      k_grad_nee_init<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io, n);
+      k_grad_nee_init<<<(n + kGradInitBlock - 1) / kGradInitBlock, kGradInitBlock, 0, s>>>(dev, ws, io, n);
       const uint32_t gv = (n + kGradVertexBlock - 1) / kGradVertexBlock + 3;   // three lists, each rounded up to whole blocks
       for (uint32_t k = dev.L - 1; k >= 1; --k) k_grad_nee_vertex<<<gv, kGradVertexBlock, 0, s>>>(dev, ws, io, k);
       k_grad_nee_finish<<<(n + kGradBlock - 1) / kGradBlock, kGradBlock, 0, s>>>(dev, ws, io, n);
@@ -317,8 +316,8 @@ struct HookEval {
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o = align256(o + bytes); return at; };
     const bool gn = grad && sc->dev.nee;
-    const size_t q = take(96 * N), hits = take(8 * N), ring = take(8 * wave_ring_entries(sc->dev, N)), rec = take(grad ? 16 * N * (L + (gn ? 1 : 0)) : 0),
-                 rec2 = take(gn ? 16 * N * (L + 1) : 0), rec3 = take(gn ? 16 * N * (L + 1) : 0), adj = take(gn ? 48 * N : 0),
+    const size_t q = take(96 * N), hits = take(8 * N), ring = take(8 * wave_ring_entries(sc->dev, N)), rec = take(grad ? 16 * N * (gn ? 1 : L) : 0),
+                 vrec = take(gn ? 48 * N * L : 0), adj = take(gn ? 48 * N : 0),
                  pinfo = take(grad ? 4 * N : 0), gl = take(grad ? 4 * N * (sc->dev.nee ? 3 * L : 1) : 0), ctl = take(4 * kCtlWords);
     cudaError_t e = ws_mem.alloc(o);
     if (e == cudaSuccess) e = xpl.alloc(16 * N * sc->dev.planes);
@@ -327,8 +326,8 @@ struct HookEval {
     if (e != cudaSuccess) return e;
     char* b = ws_mem.as<char>();
     ws.qa = (float4*)(b + q); ws.qb = ws.qa + 3 * N; ws.hits = (uint2*)(b + hits); ws.ring = (uint2*)(b + ring); ws.rec = (float4*)(b + rec);
-    ws.rec2 = (float4*)(b + rec2); ws.rec3 = (float4*)(b + rec3); ws.adj = (float4*)(b + adj);
-    ws.pinfo = (uint32_t*)(b + pinfo); ws.gradlist = (uint32_t*)(b + gl); ws.ctl = (uint32_t*)(b + ctl); ws.cap = n;
+    ws.vrec = (float4*)(b + vrec); ws.adj = (float4*)(b + adj);
+    ws.pinfo = grad ? (uint32_t*)(b + pinfo) : nullptr; ws.gradlist = (uint32_t*)(b + gl); ws.ctl = (uint32_t*)(b + ctl); ws.cap = n;
     ws.tag = 1;
     return cudaMemsetAsync(ws.ring, 0, 8 * wave_ring_entries(sc->dev, N), stream);   // fresh memory: no entry carries tag 1
   }
@@ -558,8 +557,8 @@ dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_stat
   h->state_bytes = L.total; h->state_base = dev_state;
   EvalWs& ws = h->ws;
   ws.qa = (float4*)(b + L.q); ws.qb = ws.qa + 3 * (size_t)cp.N; ws.hits = (uint2*)(b + L.hits); ws.ring = (uint2*)(b + L.ring);
-  ws.rec = (float4*)(b + L.rec); ws.rec2 = (float4*)(b + L.rec2); ws.rec3 = (float4*)(b + L.rec3); ws.adj = (float4*)(b + L.adj);
-  ws.pinfo = (uint32_t*)(b + L.pinfo); ws.gradlist = (uint32_t*)(b + L.gradlist); ws.ctl = (uint32_t*)(b + L.ctl); ws.cap = cp.N;
+  ws.rec = (float4*)(b + L.rec); ws.vrec = (float4*)(b + L.vrec); ws.adj = (float4*)(b + L.adj);
+  ws.pinfo = cp.grad ? (uint32_t*)(b + L.pinfo) : nullptr; ws.gradlist = (uint32_t*)(b + L.gradlist); ws.ctl = (uint32_t*)(b + L.ctl); ws.cap = cp.N;
   *out = h;
   return DR_OK;
 }

@@ -73,12 +73,14 @@ struct EvalWs {
   uint2* hits;         // cap: (bits(t), triangle in leaf order or kMiss)   (loop form)
   uint2* ring;         // wave_ring_entries() ray entries, written once per evaluation, never reused      (k_wave)
   float4* rec;         // L * cap (score only): incoming direction and triangle of vertex k of state s at [k * cap + s]
-                       //   next-event estimation: (L + 1) planes, the terminal emitter hit of a path is recorded too, and the
-                       //   vertex' material kind sits in bits 30-31 of the triangle word; plane 0 = (masks, segments, terminal, vertices)
-  float4* rec2;        // (L + 1) * cap, next-event estimation + score: (origin of the ray that reached vertex k, density of its direction)
-  float4* rec3;        // (L + 1) * cap, next-event estimation + score: (throughput before vertex k, 0)
-  float4* adj;         // 3 * cap, next-event estimation + score: adjoints between the steps of the reverse sweep (dr_grad.cuh)
-  uint32_t* pinfo;     // cap (score only): refract mask | rays << 16 of the finished path
+                       //   next-event estimation: cap entries, the header of a finished path (masks, segments, terminal triangle, vertices)
+  float4* vrec;        // next-event estimation + score: 3 * L * cap, the 48-byte record of the ray that reached vertex k = 1 .. L of
+                       //   state s at [3 ((k - 1) cap + s)]: (direction, triangle | material kind << 30) (origin, density of the
+                       //   direction) (throughput before the vertex, material index); the terminal emitter hit of a path is recorded too
+  float4* adj;         // next-event estimation + score: 3 * cap, the 48-byte adjoint record of state s between the launches of
+                       //   the reverse sweep at [3 s] (dr_grad.cuh)
+  uint32_t* pinfo;     // cap (score only, else null): refract mask | rays << 16 of the finished path; with next-event estimation: the
+                       //   material kinds of the path's vertices, two bits each (vertex k at bits 2 (k - 1)), OR-ed in by the shading
   uint32_t* gradlist;  // cap (score only); 3 * L * cap with next-event estimation: list (vertex index k, material kind) at [(3 k + kind) * cap, ...)
   uint32_t* ctl;       // kCtlWords
   uint32_t cap;
@@ -147,6 +149,7 @@ __global__ void __launch_bounds__(kShadeBlock) k_raygen(DevScene sc, EvalWs ws, 
     r[0] = q0; r[1] = q1; r[2] = q2;
     if (sc.nee) {
       r[3] = make_float4(0.f, 0.f, 0.f, -1.f);          // the camera ray has no direction density
+      if (ws.pinfo) ws.pinfo[s] = 0u;                    // vertex kinds of this path (record_vertex)
       io.f[s] = make_float4(0.f, 0.f, 0.f, 0.f);        // emitter connections accumulate here
       if (io.nrays) io.nrays[s] = 0u;
     }
@@ -374,7 +377,6 @@ struct ShadeOut {
   float3 sh_o, sh_d, cpend;
   float sh_len;          // distance from sh_o to the sampled emitter point
   uint32_t light_id, lobe;
-  uint32_t nv;           // sampling vertices of a path that ended here (bin of the reverse-pass list)
   bool cont, shadow, want_grad;
 };
 
@@ -404,12 +406,14 @@ __device__ __forceinline__ void finish_path(const DevScene& sc_, const EvalWs& w
 }
 
 // next-event estimation + score: what the reverse sweep (dr_grad.cuh) needs of the ray that reached vertex k
+__device__ __forceinline__ size_t vrec_at(const EvalWs& ws, uint32_t k, uint32_t s) { return 3 * ((size_t)(k - 1u) * ws.cap + s); }
 __device__ __forceinline__ void record_vertex(const EvalWs& ws, uint32_t k, uint32_t s, float3 o, float3 d, uint32_t li, uint32_t kind,
-                                              float pb_prev, float T0, float T1, float T2) {
-  const size_t at = (size_t)k * ws.cap + s;
-  __stcs(&ws.rec[at], make_float4(d.x, d.y, d.z, __uint_as_float(li | (kind << 30))));
-  __stcs(&ws.rec2[at], make_float4(o.x, o.y, o.z, pb_prev));
-  __stcs(&ws.rec3[at], make_float4(T0, T1, T2, 0.f));
+                                              uint32_t mi, float pb_prev, float T0, float T1, float T2) {
+  float4* r = ws.vrec + vrec_at(ws, k, s);   // written once, read by the reverse sweep only: evict first
+  __stcs(r, make_float4(d.x, d.y, d.z, __uint_as_float(li | (kind << 30))));
+  __stcs(r + 1, make_float4(o.x, o.y, o.z, pb_prev));
+  __stcs(r + 2, make_float4(T0, T1, T2, __uint_as_float(mi)));
+  if (kind < 3u) atomicOr(&ws.pinfo[s], kind << (2u * (k - 1u)));   // no return value: a reduction at L2
 }
 
 template <bool GRAD, bool NEE>
@@ -445,7 +449,7 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
         const float4 m2 = __ldg(&sc.mats[3 * mi + 2]);
         const V3<float> ov{o.x, o.y, o.z}, dv{d.x, d.y, d.z};
         const float w_b = emitter_weight<float, NEE>(sc, xyz(t0), fr.nf, ov, dv, pb_prev, pb_prev >= 0.f);   // dn < 0: nf = n
-        if (GRAD && NEE && sc.nee) record_vertex(ws, k, s, o, d, li, 3u, pb_prev, T0, T1, T2);   // the reverse sweep starts here
+        if (GRAD && NEE && sc.nee) record_vertex(ws, k, s, o, d, li, 3u, mi, pb_prev, T0, T1, T2);   // the reverse sweep starts here
         f0 = T0 * m1.z * w_b; f1 = T1 * m1.w * w_b; f2 = T2 * m2.x * w_b;
       } else {
         sig = fnv(sig, 5u);
@@ -454,7 +458,7 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
     } else if (k < sc.L) {
       term = kTermNone;
       const float4 u = x_vertex(sc, io, s, k);
-      if (GRAD && NEE && sc.nee) record_vertex(ws, k, s, o, d, li, kind, pb_prev, T0, T1, T2);
+      if (GRAD && NEE && sc.nee) record_vertex(ws, k, s, o, d, li, kind, mi, pb_prev, T0, T1, T2);
       else if (GRAD) __stcs(&ws.rec[(size_t)k * cap + s], make_float4(d.x, d.y, d.z, __uint_as_float(li)));   // written once, read by k_grad only: evict first
       const V3<float> ov{o.x, o.y, o.z}, dv{d.x, d.y, d.z};
       VertexOut<float> vo;
@@ -494,7 +498,6 @@ __device__ __forceinline__ void shade_vertex(const DevScene& sc, const EvalWs& w
       term = kTermNone;   // length cap on a surface: nothing is added
     }
   }
-  out.nv = k - 1u;
   if (done) finish_path<NEE>(sc, ws, io, k, s, f0, f1, f2, sig, info, k - 1u, term, GRAD, out.want_grad, bad);
 }
 

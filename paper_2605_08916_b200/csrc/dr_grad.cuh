@@ -31,10 +31,10 @@ struct VtxFrozen {     // what the replay fixes for one vertex
   bool reflect, vis;
 };
 
-__device__ __forceinline__ void load_vertex(const DevScene& sc, uint32_t li, float3 d, VtxFrozen& f) {
+// mi: the triangle's material index, known from the vertex record so that triangle and material arrive together
+__device__ __forceinline__ void load_vertex(const DevScene& sc, uint32_t li, uint32_t mi, float3 d, VtxFrozen& f) {
   const float4 t0 = __ldg(&sc.tris[3 * li]), t1 = __ldg(&sc.tris[3 * li + 1]), t2 = __ldg(&sc.tris[3 * li + 2]);
   const float3 e1 = make_float3(t0.w, t1.x, t1.y), e2 = make_float3(t1.z, t1.w, t2.x);
-  const uint32_t mi = __float_as_uint(t2.z);
   f.m0 = __ldg(&sc.mats[3 * mi]); f.m1 = __ldg(&sc.mats[3 * mi + 1]);
   f.kind = __float_as_uint(f.m0.x);
   f.v0 = xyz(t0);
@@ -96,36 +96,51 @@ constexpr uint32_t kRecLiMask = 0x3FFFFFFFu;   // ws.rec[k].w = triangle (leaf o
 // list of the paths whose vertex k has material `kind`: entries ws.gradlist[(3 k + kind) * cap ...], count ws.ctl[kCtlGradKind + 3 k + kind]
 __device__ __forceinline__ uint32_t grad_list(uint32_t k, uint32_t kind) { return 3u * k + kind; }
 
-// Per state, in index order (the shading wrote f, the header ws.rec[s] and the vertex records of every finished path):
-// what the path's last ray found -- R (radiance per unit throughput) and the adjoints of that ray -- and the path's vertices
-// onto the (k, kind) lists, one atomic per warp, list and vertex index.
-__global__ void __launch_bounds__(kGradBlock) k_grad_nee_init(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
-  const uint32_t s = blockIdx.x * kGradBlock + threadIdx.x;
+// Per state, in index order (the shading wrote f, the header ws.rec[s], the vertex records and the vertex kinds ws.pinfo[s] of
+// every finished path): the path's vertices go onto the (k, kind) lists -- counted per block in shared memory, one atomic per
+// block and list -- and what the path's last ray found, R (radiance per unit throughput) and the adjoints of that ray, goes
+// into ws.adj.
+constexpr int kGradInitBlock = 256;
+constexpr int kGradLists = 3 * kMaxPathLen;
+__global__ void __launch_bounds__(kGradInitBlock) k_grad_nee_init(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
+  __shared__ uint32_t s_cnt[kGradInitBlock / 32][kGradLists];   // entries of warp w for list j; then their offset in the list
+  const uint32_t s = blockIdx.x * kGradInitBlock + threadIdx.x;
   const size_t cap = ws.cap;
-  const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
+  const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5, lt = (1u << lane) - 1u;
   const bool listed = s < n && io.f[s].w > 0.f;   // finish_path: p > 0
-  uint32_t nv = 0, term = kTermNone;
-  if (s < n) ws.pinfo[s] = 0u;   // "score not finite" flag of this evaluation
+  uint32_t nv = 0, term = kTermNone, kinds = 0;
   if (listed) {
     const float4 hdr = ws.rec[s];
     term = __float_as_uint(hdr.z); nv = __float_as_uint(hdr.w);
+    kinds = ws.pinfo[s];
   }
   {
     const unsigned lm = __ballot_sync(0xFFFFFFFFu, listed);
     if (lane == 0 && lm && io.grad_ctr) atomicAdd(io.grad_ctr, (unsigned long long)__popc(lm));
   }
+  for (uint32_t j = lane; j < (uint32_t)kGradLists; j += 32) s_cnt[wid][j] = 0;
+  __syncwarp();
   const uint32_t kmax = __reduce_max_sync(0xFFFFFFFFu, nv);
   for (uint32_t k = 1; k <= kmax; ++k) {
-    const uint32_t kind = k <= nv ? (__float_as_uint(ws.rec[(size_t)k * cap + s].w) >> 30) : 3u;
+    const uint32_t kind = k <= nv ? ((kinds >> (2u * (k - 1u))) & 3u) : 3u;
 #pragma unroll
     for (uint32_t q = 0; q < 3; ++q) {
       const unsigned m = __ballot_sync(0xFFFFFFFFu, kind == q);
-      if (!m) continue;
-      uint32_t base = 0;
-      if (lane == (unsigned)(__ffs(m) - 1)) base = atomicAdd(&ws.ctl[kCtlGradKind + grad_list(k, q)], (uint32_t)__popc(m));
-      base = __shfl_sync(0xFFFFFFFFu, base, __ffs(m) - 1);
-      if (kind == q) ws.gradlist[(size_t)grad_list(k, q) * cap + base + __popc(m & lt)] = s;
+      if (lane == 0) s_cnt[wid][grad_list(k, q)] = __popc(m);
     }
+  }
+  __syncthreads();
+  if (threadIdx.x < kGradLists) {   // one thread per list: the block's entries, one atomic, the warps' offsets
+    uint32_t tot = 0;
+    for (int w = 0; w < kGradInitBlock / 32; ++w) tot += s_cnt[w][threadIdx.x];
+    uint32_t base = tot ? atomicAdd(&ws.ctl[kCtlGradKind + threadIdx.x], tot) : 0u;
+    for (int w = 0; w < kGradInitBlock / 32; ++w) { const uint32_t c = s_cnt[w][threadIdx.x]; s_cnt[w][threadIdx.x] = base; base += c; }
+  }
+  __syncthreads();
+  for (uint32_t k = 1; k <= kmax; ++k) {
+    const uint32_t kind = k <= nv ? ((kinds >> (2u * (k - 1u))) & 3u) : 3u;
+    const unsigned m = __ballot_sync(0xFFFFFFFFu, kind < 3u) & __match_any_sync(0xFFFFFFFFu, kind);   // the lanes of my kind
+    if (kind < 3u) ws.gradlist[(size_t)grad_list(k, kind) * cap + s_cnt[wid][grad_list(k, kind)] + __popc(m & lt)] = s;
   }
   if (!listed) return;
   float3 R = make_float3(0.f, 0.f, 0.f), ob = R, db = R;
@@ -133,8 +148,8 @@ __global__ void __launch_bounds__(kGradBlock) k_grad_nee_init(DevScene sc, EvalW
   if (term == kMiss) {
     R = make_float3(sc.env[0], sc.env[1], sc.env[2]);
   } else if (term != kTermNone) {
-    const size_t at = (size_t)(nv + 1) * cap + s;   // the emitter hit was recorded as vertex nv + 1
-    const float4 rD = ws.rec[at], rO = ws.rec2[at], rT = ws.rec3[at];
+    const float4* vr = ws.vrec + vrec_at(ws, nv + 1, s);   // the emitter hit was recorded as vertex nv + 1
+    const float4 rD = vr[0], rO = vr[1], rT = vr[2];
     const float4 t0 = __ldg(&sc.tris[3 * term]), t1 = __ldg(&sc.tris[3 * term + 1]), t2 = __ldg(&sc.tris[3 * term + 2]);
     const float3 e1 = make_float3(t0.w, t1.x, t1.y), e2 = make_float3(t1.z, t1.w, t2.x);
     const uint32_t mi = __float_as_uint(t2.z);
@@ -156,9 +171,10 @@ __global__ void __launch_bounds__(kGradBlock) k_grad_nee_init(DevScene sc, EvalW
       R = make_float3(le.x * wb, le.y * wb, le.z * wb);
     }
   }
-  ws.adj[s] = make_float4(R.x, R.y, R.z, ob.x);
-  ws.adj[cap + s] = make_float4(ob.y, ob.z, db.x, db.y);
-  ws.adj[2 * cap + s] = make_float4(db.z, pbb, 0.f, 0.f);
+  float4* aj = ws.adj + 3 * (size_t)s;
+  aj[0] = make_float4(R.x, R.y, R.z, ob.x);
+  aj[1] = make_float4(ob.y, ob.z, db.x, db.y);
+  aj[2] = make_float4(db.z, pbb, 0.f, 0.f);   // .w: "score not finite" flag of the sweep
 }
 
 #ifndef DR_GRAD_MIN_BLOCKS
@@ -173,15 +189,16 @@ template <int KIND>
 __device__ __forceinline__ void grad_vertex(const DevScene& sc, const EvalWs& ws, const EvalIO& io, uint32_t k, uint32_t idx) {
   const size_t cap = ws.cap;
   const uint32_t s = ws.gradlist[(size_t)grad_list(k, KIND) * cap + idx];
-  const size_t at = (size_t)k * cap + s;
-  const float4 rD = ws.rec[at], rO = ws.rec2[at], rT = ws.rec3[at];
+  const float4* vr = ws.vrec + vrec_at(ws, k, s);
+  float4* aj = ws.adj + 3 * (size_t)s;
+  const float4 rD = vr[0], rO = vr[1], rT = vr[2];
   const uint32_t info = __float_as_uint(ws.rec[s].x);
-  const float4 a0 = ws.adj[s], a1 = ws.adj[cap + s], a2 = ws.adj[2 * cap + s];
+  const float4 a0 = aj[0], a1 = aj[1], a2 = aj[2];
   float3 R = make_float3(a0.x, a0.y, a0.z), ob = make_float3(a0.w, a1.x, a1.y), db = make_float3(a1.z, a1.w, a2.x);
   const float pbb = a2.y;
   const float3 o = xyz(rO), d = xyz(rD);
   VtxFrozen f;
-  load_vertex(sc, __float_as_uint(rD.w) & kRecLiMask, d, f);
+  load_vertex(sc, __float_as_uint(rD.w) & kRecLiMask, __float_as_uint(rT.w), d, f);
   f.reflect = !((info >> k) & 1u);
   f.vis = ((info >> (16u + k)) & 1u) != 0u;
   const float inv_phat = 1.0f / (io.f[s].w + kEps);
@@ -221,9 +238,9 @@ __device__ __forceinline__ void grad_vertex(const DevScene& sc, const EvalWs& ws
   ob = make_float3(go.x, go.y, go.z);
   db = make_float3(gd.x, gd.y, gd.z);
   if (k > 1u) {   // a vertex that samples does not use the density of the ray that reached it: pb_bar = 0
-    ws.adj[s] = make_float4(R.x, R.y, R.z, ob.x);
-    ws.adj[cap + s] = make_float4(ob.y, ob.z, db.x, db.y);
-    ws.adj[2 * cap + s] = make_float4(db.z, 0.f, 0.f, 0.f);
+    aj[0] = make_float4(R.x, R.y, R.z, ob.x);
+    aj[1] = make_float4(ob.y, ob.z, db.x, db.y);
+    aj[2] = make_float4(db.z, 0.f, 0.f, (bad || a2.w != 0.f) ? 1.f : 0.f);
   } else {        // the camera: its position is fixed, only the direction depends on the film point
     float ga = 0.f, gb = 0.f;
     if (db.x != 0.f || db.y != 0.f || db.z != 0.f) {
@@ -234,8 +251,8 @@ __device__ __forceinline__ void grad_vertex(const DevScene& sc, const EvalWs& ws
     }
     bad = bad || !(isfinite(ga) && isfinite(gb));
     io.g[s] = make_float4(ga, gb, 0.f, 0.f);
+    if (bad || a2.w != 0.f) aj[2] = make_float4(0.f, 0.f, 0.f, 1.f);
   }
-  if (bad) ws.pinfo[s] = 1u;
 }
 
 // One launch per vertex index: the blocks are dealt to the three lists of that index in turn (list lengths are known on the
@@ -256,7 +273,7 @@ __global__ void __launch_bounds__(kGradVertexBlock, DR_GRAD_MIN_BLOCKS) k_grad_n
 // Q18: a non-finite score makes the state a zero-contribution state
 __global__ void __launch_bounds__(kGradBlock) k_grad_nee_finish(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
   const uint32_t s = blockIdx.x * kGradBlock + threadIdx.x;
-  if (s >= n || !ws.pinfo[s]) return;
+  if (s >= n || !(io.f[s].w > 0.f) || ws.adj[3 * (size_t)s + 2].w == 0.f) return;
   const uint32_t nv = __float_as_uint(ws.rec[s].w);
   io.f[s] = make_float4(0.f, 0.f, 0.f, 0.f);
   for (uint32_t k = 0; k <= nv; ++k) io.g[(size_t)k * io.stride + s] = make_float4(0.f, 0.f, 0.f, 0.f);

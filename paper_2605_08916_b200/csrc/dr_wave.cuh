@@ -288,7 +288,7 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
     const bool phase_b = (pay >> 31) != 0u;
     float4* rec = ws.qa + kRecWords * (size_t)s;
     bool want_grad = false, push = false;     // push: this lane publishes a queue entry (`entry`)
-    uint32_t entry = 0, grad_bin = 0;
+    uint32_t entry = 0;
     if (mine && !phase_b) {
       const float4 Q0 = __ldcg(rec), Q1 = __ldcg(rec + 1), Q2 = __ldcg(rec + 2);
       const float pb_prev = NEE ? __ldcg(rec + 3).w : -1.f;
@@ -299,7 +299,6 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
       ShadeOut so;
       shade_vertex<GRAD, NEE>(sc, ws, io, k, Q0, Q1, Q2, pb_prev, h, s, so, bad);
       want_grad = so.want_grad;
-      grad_bin = so.nv;
       if (so.cont || so.shadow) {
         __stcg(rec, so.n0); __stcg(rec + 1, so.n1); __stcg(rec + 2, so.n2);
         if (NEE) __stcg(rec + 3, make_float4(so.cpend.x, so.cpend.y, so.cpend.z, so.pb_next));
@@ -326,7 +325,6 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
       const uint32_t sig = fnv(fnv(__float_as_uint(Q1.w), vis ? 7u : 6u), aim >> 28);
       if (Q2.x == 0.f && Q2.y == 0.f && Q2.z == 0.f) {         // the direction sample had zero weight: the path ends here
         finish_path<NEE>(sc, ws, io, k, s, 0.f, 0.f, 0.f, sig, info, k, kTermNone, GRAD, want_grad, bad);
-        grad_bin = k;
       } else {
         __stcg(rec + 1, make_float4(Q1.x, Q1.y, Q1.z, __uint_as_float(sig)));
         __stcg(rec + 2, make_float4(Q2.x, Q2.y, Q2.z, __uint_as_float(info)));
