@@ -163,8 +163,8 @@ void prof_drain(dr_chains* c) {
   for (size_t k = 0; k < c->ev_used; ++k) {
     float ms = 0.f;
     if (cudaEventElapsedTime(&ms, c->ev[2 * k], c->ev[2 * k + 1]) == cudaSuccess) {
-      c->prof_ms[c->ev_kind[k]] += ms;
-      c->prof_launches[c->ev_kind[k]] += 1;
+      c->prof_ms[c->ev_kind[k] & 0xFF] += ms;
+      c->prof_launches[c->ev_kind[k] & 0xFF] += (uint64_t)(c->ev_kind[k] >> 8);   // kernel launches inside the pair
     }
   }
   c->ev_used = 0;
@@ -172,13 +172,13 @@ void prof_drain(dr_chains* c) {
 
 struct ProfScope {
   dr_chains* c; cudaStream_t s; size_t k; bool on;
-  ProfScope(dr_chains* c_, int kind, cudaStream_t s_) : c(c_), s(s_), k(0), on(c_ && c_->profiling) {
+  ProfScope(dr_chains* c_, int kind, cudaStream_t s_, int launches = 1) : c(c_), s(s_), k(0), on(c_ && c_->profiling) {
     if (!on) return;
     if (c->ev_used == kMaxPairs) { cudaStreamSynchronize(s); prof_drain(c); }
     k = c->ev_used++;
     while (c->ev.size() < 2 * (k + 1)) { cudaEvent_t e; cudaEventCreate(&e); c->ev.push_back(e); }
     if (c->ev_kind.size() <= k) c->ev_kind.resize(k + 1);
-    c->ev_kind[k] = kind;
+    c->ev_kind[k] = kind | (launches << 8);
     cudaEventRecord(c->ev[2 * k], s);
   }
   ~ProfScope() { if (on) cudaEventRecord(c->ev[2 * k + 1], s); }
@@ -235,7 +235,7 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
     }
   }
   if (grad) {
-    ProfScope ps(prof, DR_PROF_GRAD, s);
+    ProfScope ps(prof, DR_PROF_GRAD, s, dev.nee ? (int)dev.L + 1 : 1);   // with next-event estimation: init, L - 1 vertex launches, finish
     if (dev.nee) {   // one launch per vertex index and material kind, last vertex first (dr_grad.cuh)
       k_grad_nee_init<<<(n + kGradInitBlock - 1) / kGradInitBlock, kGradInitBlock, 0, s>>>(dev, ws, io, n);
       const uint32_t gv = (n + kGradVertexBlock - 1) / kGradVertexBlock + 3;   // three lists, each rounded up to whole blocks
