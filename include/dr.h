@@ -219,8 +219,10 @@ dr_status dr_trace_rays(const dr_scene* scene, const float* dev_o, const float* 
 dr_status dr_eval_states(const dr_scene* scene, const float* dev_x, uint32_t n, float* dev_f, float* dev_p,
                          uint32_t* dev_pix, float* dev_score, uint32_t* dev_nrays, uint32_t* dev_sig, void* stream);
 /* The same, choosing the form of rows a3-a5 (identical results, state by state): 0 = default, 1 = one k_trace + k_shade
- * launch per segment, 2 = one persistent k_wave launch (csrc/dr_wave.cuh).  dr_chains_set_eval_form does the same for
- * the evaluations inside dr_chains_init / dr_step. */
+ * launch per segment, 2 = one persistent k_wave launch (csrc/dr_wave.cuh) in the block shape the default would take for n
+ * states, 3 / 4 = k_wave in its small / big block shape (640 threads with two triangle slots per lane below 400 000
+ * states -- 160 000 with next-event estimation --, 768 threads with one above: csrc/dr_eval.cuh).  dr_chains_set_eval_form does the same for the evaluations inside
+ * dr_chains_init / dr_step. */
 dr_status dr_eval_states_form(const dr_scene* scene, const float* dev_x, uint32_t n, float* dev_f, float* dev_p,
                               uint32_t* dev_pix, float* dev_score, uint32_t* dev_nrays, uint32_t* dev_sig, int32_t form,
                               void* stream);

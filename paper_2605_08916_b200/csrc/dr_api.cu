@@ -79,7 +79,7 @@ struct dr_chains {
   uint64_t prof_launches[DR_PROF_COUNT] = {};
   EvalWs ws{};
   uint32_t eval_tag = 0;           // k_wave: tag of the last evaluation (dr_wave.cuh)
-  int eval_form = 0;               // test hook dr_chains_set_eval_form: 0 = default choice, 1 = per-segment loop, 2 = k_wave
+  int eval_form = 0;               // test hook dr_chains_set_eval_form: 0 = default choice, 1 = per-segment loop, 2 = k_wave, 3 / 4 = k_wave in the small / big block shape
   void* hook_scratch = nullptr;    // device staging of dr_chains_download / _upload (row-major copies), allocated on first use
   void* d_rho = nullptr;           // f4: (probability, running sum) per film tile
   ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); cudaFree(hook_scratch); cudaFree(d_rho); }
@@ -186,7 +186,36 @@ struct ProfScope {
 
 // Rows a3-a6 for n states (dr_eval.cuh): raygen, then trace + shade of every segment, then the reverse pass.
 // prof may be null (test hooks).  io.g must be zero on entry when grad is set.  form: 0 = default (one persistent
-// k_wave launch; the per-segment loop for the counting pass and for very large n), 1 = loop, 2 = k_wave.
+// k_wave launch, in the small block shape below kWaveSmallBelow states; the per-segment loop for the counting pass and for very
+// large n), 1 = loop, 2 = k_wave, 3 / 4 = k_wave in the small / big block shape.
+// shared memory of a traversal block of `block` threads: one constant word + per-thread node and triangle stacks
+size_t trace_stack_bytes(uint32_t stack_cap, int block) {
+  return ((size_t)(stack_cap + kTriStack) * sizeof(uint2) + (size_t)kTriStack * sizeof(uint32_t)) * block + 16;
+}
+
+// k_wave in the block shape C (dr_eval.cuh TraceBig / TraceSmall)
+template <class C>
+void launch_wave(const DevScene& dev, const EvalWs& ws, const EvalIO& io, uint32_t n, bool grad, bool stats, int n_sm, cudaStream_t s) {
+  const size_t sm = trace_stack_bytes(dev.stack_cap, C::kBlock) + kWaveExtraSmem;
+  if (dev.nee) {
+    if (stats) {   // the counting pass of a scene with next-event estimation (others count in k_trace<true>)
+      if (grad) k_wave<true, true, true, C><<<n_sm, C::kBlock, sm, s>>>(dev, ws, io, n);
+      else k_wave<false, true, true, C><<<n_sm, C::kBlock, sm, s>>>(dev, ws, io, n);
+    } else if (grad) k_wave<true, false, true, C><<<n_sm, C::kBlock, sm, s>>>(dev, ws, io, n);
+    else k_wave<false, false, true, C><<<n_sm, C::kBlock, sm, s>>>(dev, ws, io, n);
+  } else if (grad) k_wave<true, false, false, C><<<n_sm, C::kBlock, sm, s>>>(dev, ws, io, n);
+  else k_wave<false, false, false, C><<<n_sm, C::kBlock, sm, s>>>(dev, ws, io, n);
+}
+template <class C>
+cudaError_t wave_allow_smem() {
+  const void* waves[] = {(const void*)k_wave<false, false, false, C>, (const void*)k_wave<true, false, false, C>, (const void*)k_wave<false, false, true, C>,
+                         (const void*)k_wave<true, false, true, C>, (const void*)k_wave<false, true, true, C>, (const void*)k_wave<true, true, true, C>};
+  cudaError_t e = cudaSuccess;
+  for (const void* w : waves)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(w, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  return e;
+}
+
 dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const EvalIO& io, uint32_t n, bool grad, bool stats,
                       int form, cudaStream_t s) {
   const DevScene& dev = sc->dev;
@@ -198,8 +227,9 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
     CUDA_TRY(cudaGetLastError());
     return DR_OK;
   }
+  if (form < 0 || form > 4) return fail(DR_ERR_INVALID_ARG, "evaluation form must be 0 .. 4");
   if (dev.nee && (!sc->wave_ok || form == 1)) return fail(DR_ERR_UNSUPPORTED, "next-event estimation runs in k_wave only (no per-segment loop)");
-  const bool wave = dev.nee || (!stats && sc->wave_ok && (form == 2 || (form == 0 && n < kWaveMaxStates)));
+  const bool wave = dev.nee || (!stats && sc->wave_ok && (form >= 2 || (form == 0 && n < kWaveMaxStates)));
   CUDA_TRY(cudaMemsetAsync(ws.ctl, 0, 4 * kCtlWords, s));
   {
     ProfScope ps(prof, DR_PROF_RAYGEN, s);
@@ -211,15 +241,9 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
 #endif
   if (wave) {
     ProfScope ps(prof, DR_PROF_TRACE, s);
-    const size_t sm = sc->trace_smem + kWaveExtraSmem;
-    if (dev.nee) {
-      if (stats) {   // the counting pass of a scene with next-event estimation (others count in k_trace<true>)
-        if (grad) k_wave<true, true, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
-        else k_wave<false, true, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
-      } else if (grad) k_wave<true, false, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
-      else k_wave<false, false, true><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
-    } else if (grad) k_wave<true, false, false><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
-    else k_wave<false, false, false><<<sc->n_sm, kTraceBlock, sm, s>>>(dev, ws, io, n);
+    const bool small = form == 3 || (form != 4 && n < (dev.nee ? kWaveSmallBelowNee : kWaveSmallBelow));
+    if (small) launch_wave<TraceSmall>(dev, ws, io, n, grad, stats, sc->n_sm, s);
+    else launch_wave<TraceBig>(dev, ws, io, n, grad, stats, sc->n_sm, s);
   } else
   for (uint32_t k = 1; k <= dev.L; ++k) {
     const float4* q = (k & 1u) ? ws.qa : ws.qb;
@@ -396,19 +420,17 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   dev.nodes = (const uint4*)s->d_nodes; dev.tris = (const float4*)s->d_tris; dev.mats = (const float4*)s->d_mats;
   dev.n_nodes = (uint32_t)bvh.nodes.size();
   dev.stack_cap = bvh.depth + 1;  // node groups: at most one per level
-  const size_t stack_bytes = ((size_t)(dev.stack_cap + kTriStack) * sizeof(uint2) + (size_t)kTriStack * sizeof(uint32_t)) * kTraceBlock + 16;  // + the constant word of k_trace
+  const size_t stack_bytes = trace_stack_bytes(dev.stack_cap, std::max(kTraceBlock, TraceSmall::kBlock));
   if (stack_bytes > kMaxDynSmem) {   // (depth + 1) node groups per thread no longer fit the block's shared memory
     dr_scene_destroy(s);
     return fail(DR_ERR_UNSUPPORTED, "BVH8 deeper than the traversal stack allows");
   }
-  s->trace_smem = stack_bytes;
-  s->wave_ok = s->trace_smem + kWaveExtraSmem <= kMaxDynSmem;
+  s->trace_smem = trace_stack_bytes(dev.stack_cap, kTraceBlock);
+  s->wave_ok = stack_bytes + kWaveExtraSmem <= kMaxDynSmem;
   e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
-  const void* waves[] = {(const void*)k_wave<false, false, false>, (const void*)k_wave<true, false, false>, (const void*)k_wave<false, false, true>,
-                         (const void*)k_wave<true, false, true>, (const void*)k_wave<false, true, true>, (const void*)k_wave<true, true, true>};
-  for (const void* w : waves)
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(w, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = wave_allow_smem<TraceBig>();
+  if (e == cudaSuccess) e = wave_allow_smem<TraceSmall>();
   if (e != cudaSuccess) {
     dr_scene_destroy(s);
     return fail(DR_ERR_CUDA, std::string("k_trace shared memory: ") + cudaGetErrorString(e));
@@ -567,7 +589,7 @@ dr_status dr_chains_destroy(dr_chains* c) { delete c; return DR_OK; }
 
 dr_status dr_chains_set_eval_form(dr_chains* c, int32_t form) {
   if (!c) return fail(DR_ERR_INVALID_ARG, "null chains");
-  if (form < 0 || form > 2) return fail(DR_ERR_INVALID_ARG, "form must be 0, 1 or 2");
+  if (form < 0 || form > 4) return fail(DR_ERR_INVALID_ARG, "form must be 0 .. 4");
   c->eval_form = form;
   return DR_OK;
 }
@@ -838,7 +860,7 @@ dr_status dr_eval_states(const dr_scene* sc, const float* x, uint32_t n, float* 
 dr_status dr_eval_states_form(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score,
                               uint32_t* nrays, uint32_t* sig, int32_t form, void* stream) {
   if (!sc) return fail(DR_ERR_INVALID_ARG, "null scene");
-  if (form < 0 || form > 2) return fail(DR_ERR_INVALID_ARG, "form must be 0, 1 or 2");
+  if (form < 0 || form > 4) return fail(DR_ERR_INVALID_ARG, "form must be 0 .. 4");
   if (!n) return DR_OK;  // empty input
   if (!x || !f || !p || !pix || !nrays || !sig) return fail(DR_ERR_INVALID_ARG, "null argument");
   return eval_rows(sc, x, n, f, p, pix, score, nrays, sig, nullptr, form, (cudaStream_t)stream);

@@ -48,6 +48,18 @@ namespace dr {
 constexpr int kTraceBlock = DR_TRACE_BLOCK;   // one persistent block per SM
 constexpr int kTriStack = DR_TRI_STACK;      // postponed triangle groups per ray
 constexpr int kTrisPerStep = DR_TRIS_PER_STEP;    // triangle tests per lockstep step
+// The persistent traversal block comes in two shapes (profiles/r02f_tuning.md).  Big: 768 threads, one prefetched triangle per
+// lane (80 registers): the most resident warps, best throughput, for evaluations that keep every lane supplied.  Small: 640
+// threads, two triangle slots (96 registers): 12 % fewer lockstep steps per ray, for evaluations that wait on the latency of
+// a path's dependent segments (below kWaveSmallBelow states: 25 % faster at 2^14 states, 8 % at 2^18).
+#ifndef DR_TRACE_BLOCK_SMALL
+#define DR_TRACE_BLOCK_SMALL 640
+#endif
+#ifndef DR_TRIS_PER_STEP_SMALL
+#define DR_TRIS_PER_STEP_SMALL 2
+#endif
+struct TraceBig { static constexpr int kBlock = DR_TRACE_BLOCK, kTris = DR_TRIS_PER_STEP; };
+struct TraceSmall { static constexpr int kBlock = DR_TRACE_BLOCK_SMALL, kTris = DR_TRIS_PER_STEP_SMALL; };
 constexpr int kShadeBlock = 256;
 constexpr int kGradBlock = 128;
 constexpr uint32_t kFetchChunk = DR_FETCH_CHUNK;   // rays a warp takes from the queue per atomic
@@ -160,18 +172,18 @@ __global__ void __launch_bounds__(kShadeBlock) k_raygen(DevScene sc, EvalWs ws, 
 }
 
 // ---- a4: closest hit, persistent ---------------------------------------------------------------------------------
-// Per-thread stacks in shared memory, entry e of thread t at base[e * kTraceBlock] (bank = lane: conflict-free).
+// Per-thread stacks in shared memory, entry e of thread t at base[e * BLOCK] (bank = lane: conflict-free).
 // Node groups grow up from entry 0; postponed triangle groups (tx, ty | tm) live in their own kTriStack entries above them.
-struct SmemStack {
+template <int BLOCK> struct SmemStack {
   uint2* base;
-  __device__ __forceinline__ void push(int sp, uint2 v) { base[sp * kTraceBlock] = v; }
-  __device__ __forceinline__ uint2 pop(int sp) const { return base[sp * kTraceBlock]; }
+  __device__ __forceinline__ void push(int sp, uint2 v) { base[sp * BLOCK] = v; }
+  __device__ __forceinline__ uint2 pop(int sp) const { return base[sp * BLOCK]; }
 };
-struct SmemTriStack {
+template <int BLOCK> struct SmemTriStack {
   uint2* base;     // (tx, ty)
   uint32_t* base3; // tm
-  __device__ __forceinline__ void push(int sp, const TravState& s) { base[sp * kTraceBlock] = make_uint2(s.tx, s.ty); base3[sp * kTraceBlock] = s.tm; }
-  __device__ __forceinline__ void pop(int sp, TravState& s) const { const uint2 e = base[sp * kTraceBlock]; s.tx = e.x; s.ty = e.y; s.tm = base3[sp * kTraceBlock]; }
+  __device__ __forceinline__ void push(int sp, const TravState& s) { base[sp * BLOCK] = make_uint2(s.tx, s.ty); base3[sp * BLOCK] = s.tm; }
+  __device__ __forceinline__ void pop(int sp, TravState& s) const { const uint2 e = base[sp * BLOCK]; s.tx = e.x; s.ty = e.y; s.tm = base3[sp * BLOCK]; }
 };
 
 __device__ __forceinline__ void tri_one(const DevScene& sc, TravRay& r, TravState& s) {
@@ -188,26 +200,26 @@ struct TriSlot {
 
 // One lockstep step of the traversal for this lane (parts A, N, T, F of the comment above k_trace).  Returns true if
 // the lane's ray finished in this step (its closest hit is in r; the caller stores it and clears `active`).
-struct TravLane {
+template <int K> struct TravLane {
   TravRay r;
   TravState s;
   uint4 w0, w1, w2, w3, w4;      // words of the node to test next (valid if has_node)
-  TriSlot tri[kTrisPerStep];
+  TriSlot tri[K];
   int tsp;                       // postponed triangle groups
   bool active, has_node;
 };
 
-__device__ __forceinline__ void trav_lane_init(TravLane& L, uint32_t one) {   // an idle lane
+template <int K> __device__ __forceinline__ void trav_lane_init(TravLane<K>& L, uint32_t one) {   // an idle lane
   L.active = false; L.has_node = false; L.tsp = 0;
   trav_setup(L.r, 0.f, 0.f, 0.f, 1.f, 1.f, 1.f, one);
   trav_begin(L.s);
   L.w0 = L.w1 = L.w2 = L.w3 = L.w4 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
-  for (int it = 0; it < kTrisPerStep; ++it) { L.tri[it].li = kMiss; L.tri[it].t0 = L.tri[it].t1 = make_float4(0.f, 0.f, 0.f, 0.f); L.tri[it].t2 = make_float2(0.f, 0.f); }
+  for (int it = 0; it < K; ++it) { L.tri[it].li = kMiss; L.tri[it].t0 = L.tri[it].t1 = make_float4(0.f, 0.f, 0.f, 0.f); L.tri[it].t2 = make_float2(0.f, 0.f); }
 }
 
-template <bool STATS>
-__device__ __forceinline__ bool trav_step(const DevScene& sc, const uint4* smem, SmemStack& st, SmemTriStack& tst, TravLane& L,
+template <bool STATS, int BLOCK, int K>
+__device__ __forceinline__ bool trav_step(const DevScene& sc, const uint4* smem, SmemStack<BLOCK>& st, SmemTriStack<BLOCK>& tst, TravLane<K>& L,
                                           uint32_t& nn, uint32_t& nt) {
   TravRay& r = L.r;
   TravState& s = L.s;
@@ -262,7 +274,7 @@ __device__ __forceinline__ bool trav_step(const DevScene& sc, const uint4* smem,
   }
   // T: triangle tests
 #pragma unroll
-  for (int it = 0; it < kTrisPerStep; ++it) {
+  for (int it = 0; it < K; ++it) {
     const bool valid = tri[it].li != kMiss;
     if (STATS) nt += valid ? 1u : 0u;
     tri_test_bf(tri[it].t0, tri[it].t1, tri[it].t2, tri[it].li, valid, r);  // reads every loaded word (dr_types.h TriPacked)
@@ -271,7 +283,7 @@ __device__ __forceinline__ bool trav_step(const DevScene& sc, const uint4* smem,
   {
     bool have_any = false;
 #pragma unroll
-    for (int it = 0; it < kTrisPerStep; ++it) {
+    for (int it = 0; it < K; ++it) {
       const bool popt = active && s.ty == 0u && tsp > 0;
       tsp -= popt ? 1 : 0;
       if (popt) tst.pop(tsp, s);
@@ -309,14 +321,14 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
   if (threadIdx.x == 0) smem[0].x = 0x3F800000u;   // one 16-byte word in front of the stacks
   __syncthreads();
   const uint32_t one = *(volatile uint32_t*)&smem[0].x;  // bits of 1.0f in a register the compiler cannot fold (dr_traverse.cuh qmagic)
-  SmemStack st{reinterpret_cast<uint2*>(smem + 1u) + threadIdx.x};
-  SmemTriStack tst{st.base + (size_t)sc.stack_cap * kTraceBlock, nullptr};
+  SmemStack<kTraceBlock> st{reinterpret_cast<uint2*>(smem + 1u) + threadIdx.x};
+  SmemTriStack<kTraceBlock> tst{st.base + (size_t)sc.stack_cap * kTraceBlock, nullptr};
   tst.base3 = reinterpret_cast<uint32_t*>(tst.base + (size_t)kTriStack * kTraceBlock - threadIdx.x) + threadIdx.x;
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr unsigned kFull = 0xFFFFFFFFu;
   uint32_t wnext = 0, wend = 0;  // this warp's private range of the queue
   bool drained = false;
-  TravLane L;
+  TravLane<kTrisPerStep> L;
   uint32_t ridx = 0, nn = 0, nt = 0;
   trav_lane_init(L, one);
   for (;;) {
@@ -349,7 +361,7 @@ k_trace(DevScene sc, const float4* __restrict__ q, uint32_t cap, const uint32_t*
     if (!act) break;
     // ---- lockstep traversal
     do {
-      const bool done = trav_step<STATS>(sc, smem, st, tst, L, nn, nt);
+      const bool done = trav_step<STATS, kTraceBlock, kTrisPerStep>(sc, smem, st, tst, L, nn, nt);
       if (done) hits[ridx] = make_uint2(__float_as_uint(L.r.t), L.r.li);
       L.active = L.active && !done;
       act = __ballot_sync(kFull, L.active);

@@ -64,7 +64,10 @@ constexpr uint32_t kWaveIdleLimit = DR_WAVE_IDLE_LIMIT;   // idle rounds of >= 2
 #endif
 template <bool NEE> constexpr int kWaveShadeWarps = NEE ? DR_WAVE_SHADE_WARPS_NEE : DR_WAVE_SHADE_WARPS;   // of the block's warps; the others trace
 constexpr int kWaveRefillBelow = DR_WAVE_REFILL_BELOW;   // a trace warp flushes its finished rays and refills below this many busy lanes
-template <bool NEE> constexpr int kWaveTraceThreads = kTraceBlock - 32 * kWaveShadeWarps<NEE>;
+template <bool NEE, int BLOCK> constexpr int kWaveTraceThreads = BLOCK - 32 * kWaveShadeWarps<NEE>;
+// evaluations of fewer states run in the small block shape (dr_eval.cuh TraceSmall); measured crossovers on configs[3]: between
+// 2^18 and 589 824 states without, between 2^16 and 2^18 with next-event estimation (profiles/r02f_tuning.md)
+constexpr uint32_t kWaveSmallBelow = 400000u, kWaveSmallBelowNee = 160000u;
 #ifndef DR_WAVE_HIT_CAP
 #define DR_WAVE_HIT_CAP 1024
 #endif
@@ -118,13 +121,13 @@ __device__ __noinline__ uint32_t wave_idle_wait(const EvalWs& ws, uint32_t n, ui
 // t_max just behind the sampled point and stop at the first other triangle hit clearly in front of it (kShadowBand): the
 // closest hit is then not that emitter either way, so the visibility decision is the one of the full closest-hit query.
 constexpr float kShadowBand = 1e-3f;
-template <bool STATS, bool NEE>
-__device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs& ws, uint32_t n, const uint4* smem, SmemStack& st,
-                                                SmemTriStack& tst, WaveShared* wsh, uint32_t* h_pay, uint32_t* h_t, uint32_t* h_li,
+template <bool STATS, bool NEE, int BLOCK, int K>
+__device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs& ws, uint32_t n, const uint4* smem, SmemStack<BLOCK>& st,
+                                                SmemTriStack<BLOCK>& tst, WaveShared* wsh, uint32_t* h_pay, uint32_t* h_t, uint32_t* h_li,
                                                 uint32_t one, unsigned long long* work) {
   const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr unsigned kFull = 0xFFFFFFFFu;
-  TravLane L;
+  TravLane<K> L;
   uint32_t pay = 0, nn = 0, nt = 0;       // payload (state | segment) of the ray this lane holds
   trav_lane_init(L, one);
   uint32_t claim = 0, taken = kFetchChunk;  // the claimed chunk: entries claim + [taken, kFetchChunk) are still to be handed out
@@ -222,12 +225,12 @@ __device__ __forceinline__ void wave_trace_loop(const DevScene& sc, const EvalWs
     }
     // ---- lockstep traversal; a finished lane keeps its hit in L.r until the flush before the next refill
     do {
-      bool done = trav_step<STATS>(sc, smem, st, tst, L, nn, nt);
+      bool done = trav_step<STATS, BLOCK, K>(sc, smem, st, tst, L, nn, nt);
       if (NEE && L.active && !done && sh_lim >= 0.f && L.r.id != 0xFFFFFFFFu && L.r.id != sh_id && L.r.t < sh_lim) {
         done = true;                                   // occluded: drop what is still requested or stacked
         L.has_node = false;
 #pragma unroll
-        for (int it = 0; it < kTrisPerStep; ++it) L.tri[it].li = kMiss;
+        for (int it = 0; it < K; ++it) L.tri[it].li = kMiss;
       }
       pend = pend || done;
       L.active = L.active && !done;
@@ -367,16 +370,18 @@ __device__ __forceinline__ void wave_shade_loop(const DevScene& sc, const EvalWs
 
 // ---- the kernel -----------------------------------------------------------------------------------------------------
 // NEE: the scene uses next-event estimation (two-phase vertices, shadow rays); STATS: the counting pass (NEE scenes only)
-template <bool GRAD, bool STATS, bool NEE>
-__global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
+// C: the block shape, TraceBig or TraceSmall (dr_eval.cuh)
+template <bool GRAD, bool STATS, bool NEE, class C>
+__global__ void __launch_bounds__(C::kBlock, 1) k_wave(DevScene sc, EvalWs ws, EvalIO io, uint32_t n) {
+  constexpr int kB = C::kBlock;
   static_assert((kFetchChunk & (kFetchChunk - 1u)) == 0 && kFetchChunk <= 32, "chunk: power of two, one entry per lane");
   extern __shared__ uint4 smem[];
   if (n == 0) return;
   // shared memory: one constant word | node stacks | triangle stacks | ring counters | ring
-  SmemStack st{reinterpret_cast<uint2*>(smem + 1u) + threadIdx.x};
-  SmemTriStack tst{st.base + (size_t)sc.stack_cap * kTraceBlock, nullptr};
-  tst.base3 = reinterpret_cast<uint32_t*>(tst.base + (size_t)kTriStack * kTraceBlock - threadIdx.x) + threadIdx.x;
-  uint32_t* tail = tst.base3 - threadIdx.x + (size_t)kTriStack * kTraceBlock;
+  SmemStack<kB> st{reinterpret_cast<uint2*>(smem + 1u) + threadIdx.x};
+  SmemTriStack<kB> tst{st.base + (size_t)sc.stack_cap * kB, nullptr};
+  tst.base3 = reinterpret_cast<uint32_t*>(tst.base + (size_t)kTriStack * kB - threadIdx.x) + threadIdx.x;
+  uint32_t* tail = tst.base3 - threadIdx.x + (size_t)kTriStack * kB;
   WaveShared* wsh = reinterpret_cast<WaveShared*>(tail);
   uint32_t* h_pay = tail + sizeof(WaveShared) / 4;
   uint32_t* h_t = h_pay + kHitCap;
@@ -387,8 +392,8 @@ __global__ void __launch_bounds__(kTraceBlock, 1) k_wave(DevScene sc, EvalWs ws,
   }
   __syncthreads();
   const uint32_t one = *(volatile uint32_t*)&smem[0].x;  // dr_traverse.cuh qmagic
-  if (threadIdx.x >= (unsigned)kWaveTraceThreads<NEE>) wave_shade_loop<GRAD, NEE>(sc, ws, io, n, wsh, h_pay, h_t, h_li);
-  else wave_trace_loop<STATS, NEE>(sc, ws, n, smem, st, tst, wsh, h_pay, h_t, h_li, one, io.work);
+  if (threadIdx.x >= (unsigned)kWaveTraceThreads<NEE, kB>) wave_shade_loop<GRAD, NEE>(sc, ws, io, n, wsh, h_pay, h_t, h_li);
+  else wave_trace_loop<STATS, NEE, kB, C::kTris>(sc, ws, n, smem, st, tst, wsh, h_pay, h_t, h_li, one, io.work);
 }
 
 }  // namespace dr

@@ -658,12 +658,13 @@ def test_wave_kernel_equals_segment_loop(dr, oracle, torch_, case, score):
     desc, gsc, _ = _full_scene(dr, oracle, name, make) if name in ("caustic", "machines") else (make(), None, None)
     gsc = gsc or dr.Scene(desc)
     x = torch_.from_numpy(S.seeded_states(n, desc.dim, 11)).cuda()
-    a = gsc.eval_states(x, score, form=2)
+    a = gsc.eval_states(x, score, form=2)                                        # the block shape chosen by the size
     b = gsc.eval_states(x, score, form=1)
     assert int(a["nrays"].sum()) > n                                             # paths do bounce
     _same_eval(a, b)
-    c = gsc.eval_states(x, score, form=2)                                        # and again: a second launch on fresh memory
-    _same_eval(a, c)
+    for form in (3, 4):                                                          # both block shapes (640 threads and two triangle
+        c = gsc.eval_states(x, score, form=form)                                 # slots per lane; 768 and one), each a further
+        _same_eval(a, c)                                                         # launch on fresh memory
 
 
 def test_chains_run_identically_in_both_forms(dr, torch_):
@@ -673,16 +674,17 @@ def test_chains_run_identically_in_both_forms(dr, torch_):
     gsc = dr.Scene(desc)
     for method in ("metropolis", "mala_restore", "diffusion_restore"):
         out = []
-        for form in (2, 1):
+        for form in (2, 1, 4):
             ch = dr.Chains(gsc, method, 20000, seed=5)
             ch.set_eval_form(form)
             ch.init(1)
             ch.step(6)
             out.append((ch.download(), ch.stats()))
-        (sa, ta), (sb, tb) = out
-        for k in sa:
-            assert np.array_equal(sa[k].view(np.uint8), sb[k].view(np.uint8)), (method, k)
-        assert ta["tours"] == tb["tours"] and ta["rays"] == tb["rays"] and ta["mh_accepts"] == tb["mh_accepts"]
+        (sa, ta) = out[0]
+        for sb, tb in out[1:]:
+            for k in sa:
+                assert np.array_equal(sa[k].view(np.uint8), sb[k].view(np.uint8)), (method, k)
+            assert ta["tours"] == tb["tours"] and ta["rays"] == tb["rays"] and ta["mh_accepts"] == tb["mh_accepts"]
 
 
 _STALL_SNIPPET = """
