@@ -7,7 +7,7 @@
 // runs dry once, at the end of the evaluation:
 //   * trace warps: the lockstep traversal of k_trace (trav_step); an idle lane takes the next ray of the queue.
 //     A finished ray goes, as (state | segment, t, triangle), into a small ring in the block's shared memory.
-//   * shade warps (kWaveShadeWarps<NEE> per block): take up to 32 finished rays from the block's ring, run shade_vertex
+//   * shade warps (kWaveShadeWarps<NEE, BLOCK> per block): take up to 32 finished rays from the block's ring, run shade_vertex
 //     (the code of k_shade), write the surviving paths' next rays and count the finished paths.
 // The evaluation is over when every path has finished (ctl[kCtlWaveDone] == n).
 //
@@ -62,9 +62,14 @@ constexpr uint32_t kWaveIdleLimit = DR_WAVE_IDLE_LIMIT;   // idle rounds of >= 2
 #else
 #define DR_CHECK(cond, bit) do { } while (0)
 #endif
-template <bool NEE> constexpr int kWaveShadeWarps = NEE ? DR_WAVE_SHADE_WARPS_NEE : DR_WAVE_SHADE_WARPS;   // of the block's warps; the others trace
+#ifndef DR_WAVE_SHADE_WARPS_NEE_SMALL
+#define DR_WAVE_SHADE_WARPS_NEE_SMALL 3   // small evaluations do not keep five shade warps busy: 1.32 against 1.50 ms per frame at 2^14 chains
+#endif
+// shade warps of a block of BLOCK threads (the other warps trace)
+template <bool NEE, int BLOCK> constexpr int kWaveShadeWarps =
+    !NEE ? DR_WAVE_SHADE_WARPS : (BLOCK == TraceSmall::kBlock && TraceSmall::kBlock != TraceBig::kBlock ? DR_WAVE_SHADE_WARPS_NEE_SMALL : DR_WAVE_SHADE_WARPS_NEE);
 constexpr int kWaveRefillBelow = DR_WAVE_REFILL_BELOW;   // a trace warp flushes its finished rays and refills below this many busy lanes
-template <bool NEE, int BLOCK> constexpr int kWaveTraceThreads = BLOCK - 32 * kWaveShadeWarps<NEE>;
+template <bool NEE, int BLOCK> constexpr int kWaveTraceThreads = BLOCK - 32 * kWaveShadeWarps<NEE, BLOCK>;
 // evaluations of fewer states run in the small block shape (dr_eval.cuh TraceSmall); measured crossovers on configs[3]: between
 // 2^18 and 589 824 states without, between 2^16 and 2^18 with next-event estimation (profiles/r02f_tuning.md)
 constexpr uint32_t kWaveSmallBelow = 400000u, kWaveSmallBelowNee = 160000u;
