@@ -134,6 +134,44 @@ def run_reference(args):
     }))
 
 
+def second_reading(dr, torch, args, n_local):
+    """The same scene, method and ensemble with next-event estimation + MIS (Q21): the paper does not say which path
+    construction it uses, and under Q21 the Langevin step, the score and the race do real work.  A short
+    run of the same frame loop: its numbers go into the JSON line beside the headline ones (`python bench.py --nee` is the full run)."""
+    desc = make_desc(args.scene, True)
+    chains = dr.Chains(dr.Scene(desc), args.method, n_local, seed=4)
+    stream = torch.cuda.current_stream()
+    steps, warm = min(args.steps, 60), max(args.warmup, 3)
+    chains.init(0)
+    for _ in range(warm):
+        chains.step(1); chains.resolve()
+    torch.cuda.synchronize()
+    st0 = chains.stats()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        chains.step(1); chains.resolve()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    st1 = chains.stats()
+    pf = min(steps, 8)
+    chains.profile_enable(True)
+    for _ in range(pf):
+        chains.step(1); chains.resolve()
+    prof = chains.profile_read()
+    chains.profile_enable(False)
+    return {"path_construction": "direction sampling + next-event estimation with MIS (Q21)", "steps": steps, "warmup": warm,
+            "ms_per_step": ms / steps, "value": n_local * steps / (ms * 1e-3), "unit": UNIT,
+            "mrays_per_s": (st1["rays"] - st0["rays"]) / (ms * 1e-3) / 1e6,
+            "rays_per_mutation": (st1["rays"] - st0["rays"]) / (n_local * steps),
+            "kernels_ms_per_frame": {k: v["ms"] / pf for k, v in prof.items()},
+            "kernel_launches_per_frame": sum(v["launches"] for v in prof.values()) / pf,
+            "kill_fraction_last": st1["kills_last_step"] / n_local,
+            "zeta_lit_fraction_of_uniform_samples": st1["lit_init"] / n_local,
+            "grad_list_share_of_evaluations": (st1["grad_states"] - st0["grad_states"]) / (n_local * steps)}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -145,6 +183,7 @@ def main():
     ap.add_argument("--chains", type=int, default=0, help="chains per GPU (default: one per pixel)")
     ap.add_argument("--nee", action="store_true", help="path construction with next-event estimation + MIS (second reading, DESIGN.md Q21)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-second-reading", action="store_true", help="skip the short run of the other path construction (N = 1 only)")
     ap.add_argument("--e2e-steps", type=int, default=10)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -350,6 +389,9 @@ def main():
                                "peak_source": pk["source"]},
         "e2e": e2e,
     }
+    if world == 1 and not args.nee and not args.no_second_reading:
+        del chains
+        out["second_reading"] = second_reading(dr, torch, args, n_local)
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(desc, args.method, 32768, 6, 4)
     print(json.dumps(out))
