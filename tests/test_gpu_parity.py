@@ -687,6 +687,45 @@ def test_chains_run_identically_in_both_forms(dr, torch_):
             assert ta["tours"] == tb["tours"] and ta["rays"] == tb["rays"] and ta["mh_accepts"] == tb["mh_accepts"]
 
 
+def test_chains_with_nee_run_identically_in_both_block_shapes(dr, torch_):
+    """Next-event estimation has no per-segment loop: the two block shapes of k_wave (640 threads with two triangle slots per lane
+    and three shade warps, 768 with one and five) check each other, through the whole step of a gradient sampler -- shading with
+    shadow rays, vertex records, the reverse sweep per vertex index, MH decision -- bit for bit after 5 iterations."""
+    desc = S.mini_machines()
+    desc.nee = True
+    gsc = dr.Scene(desc)
+    for method in ("mala", "diffusion_restore"):
+        out = []
+        for form in (3, 4):
+            ch = dr.Chains(gsc, method, 30000, seed=6)
+            ch.set_eval_form(form)
+            ch.init(2)
+            ch.step(5)
+            out.append((ch.download(), ch.stats()))
+        (sa, ta), (sb, tb) = out
+        for k in sa:
+            assert np.array_equal(sa[k].view(np.uint8), sb[k].view(np.uint8)), (method, k)
+        assert ta["tours"] == tb["tours"] and ta["rays"] == tb["rays"] and ta["grad_states"] == tb["grad_states"] > 0
+
+
+def test_profile_counts_every_kernel_launch(dr, torch_):
+    """dr_profile_read: 8 launches per frame without, 8 + L with next-event estimation and a score (the reverse sweep is an init
+    launch, one launch per vertex index and a finish launch); bench.py's gpu_launches is this count."""
+    for nee, want in ((False, 8), (True, None)):
+        desc = S.mini_machines()
+        desc.nee = nee
+        ch = dr.Chains(dr.Scene(desc), "diffusion_restore", 4096, seed=3)
+        ch.init(0)
+        ch.profile_enable(True)
+        ch.step(3)
+        ch.resolve()
+        prof = ch.profile_read()
+        ch.profile_enable(False)
+        n = sum(v["launches"] for v in prof.values())
+        per_step = 7 + (desc.max_path_len + 1 if nee else 1) - 1      # propose, raygen, k_wave, score, decide, scan, scatter
+        assert n == 3 * per_step + 1, (nee, n, prof)                  # + one resolve
+
+
 _STALL_SNIPPET = """
 import sys, numpy as np, torch
 sys.path.insert(0, {root!r})
