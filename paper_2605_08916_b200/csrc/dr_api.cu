@@ -82,7 +82,9 @@ struct dr_chains {
   int eval_form = 0;               // test hook dr_chains_set_eval_form: 0 = default choice, 1 = per-segment loop, 2 = k_wave, 3 / 4 = k_wave in the small / big block shape
   void* hook_scratch = nullptr;    // device staging of dr_chains_download / _upload (row-major copies), allocated on first use
   void* d_rho = nullptr;           // f4: (probability, running sum) per film tile
-  ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); cudaFree(hook_scratch); cudaFree(d_rho); }
+  uint32_t* h_last_rays = nullptr; // pinned: rays of the last k_wave evaluation that has finished (copied behind every evaluation, read
+                                   // without waiting: it picks the block shape of the next one, which does not change any result)
+  ~dr_chains() { for (cudaEvent_t e : ev) cudaEventDestroy(e); cudaFree(hook_scratch); cudaFree(d_rho); if (h_last_rays) cudaFreeHost(h_last_rays); }
 };
 
 namespace {
@@ -241,9 +243,15 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
 #endif
   if (wave) {
     ProfScope ps(prof, DR_PROF_TRACE, s);
-    const bool small = form == 3 || (form != 4 && n < (dev.nee ? kWaveSmallBelowNee : kWaveSmallBelow));
+    // the block shape: by the rays the ensemble's last finished evaluation made, if that is known, else by the number of states
+    bool small = n < (dev.nee ? kWaveSmallBelowNee : kWaveSmallBelow);
+    const uint32_t last_rays = prof && prof->h_last_rays ? *(volatile uint32_t*)prof->h_last_rays : 0u;
+    if (last_rays) small = last_rays < kWaveSmallBelowRays;
+    if (form == 3) small = true;
+    if (form == 4) small = false;
     if (small) launch_wave<TraceSmall>(dev, ws, io, n, grad, stats, sc->n_sm, s);
     else launch_wave<TraceBig>(dev, ws, io, n, grad, stats, sc->n_sm, s);
+    if (prof && prof->h_last_rays && !stats) cudaMemcpyAsync(prof->h_last_rays, ws.ctl + kCtlWaveReserve, 4, cudaMemcpyDeviceToHost, s);
   } else
   for (uint32_t k = 1; k <= dev.L; ++k) {
     const float4* q = (k & 1u) ? ws.qa : ws.qb;
@@ -581,6 +589,8 @@ dr_status dr_chains_create(const dr_scene* s, const dr_config* c, void* dev_stat
   ws.qa = (float4*)(b + L.q); ws.qb = ws.qa + 3 * (size_t)cp.N; ws.hits = (uint2*)(b + L.hits); ws.ring = (uint2*)(b + L.ring);
   ws.rec = (float4*)(b + L.rec); ws.vrec = (float4*)(b + L.vrec); ws.adj = (float4*)(b + L.adj);
   ws.pinfo = cp.grad ? (uint32_t*)(b + L.pinfo) : nullptr; ws.gradlist = (uint32_t*)(b + L.gradlist); ws.ctl = (uint32_t*)(b + L.ctl); ws.cap = cp.N;
+  if (cudaHostAlloc((void**)&h->h_last_rays, sizeof(uint32_t), cudaHostAllocDefault) == cudaSuccess) *h->h_last_rays = 0u;
+  else { h->h_last_rays = nullptr; (void)cudaGetLastError(); }   // only a hint: without it the shape goes by the number of states
   *out = h;
   return DR_OK;
 }

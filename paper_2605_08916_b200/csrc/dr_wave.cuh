@@ -73,6 +73,10 @@ template <bool NEE, int BLOCK> constexpr int kWaveTraceThreads = BLOCK - 32 * kW
 // evaluations of fewer states run in the small block shape (dr_eval.cuh TraceSmall); measured crossovers on configs[3]: between
 // 2^18 and 589 824 states without, between 2^16 and 2^18 with next-event estimation (profiles/r02f_tuning.md)
 constexpr uint32_t kWaveSmallBelow = 400000u, kWaveSmallBelowNee = 160000u;
+// a chain ensemble knows better: the rays its last evaluation made (configs[3]: 3.6 M rays at 2^18 states are faster in the small
+// shape, 8.2 M at 589 824 in the big one; with next-event estimation 2.6 M small, 5.2 M big; the caustic scene's 2.2 M rays at
+// 2^20 states small: 0.97 against 1.16 ms)
+constexpr uint32_t kWaveSmallBelowRays = 4500000u;
 #ifndef DR_WAVE_HIT_CAP
 #define DR_WAVE_HIT_CAP 1024
 #endif
