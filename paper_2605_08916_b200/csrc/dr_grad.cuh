@@ -180,6 +180,9 @@ __global__ void __launch_bounds__(kGradInitBlock) k_grad_nee_init(DevScene sc, E
 #ifndef DR_GRAD_MIN_BLOCKS
 #define DR_GRAD_MIN_BLOCKS 4
 #endif
+#ifndef DR_GRAD_LAMBERT_SPLIT
+#define DR_GRAD_LAMBERT_SPLIT 1
+#endif
 // Vertex k of every path whose vertex k has material KIND (0 Lambert, 1 dielectric, 2 GGX).
 // Phi depends on the ray (o, d) through the hit point h = o + t d on the frozen plane, t = ((v0 - o).n) / (d.n), and -- for a
 // dielectric or GGX vertex only -- on d itself.  With P = I - d n^T / (d.n):  dPhi/do = P^T dPhi/dh,  dPhi/dd = t P^T dPhi/dh
@@ -217,6 +220,38 @@ __device__ __forceinline__ void grad_vertex(const DevScene& sc, const EvalWs& ws
     gd = make_float4(tp * go.x + (db.x * w.x.d[0] + db.y * w.y.d[0] + db.z * w.z.d[0]),
                      tp * go.y + (db.x * w.x.d[1] + db.y * w.y.d[1] + db.z * w.z.d[1]),
                      tp * go.z + (db.x * w.x.d[2] + db.y * w.y.d[2] + db.z * w.z.d[2]), 0.f);
+  } else if (KIND == 0 && DR_GRAD_LAMBERT_SPLIT) {
+    // Lambert: the direction sample depends on (u1, u2) alone (two tangents), the connection on (h, v1, v2) alone (five): each
+    // part is differentiated once with just its own tangents, instead of the whole vertex twice with four
+    const float4 u = io.x[(size_t)k * io.stride + s];
+    const float3 lumT = make_float3(0.2126f * rT.x, 0.7152f * rT.y, 0.0722f * rT.z);
+    W = make_float3(f.m0.y, f.m0.z, f.m0.w);
+    float3 gh = ob;                                             // o2 = h + const
+    {
+      typedef Du<5> D;
+      V3<D> H;                                                  // h = o + t d, as the shading computes it
+      H.x = du_var<5>(o.x + d.x * tp, 0); H.y = du_var<5>(o.y + d.y * tp, 1); H.z = du_var<5>(o.z + d.z * tp, 2);
+      const V3<D> Dc{du_const<5>(d.x), du_const<5>(d.y), du_const<5>(d.z)};
+      VertexOut<D> vo;
+      uint32_t lj = 0;
+      nee_connect<D>(sc, f.fr, f.m0, f.m1, 0u, Dc, H, du_var<5>(u.z, 3), du_var<5>(u.w, 4), vo, lj);
+      if (vo.nee_valid && f.vis) {
+        const D c0 = vo.fcos[0] * vo.lw[0], c1 = vo.fcos[1] * vo.lw[1], c2 = vo.fcos[2] * vo.lw[2];
+        C = make_float3(c0.v, c1.v, c2.v);
+        const D phi = c0 * lumT.x + c1 * lumT.y + c2 * lumT.z;
+        gh = make_float3(gh.x + phi.d[0], gh.y + phi.d[1], gh.z + phi.d[2]);
+        gu.z = phi.d[3]; gu.w = phi.d[4];
+      }
+    }
+    {
+      const V3<Du<2>> w = lambert_dir<Du<2>>(f.fr, du_var<2>(u.x, 0), du_var<2>(u.y, 1));
+      const Du<2> pb = sqrt_t(1.0f - du_var<2>(u.x, 0)) * kInvPi;
+      gu.x = (db.x * w.x.d[0] + db.y * w.y.d[0] + db.z * w.z.d[0]) + pb.d[0] * pbb;
+      gu.y = (db.x * w.x.d[1] + db.y * w.y.d[1] + db.z * w.z.d[1]) + pb.d[1] * pbb;
+    }
+    const float c = dot3(d, gh) / dnn;
+    go = make_float4(gh.x - n.x * c, gh.y - n.y * c, gh.z - n.z * c, 0.f);   // P^T dPhi/dh
+    gd = make_float4(tp * go.x, tp * go.y, tp * go.z, 0.f);
   } else {
     const float4 u = io.x[(size_t)k * io.stride + s];
     const float3 lumT = make_float3(0.2126f * rT.x, 0.7152f * rT.y, 0.0722f * rT.z);

@@ -62,18 +62,11 @@ template <class T> struct VertexOut {
   bool pb_valid, alive, nee_valid;
 };
 
-// hit: the point on the triangle's plane.  `decide`: take the lobe decision here (float instantiation) or use `reflect`.
+// Emitter connection of a Lambert / GGX vertex at `hit` (Q21): fills out.nee_valid, out.y, out.fcos, out.lw and light_j.
+// A function of (hit, v1, v2) -- and of d for a GGX vertex -- so that the score's reverse sweep can differentiate it on its own.
 template <class T, bool NEE = true>
-__device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const Frame& fr, float dn, float4 m0, float4 m1, uint32_t kind,
-                                          V3<T> o, V3<T> d, T u1, T u2, T v1, T v2, bool decide, bool& reflect, VertexOut<T>& out,
-                                          V3<T>& hit_out, uint32_t& light_j) {
-  const float side = dn < 0.f ? 1.f : -1.f;
-  const float3 n = fr.nf * side;   // the geometric normal again (exact: * +-1)
-  // 1b: hit point on the frozen triangle's plane, t = ((v0 - o).n) / (d.n)
-  const T tp = dotf(vsubf(v0, o), n) / dotf(d, n);
-  V3<T> hit;
-  hit.x = o.x + d.x * tp; hit.y = o.y + d.y * tp; hit.z = o.z + d.z * tp;
-  hit_out = hit;
+__device__ __forceinline__ void nee_connect(const DevScene& sc, const Frame& fr, float4 m0, float4 m1, uint32_t kind, V3<T> d, V3<T> hit,
+                                            T v1, T v2, VertexOut<T>& out, uint32_t& light_j) {
   out.nee_valid = false;
   out.fcos[0] = out.fcos[1] = out.fcos[2] = out.lw[0] = out.lw[1] = out.lw[2] = lift_t<T>(0.f);
   // ---- next-event estimation at a Lambert / GGX vertex (Q21)
@@ -119,6 +112,21 @@ __device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const F
       out.lw[0] = L.le.x * w_l / p_l; out.lw[1] = L.le.y * w_l / p_l; out.lw[2] = L.le.z * w_l / p_l;
     }
   }
+}
+
+// hit: the point on the triangle's plane.  `decide`: take the lobe decision here (float instantiation) or use `reflect`.
+template <class T, bool NEE = true>
+__device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const Frame& fr, float dn, float4 m0, float4 m1, uint32_t kind,
+                                          V3<T> o, V3<T> d, T u1, T u2, T v1, T v2, bool decide, bool& reflect, VertexOut<T>& out,
+                                          V3<T>& hit_out, uint32_t& light_j) {
+  const float side = dn < 0.f ? 1.f : -1.f;
+  const float3 n = fr.nf * side;   // the geometric normal again (exact: * +-1)
+  // 1b: hit point on the frozen triangle's plane, t = ((v0 - o).n) / (d.n)
+  const T tp = dotf(vsubf(v0, o), n) / dotf(d, n);
+  V3<T> hit;
+  hit.x = o.x + d.x * tp; hit.y = o.y + d.y * tp; hit.z = o.z + d.z * tp;
+  hit_out = hit;
+  nee_connect<T, NEE>(sc, fr, m0, m1, kind, d, hit, v1, v2, out, light_j);
   // ---- direction sample
   out.alive = true;
   out.pb_valid = false;
