@@ -183,6 +183,9 @@ __global__ void __launch_bounds__(kGradInitBlock) k_grad_nee_init(DevScene sc, E
 #ifndef DR_GRAD_LAMBERT_SPLIT
 #define DR_GRAD_LAMBERT_SPLIT 1
 #endif
+#ifndef DR_GRAD_GGX_SPLIT
+#define DR_GRAD_GGX_SPLIT 1
+#endif
 // Vertex k of every path whose vertex k has material KIND (0 Lambert, 1 dielectric, 2 GGX).
 // Phi depends on the ray (o, d) through the hit point h = o + t d on the frozen plane, t = ((v0 - o).n) / (d.n), and -- for a
 // dielectric or GGX vertex only -- on d itself.  With P = I - d n^T / (d.n):  dPhi/do = P^T dPhi/dh,  dPhi/dd = t P^T dPhi/dh
@@ -252,6 +255,49 @@ __device__ __forceinline__ void grad_vertex(const DevScene& sc, const EvalWs& ws
     const float c = dot3(d, gh) / dnn;
     go = make_float4(gh.x - n.x * c, gh.y - n.y * c, gh.z - n.z * c, 0.f);   // P^T dPhi/dh
     gd = make_float4(tp * go.x, tp * go.y, tp * go.z, 0.f);
+  } else if (KIND == 2 && DR_GRAD_GGX_SPLIT) {
+    // GGX: Phi = Phi_conn(h, d, v1, v2) + Phi_dir(d, u1, u2) + o2 . o_bar.  The connection is differentiated in two passes of four
+    // tangents, (h, v1) and (d, v2), the direction sample once over (d, u1, u2): three passes of the whole vertex before
+    const float4 u = io.x[(size_t)k * io.stride + s];
+    const float3 lumT = make_float3(0.2126f * rT.x, 0.7152f * rT.y, 0.0722f * rT.z);
+    const float3 h = make_float3(o.x + d.x * tp, o.y + d.y * tp, o.z + d.z * tp);   // as the shading computes it
+    float3 gh = make_float3(0.f, 0.f, 0.f), gdd = gh;      // dPhi/dh, dPhi/dd at fixed h
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+      typedef Du<4> D;
+      V3<D> H{du_const<4>(h.x), du_const<4>(h.y), du_const<4>(h.z)}, Dd{du_const<4>(d.x), du_const<4>(d.y), du_const<4>(d.z)};
+      D V1 = du_const<4>(u.z), V2 = du_const<4>(u.w);
+      if (pass == 0) { H.x.d[0] = 1.f; H.y.d[1] = 1.f; H.z.d[2] = 1.f; V1.d[3] = 1.f; }
+      else { Dd.x.d[0] = 1.f; Dd.y.d[1] = 1.f; Dd.z.d[2] = 1.f; V2.d[3] = 1.f; }
+      VertexOut<D> vo;
+      uint32_t lj = 0;
+      nee_connect<D>(sc, f.fr, f.m0, f.m1, 2u, Dd, H, V1, V2, vo, lj);
+      if (vo.nee_valid && f.vis) {
+        const D c0 = vo.fcos[0] * vo.lw[0], c1 = vo.fcos[1] * vo.lw[1], c2 = vo.fcos[2] * vo.lw[2];
+        const D phi = c0 * lumT.x + c1 * lumT.y + c2 * lumT.z;
+        if (pass == 0) { C = make_float3(c0.v, c1.v, c2.v); gh = make_float3(phi.d[0], phi.d[1], phi.d[2]); gu.z = phi.d[3]; }
+        else { gdd = make_float3(phi.d[0], phi.d[1], phi.d[2]); gu.w = phi.d[3]; }
+      }
+    }
+    {
+      typedef Du<5> D;
+      const V3<D> Dd{du_var<5>(d.x, 0), du_var<5>(d.y, 1), du_var<5>(d.z, 2)};
+      VertexOut<D> vo;
+      vo.alive = true; vo.pb_valid = false; vo.pb = du_const<5>(0.f);
+      ggx_sample<D>(sc, f.fr, f.m0, f.m1, Dd, du_var<5>(u.x, 3), du_var<5>(u.y, 4), vo);
+      W = make_float3(vo.W[0].v, vo.W[1].v, vo.W[2].v);
+      if (vo.alive) {
+        D phi = vo.W[0] * (lumT.x * R.x) + vo.W[1] * (lumT.y * R.y) + vo.W[2] * (lumT.z * R.z);
+        phi = phi + vo.d2.x * db.x + vo.d2.y * db.y + vo.d2.z * db.z;
+        if (vo.pb_valid) phi = phi + vo.pb * pbb;
+        gdd = make_float3(gdd.x + phi.d[0], gdd.y + phi.d[1], gdd.z + phi.d[2]);
+        gu.x = phi.d[3]; gu.y = phi.d[4];
+        gh = gh + ob;                                        // o2 = h + const
+      }
+    }
+    const float c = dot3(d, gh) / dnn;
+    go = make_float4(gh.x - n.x * c, gh.y - n.y * c, gh.z - n.z * c, 0.f);   // P^T dPhi/dh
+    gd = make_float4(tp * go.x + gdd.x, tp * go.y + gdd.y, tp * go.z + gdd.z, 0.f);
   } else {
     const float4 u = io.x[(size_t)k * io.stride + s];
     const float3 lumT = make_float3(0.2126f * rT.x, 0.7152f * rT.y, 0.0722f * rT.z);

@@ -114,6 +114,27 @@ __device__ __forceinline__ void nee_connect(const DevScene& sc, const Frame& fr,
   }
 }
 
+// Direction sample of a GGX vertex: out.alive, out.d2, out.W and, with next-event estimation, the density out.pb of d2.
+// A function of (d, u1, u2): the reverse sweep differentiates it on its own (out.alive / pb_valid / pb must come in cleared).
+template <class T, bool NEE = true>
+__device__ __forceinline__ void ggx_sample(const DevScene& sc, const Frame& fr, float4 m0, float4 m1, V3<T> d, T u1, T u2, VertexOut<T>& out) {
+  T c5, G1;
+  V3<T> hm;
+  if (!ggx_dir<T>(fr, m1.y, d, u1, u2, out.d2, c5, G1, &hm)) {
+    out.alive = false;
+    out.W[0] = out.W[1] = out.W[2] = lift_t<T>(0.f);
+    out.d2 = d;
+  } else {
+    out.W[0] = (m0.y + (1.0f - m0.y) * c5) * G1; out.W[1] = (m0.z + (1.0f - m0.z) * c5) * G1; out.W[2] = (m0.w + (1.0f - m0.w) * c5) * G1;
+    if (NEE && sc.nee) {
+      V3<T> wo;
+      wo.x = -dotf(d, fr.t); wo.y = -dotf(d, fr.bf); wo.z = -dotf(d, fr.nf);
+      out.pb_valid = true;
+      out.pb = ggx_g1(wo, m1.y) * ggx_d(hm, m1.y) / (wo.z * 4.0f);
+    }
+  }
+}
+
 // hit: the point on the triangle's plane.  `decide`: take the lobe decision here (float instantiation) or use `reflect`.
 template <class T, bool NEE = true>
 __device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const Frame& fr, float dn, float4 m0, float4 m1, uint32_t kind,
@@ -144,21 +165,7 @@ __device__ __forceinline__ void vertex_fn(const DevScene& sc, float3 v0, const F
     if (!reflect) off = -1.f;
     out.d2 = dielectric_dir<T>(fr, eta, reflect, d);
   } else {
-    T c5, G1;
-    V3<T> hm;
-    if (!ggx_dir<T>(fr, m1.y, d, u1, u2, out.d2, c5, G1, &hm)) {
-      out.alive = false;
-      out.W[0] = out.W[1] = out.W[2] = lift_t<T>(0.f);
-      out.d2 = d;
-    } else {
-      out.W[0] = (m0.y + (1.0f - m0.y) * c5) * G1; out.W[1] = (m0.z + (1.0f - m0.z) * c5) * G1; out.W[2] = (m0.w + (1.0f - m0.w) * c5) * G1;
-      if (NEE && sc.nee) {
-        V3<T> wo;
-        wo.x = -dotf(d, fr.t); wo.y = -dotf(d, fr.bf); wo.z = -dotf(d, fr.nf);
-        out.pb_valid = true;
-        out.pb = ggx_g1(wo, m1.y) * ggx_d(hm, m1.y) / (wo.z * 4.0f);
-      }
-    }
+    ggx_sample<T, NEE>(sc, fr, m0, m1, d, u1, u2, out);
   }
   const float k = sc.eps_ray * off;
   out.o2.x = hit.x + fr.nf.x * k; out.o2.y = hit.y + fr.nf.y * k; out.o2.z = hit.z + fr.nf.z * k;
