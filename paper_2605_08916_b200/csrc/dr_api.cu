@@ -407,6 +407,8 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   BuiltBvh bvh;
   build_bvh8(d->host_vertices, d->nv, d->host_indices, d->nt, d->host_tri_material, bvh);
   if (bvh.depth > (uint32_t)kMaxBvhDepth) return fail(DR_ERR_UNSUPPORTED, "BVH8 deeper than the traversal stack allows");
+  if (bvh.tris.size() >= (size_t(1) << 27))   // k_wave's payload has 27 bits for a state, the vertex record 30 for a triangle reference
+    return fail(DR_ERR_UNSUPPORTED, "more than 2^27 triangle references");
 
   dr_scene* s = new dr_scene();
   DevScene& dev = s->dev;
