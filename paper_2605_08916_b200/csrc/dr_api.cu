@@ -232,6 +232,7 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
   if (form < 0 || form > 4) return fail(DR_ERR_INVALID_ARG, "evaluation form must be 0 .. 4");
   if (dev.nee && (!sc->wave_ok || form == 1)) return fail(DR_ERR_UNSUPPORTED, "next-event estimation runs in k_wave only (no per-segment loop)");
   const bool wave = dev.nee || (!stats && sc->wave_ok && (form >= 2 || (form == 0 && n < kWaveMaxStates)));
+  if (wave && n > kWaveStateMask) return fail(DR_ERR_UNSUPPORTED, "k_wave addresses at most 2^27 states per evaluation");
   CUDA_TRY(cudaMemsetAsync(ws.ctl, 0, 4 * kCtlWords, s));
   {
     ProfScope ps(prof, DR_PROF_RAYGEN, s);
