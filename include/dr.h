@@ -214,6 +214,31 @@ dr_status dr_regen_queue_download(dr_chains* chains, uint32_t* host_ids, uint32_
 /* Closest hit for n rays (device arrays o[3n], d[3n] -> t[n] (-1 = miss), prim[n] (0xFFFFFFFF = miss)). */
 dr_status dr_trace_rays(const dr_scene* scene, const float* dev_o, const float* dev_d, uint32_t n, float* dev_t,
                         uint32_t* dev_prim, void* stream);
+/* dr_trace_rays for callers that must not allocate device memory at the time of the call.
+ *
+ * Who that is: code running where cudaMalloc / cudaFree are forbidden or harmful.  Examples: a real-time frame loop or a
+ * serving process with a fixed memory budget, where an allocation can fail late or stall (cudaFree waits for the whole
+ * device); a host program that has handed all of the GPU's memory to its own pool and leaves nothing for the driver; a
+ * plugin that lives inside someone else's process and is not allowed to change that process's memory footprint.
+ * dr_trace_rays takes its ray queue, hit records and queue counters (40 bytes per ray + 8) from cudaMalloc on every call
+ * and waits for the stream before it frees them.  This variant runs the SAME kernels on the same inputs and writes the same
+ * outputs (bit for bit), but its scratch is a fixed array that is part of the library image:
+ *   - the array holds DR_TRACE_NOALLOC_MAX_RAYS rays (40 bytes each + 256): about 2.5 MiB, present on every GPU that
+ *     loads the library from the moment it is loaded until the process exits, whether this call is used or not;
+ *   - n > DR_TRACE_NOALLOC_MAX_RAYS is refused with DR_ERR_INVALID_ARG and nothing is launched: split the batch;
+ *   - the call makes no cudaMalloc, cudaFree or other allocating call, and does not synchronise: the work is queued on
+ *     `stream` like every other asynchronous call of this header.  dev_o, dev_d, dev_t, dev_prim are the caller's,
+ *     as for dr_trace_rays;
+ *   - the FIRST call on each device looks up the array's device address (a cudaGetSymbolAddress, once per device,
+ *     with the scene's device current as for every call here).  Make that first call during set-up, before the
+ *     stream is put into capture mode;
+ *   - every call on a device uses the one array, and the array keeps what the last call left in it.  The call clears
+ *     the two queue counters it needs at zero itself.  Two calls whose GPU work can overlap (different streams without an
+ *     event between them, or two host threads) race on the array and give wrong hits: keep the calls of one device on one
+ *     stream, or order them with events. */
+#define DR_TRACE_NOALLOC_MAX_RAYS 65536u
+dr_status dr_trace_rays_noalloc(const dr_scene* scene, const float* dev_o, const float* dev_d, uint32_t n, float* dev_t,
+                                uint32_t* dev_prim, void* stream);
 /* Target evaluation for n states (device arrays, row-major x[n*d]) -> f[3n], p[n], pix[n], score[n*d] (if
  * non-NULL), nrays[n], sig[n]. */
 dr_status dr_eval_states(const dr_scene* scene, const float* dev_x, uint32_t n, float* dev_f, float* dev_p,

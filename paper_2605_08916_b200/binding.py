@@ -26,8 +26,9 @@ EXPORTS = [
     "dr_trace_rays", "dr_eval_states", "dr_philox_blocks", "dr_rng_transforms", "dr_resolve_image_sharded",
     "dr_eval_work_stats", "dr_profile_enable", "dr_profile_read", "dr_chains_work_stats", "dr_eval_states_form",
     "dr_chains_set_eval_form", "dr_frame_floats", "dr_pack_frame", "dr_resolve_image_packed",
-    "dr_bias_field",
+    "dr_bias_field", "dr_trace_rays_noalloc",
 ]
+TRACE_NOALLOC_MAX_RAYS = 65536   # DR_TRACE_NOALLOC_MAX_RAYS of include/dr.h
 PROF_NAMES = ["propose", "raygen", "trace", "shade", "grad", "decide", "scan", "scatter", "resolve"]
 
 
@@ -98,6 +99,7 @@ def _load():
     L.dr_chains_last_step.argtypes = [vp, vp, vp, vp]
     L.dr_regen_queue_download.argtypes = [vp, vp, C.POINTER(u32), vp]
     L.dr_trace_rays.argtypes = [vp, vp, vp, u32, vp, vp, vp]
+    L.dr_trace_rays_noalloc.argtypes = [vp, vp, vp, u32, vp, vp, vp]
     L.dr_eval_states.argtypes = [vp, vp, u32, vp, vp, vp, vp, vp, vp, vp]
     L.dr_eval_states_form.argtypes = [vp, vp, u32, vp, vp, vp, vp, vp, vp, i32, vp]
     L.dr_chains_set_eval_form.argtypes = [vp, i32]
@@ -194,6 +196,17 @@ class Scene:
         prim = torch.empty(n, dtype=torch.int32, device="cuda")
         _check(lib.dr_trace_rays(self.h, _dp(o.contiguous()), _dp(d.contiguous()), n, _dp(t), _dp(prim), _stream()))
         return t, prim
+
+    def trace_rays_noalloc(self, o: torch.Tensor, d: torch.Tensor, t: torch.Tensor, prim: torch.Tensor) -> None:
+        """dr_trace_rays_noalloc: closest hits into the caller's own t (float32) and prim (int32) tensors, for callers that
+        must not allocate GPU memory while they trace (fixed-budget frame loops and servers, hosts whose own pool owns the
+        GPU, plugins inside another process).  Unlike trace_rays, nothing is created here: outputs are passed in, the
+        scratch is a fixed 2.5 MiB array inside libdr.so.  At most TRACE_NOALLOC_MAX_RAYS rays per call (more is an error);
+        asynchronous on the current stream; calls that overlap on the GPU race on the shared scratch (include/dr.h)."""
+        n = o.shape[0]
+        assert o.is_contiguous() and d.is_contiguous() and t.is_contiguous() and prim.is_contiguous()
+        assert t.numel() == n and prim.numel() == n and t.dtype == torch.float32 and prim.dtype == torch.int32
+        _check(lib.dr_trace_rays_noalloc(self.h, _dp(o), _dp(d), n, _dp(t), _dp(prim), _stream()))
 
     def bias_field(self, stddev, c_tilde, dt, G=64, M=256) -> torch.Tensor:
         out = torch.empty(G, G, dtype=torch.float64, device="cuda")

@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -918,3 +919,69 @@ dr_status dr_rng_transforms(const uint32_t* words, uint32_t n, float* out, void*
 }
 
 }  // extern "C"
+
+// ---- dr_trace_rays_noalloc (include/dr.h): closest hits without any allocation at call time ---------------------------
+// For callers that may not call cudaMalloc / cudaFree when they trace: a frame loop or a server with a fixed memory budget
+// (an allocation can fail late, cudaFree stalls the whole device), a host whose own pool already owns the GPU's memory, a
+// plugin that must leave its host process's footprint alone.  The kernels are dr_trace_rays' own (k_pack_rays, k_trace,
+// k_unpack_hits); only where their scratch lives differs: in this array, which is part of the library image.  Every GPU
+// that loads the library carries it (2.5 MiB) until the process ends.
+constexpr size_t kNoallocCtlBytes = 256;                                                     // cnt, head (two words) + padding
+constexpr size_t kNoallocQueueBytes = 2 * sizeof(float4) * (size_t)DR_TRACE_NOALLOC_MAX_RAYS; // planes o | d
+constexpr size_t kNoallocHitsBytes = sizeof(uint2) * (size_t)DR_TRACE_NOALLOC_MAX_RAYS;
+constexpr size_t kNoallocBytes = kNoallocCtlBytes + kNoallocQueueBytes + kNoallocHitsBytes;
+
+static __device__ __align__(256) unsigned char g_trace_noalloc_scratch[kNoallocBytes];
+
+namespace {
+
+// In host code the name g_trace_noalloc_scratch is only a handle for the runtime, not a device pointer: a kernel given
+// &g_trace_noalloc_scratch[0] from here would fault (or quietly use host memory where the GPU can reach it).  The device
+// address comes from cudaGetSymbolAddress, asked once per device with that device current, and is kept here.
+constexpr int kNoallocMaxDevices = 64;
+unsigned char* g_noalloc_dev_ptr[kNoallocMaxDevices] = {};
+std::mutex g_noalloc_mutex;
+
+dr_status noalloc_scratch(unsigned char** out) {
+  int device = -1;
+  CUDA_TRY(cudaGetDevice(&device));
+  if (device < 0 || device >= kNoallocMaxDevices) return fail(DR_ERR_UNSUPPORTED, "dr_trace_rays_noalloc: device ordinal above 63");
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_dev_ptr[device]) {
+    void* p = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress(&p, g_trace_noalloc_scratch));   // first call on this device: do it before any stream capture
+    if (!p) return fail(DR_ERR_CUDA, "dr_trace_rays_noalloc: cudaGetSymbolAddress returned a null address");
+    g_noalloc_dev_ptr[device] = static_cast<unsigned char*>(p);
+  }
+  *out = g_noalloc_dev_ptr[device];
+  return DR_OK;
+}
+
+}  // namespace
+
+extern "C" dr_status dr_trace_rays_noalloc(const dr_scene* sc, const float* o, const float* d, uint32_t n, float* t, uint32_t* prim,
+                                           void* stream) {
+  if (!sc) return fail(DR_ERR_INVALID_ARG, "null scene");
+  if (sc->dev.analytic) return fail(DR_ERR_UNSUPPORTED, "analytic scene has no geometry");
+  if (n > DR_TRACE_NOALLOC_MAX_RAYS)
+    return fail(DR_ERR_INVALID_ARG, "dr_trace_rays_noalloc: n = " + std::to_string(n) + " rays exceed the fixed scratch of DR_TRACE_NOALLOC_MAX_RAYS = " +
+                                        std::to_string(DR_TRACE_NOALLOC_MAX_RAYS) + " rays; split the batch or use dr_trace_rays");
+  if (!n) return DR_OK;  // empty input: nothing to do, pointers may be null
+  if (!o || !d || !t || !prim) return fail(DR_ERR_INVALID_ARG, "null argument");
+  unsigned char* base = nullptr;
+  const dr_status st = noalloc_scratch(&base);
+  if (st != DR_OK) return st;
+  cudaStream_t s = (cudaStream_t)stream;
+  uint32_t* ctl = reinterpret_cast<uint32_t*>(base);                                   // [0] = ray count, [1] = k_trace's fetch counter
+  float4* q = reinterpret_cast<float4*>(base + kNoallocCtlBytes);                     // plane o at 0, plane d at n (as dr_trace_rays lays them out)
+  uint2* hits = reinterpret_cast<uint2*>(base + kNoallocCtlBytes + kNoallocQueueBytes);
+  // The array still holds the last call's counters: the fetch counter must start at zero.  Queue and hit entries need no clearing:
+  // k_pack_rays writes entries 0 .. n-1 of both planes and k_trace writes a hit record for each of them before k_unpack_hits reads it.
+  CUDA_TRY(cudaMemsetAsync(ctl, 0, 8, s));
+  const uint32_t g = (n + 255) / 256;
+  k_pack_rays<<<g, 256, 0, s>>>(o, d, n, q, n, ctl);
+  k_trace<false><<<sc->n_sm, kTraceBlock, sc->trace_smem, s>>>(sc->dev, q, n, ctl, ctl + 1, hits, nullptr);
+  k_unpack_hits<<<g, 256, 0, s>>>(sc->dev, hits, n, t, prim);
+  CUDA_TRY(cudaGetLastError());
+  return DR_OK;   // asynchronous: nothing is freed, so there is nothing to wait for
+}
