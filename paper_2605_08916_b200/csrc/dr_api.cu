@@ -284,7 +284,7 @@ dr_status launch_eval(dr_chains* prof, const dr_scene* sc, EvalWs ws, const Eval
     uint32_t h[kCtlWords];
     CUDA_TRY(cudaMemcpyAsync(h, ws.ctl, sizeof(h), cudaMemcpyDeviceToHost, s));
     CUDA_TRY(cudaStreamSynchronize(s));
-    if (h[kCtlWaveError] || h[kCtlWaveDone] != n || h[kCtlWaveReserve] > dev.L * ws.cap)
+    if (h[kCtlWaveError] || h[kCtlWaveDone] != n || h[kCtlWaveReserve] > wave_ring_entries(dev, ws.cap))   // with next-event estimation up to (2L - 1) entries per state
       return fail(DR_ERR_CUDA, "k_wave protocol check failed: error bits " + std::to_string(h[kCtlWaveError]) + ", finished " +
                                    std::to_string(h[kCtlWaveDone]) + " of " + std::to_string(n));
   }

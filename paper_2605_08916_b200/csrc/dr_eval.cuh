@@ -77,10 +77,11 @@ constexpr int kCtlWords = 128;
 // Workspace for up to `cap` states.  Two forms of the same evaluation use it (same results, state by state):
 //  * per-segment loop (k_trace / k_shade): ray queues qa, qb; an entry is three float4 in planes of `cap` entries,
 //      Q0 = (o.xyz, bits(state)), Q1 = (d.xyz, bits(path signature)), Q2 = (T.rgb, bits(refract mask | has_ggx << 16));
-//  * k_wave (dr_wave.cuh): the same three words live in a 64-byte record per STATE (rayrec[4 s + 0..2], the memory of
-//      qa | qb), and `ring` holds one 8-byte entry per ray: (state | (k - 1) << 27, tag of this evaluation).
+//  * k_wave (dr_wave.cuh): the same three words live in a 96-byte record per STATE (kRecWords = 6 float4: qa[kRecWords s + 0..2],
+//      words 3..5 carry the pending emitter connection and the shadow ray of next-event estimation; the memory of qa | qb),
+//      and `ring` holds one 8-byte entry per ray: (state | (k - 1) << 27, tag of this evaluation).
 struct EvalWs {
-  float4* qa;          // 3 * cap; qb = qa + 3 * cap (one allocation of 6 * cap float4: k_wave uses the first 4 * cap as records)
+  float4* qa;          // 3 * cap; qb = qa + 3 * cap (one allocation of 6 * cap float4: k_wave uses all kRecWords * cap of it as records)
   float4* qb;          // 3 * cap
   uint2* hits;         // cap: (bits(t), triangle in leaf order or kMiss)   (loop form)
   uint2* ring;         // wave_ring_entries() ray entries, written once per evaluation, never reused      (k_wave)
@@ -140,6 +141,8 @@ __device__ __forceinline__ void g_pair(const EvalIO& io, uint32_t s, uint32_t k,
 // ---- a3: camera rays -------------------------------------------------------------------------------------------
 // WAVE: the ray goes into the state's record and ring entry t (dr_wave.cuh); otherwise into slot t of queue qa.
 constexpr int kCtlWaveReserve = 48, kCtlWaveHead = 50, kCtlWaveDone = 51;   // control words of k_wave
+constexpr int kCtlWaveError = 52;   // k_wave: bits of the checks that fired (dr_wave.cuh); k_decide (dr_kernels.cuh) counts kErrTimeout into dr_stats.wave_timeouts
+enum : uint32_t { kErrIndex = 1u, kErrState = 2u, kErrOwner = 4u, kErrSegment = 8u, kErrHitRing = 16u, kErrCount = 32u, kErrTimeout = 64u };
 constexpr uint32_t kRecWords = 6;    // float4 per state record of k_wave: ray (o | state, d | signature, T | masks),
                                      // (pending emitter connection | density of the ray's direction), shadow ray (o | emitter id, lobe << 28; d | distance to the sampled point)
 // queue entries an evaluation can need: a path makes at most L rays, and with next-event estimation one shadow ray per vertex

@@ -293,7 +293,7 @@ __global__ void __launch_bounds__(kBlock) k_decide(ChainParams cp, ChainState st
     if (blockIdx.x == 0) {
       atomicAdd(&st.ctr->mutations, (unsigned long long)cp.N);
       st.ctr->iteration = n;
-      if (wave_ctl && (wave_ctl[52] & 64u)) st.ctr->wave_timeouts += 1;   // k_wave's watchdog fired in this iteration's evaluation (dr_wave.cuh)
+      if (wave_ctl && (wave_ctl[kCtlWaveError] & kErrTimeout)) st.ctr->wave_timeouts += 1;   // k_wave's watchdog fired in this iteration's evaluation (dr_wave.cuh)
     }
   }
 }

@@ -48,8 +48,7 @@ namespace dr {
 #ifndef DR_CHECKS
 #define DR_CHECKS 0             // test builds (compute-sanitizer is closed on this pool): device-side checks of the queue protocol;
 #endif                          // a violated check sets a bit of ctl[kCtlWaveError], which the evaluation hooks turn into DR_ERR_CUDA
-constexpr int kCtlWaveError = 52;
-enum : uint32_t { kErrIndex = 1u, kErrState = 2u, kErrOwner = 4u, kErrSegment = 8u, kErrHitRing = 16u, kErrCount = 32u, kErrTimeout = 64u };
+// kCtlWaveError and the kErr* bits are defined beside the other control words in dr_eval.cuh (k_decide reads the watchdog bit too)
 #ifndef DR_WAVE_IDLE_LIMIT
 #define DR_WAVE_IDLE_LIMIT (1u << 25)
 #endif
