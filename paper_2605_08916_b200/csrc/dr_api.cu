@@ -441,6 +441,10 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   s->wave_ok = stack_bytes + kWaveExtraSmem <= kMaxDynSmem;
   e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (d->nee && !s->wave_ok) {   // next-event estimation has no per-segment loop to fall back on: refuse here, not at the first evaluation
+    dr_scene_destroy(s);
+    return fail(DR_ERR_UNSUPPORTED, "next-event estimation runs in k_wave only, and this BVH8 is too deep for k_wave's shared memory");
+  }
   if (e == cudaSuccess) e = wave_allow_smem<TraceBig>();
   if (e == cudaSuccess) e = wave_allow_smem<TraceSmall>();
   if (e != cudaSuccess) {
@@ -711,7 +715,10 @@ dr_status dr_chains_work_stats(dr_chains* c, uint64_t* host_out3, void* stream) 
   return DR_OK;
 }
 
+  uint32_t wave_err = 0;
+  if (!c->scene->dev.analytic) CUDA_TRY(cudaMemcpyAsync(&wave_err, c->ws.ctl + kCtlWaveError, 4, cudaMemcpyDeviceToHost, s));
 dr_status dr_chains_stats(dr_chains* c, dr_stats* o, void* stream) {
+  if (wave_err & kErrTimeout) return fail(DR_ERR_CUDA, "k_wave's watchdog ended the counting evaluation: the counts are incomplete");
   if (!c || !o) return fail(DR_ERR_INVALID_ARG, "null argument");
   Counters h;
   CUDA_TRY(cudaMemcpyAsync(&h, c->st.ctr, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
@@ -865,7 +872,10 @@ dr_status eval_rows(const dr_scene* sc, const float* x, uint32_t n, float* f, fl
   return DR_OK;
 }
 }  // namespace
+  uint32_t wave_err = 0;   // k_wave's watchdog (dr_wave.cuh): an evaluation it ended has written partial results
+  if (!sc->dev.analytic) CUDA_TRY(cudaMemcpyAsync(&wave_err, he.ws.ctl + kCtlWaveError, 4, cudaMemcpyDeviceToHost, s));
 
+  if (wave_err & kErrTimeout) return fail(DR_ERR_CUDA, "k_wave's watchdog ended the evaluation: the outputs are incomplete");
 dr_status dr_eval_states(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score,
                          uint32_t* nrays, uint32_t* sig, void* stream) {
   return dr_eval_states_form(sc, x, n, f, p, pix, score, nrays, sig, 0, stream);

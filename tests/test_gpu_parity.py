@@ -821,3 +821,12 @@ def test_a_lost_ray_ends_in_an_error_not_in_a_hang(dr, tmp_path):
     r = subprocess.run([sys.executable, "-c", _LOST_RAY_SNIPPET.format(root=root)], env=dict(os.environ, DR_LIB=lib), capture_output=True,
                        text=True, timeout=120)
     assert r.returncode == 0 and f"DrError {dr.DR_ERR_CUDA}" in r.stdout, r.stdout + r.stderr
+# the evaluation hook and the counting pass report the watchdog as well (no partial result returned as DR_OK)
+desc = S.closed_furnace()
+x = torch.from_numpy(S.seeded_states(64, desc.dim, 3)).cuda()
+try:
+    dr.Scene(desc).eval_states(x, False, form=2)
+    print("eval: no error")
+except dr.DrError as e:
+    print("eval DrError", e.status)
+    assert f"eval DrError {dr.DR_ERR_CUDA}" in r.stdout, r.stdout + r.stderr
