@@ -105,7 +105,10 @@ typedef struct {
                                 diag(A_block), coordinate pairs (2i, 2i+1); 1 = pairs (4i, 4i+2) and (4i+1, 4i+3) (Q24) */
   uint32_t rho_grid;         /* regeneration density rho (future work L824): 0 = uniform; G in 1..64:
                                 piecewise constant on a G x G tiling of the film coordinates (x0, x1), uniform in the others;
-                                the killing rate becomes (rho / rho_lambda) kappa0 / p_hat */
+                                the killing rate becomes (rho / rho_lambda) kappa0 / p_hat.  Plain Metropolis / MALA never regenerate:
+                                for them rho only sets where the chains START (dr_chains_init draws x ~ rho and the bootstrap of
+                                p_lambda divides by rho); their stationary law is unchanged.  DR_PATH_TRACING averages its samples
+                                with unit weight, so a non-uniform draw would bias it: rho_grid != 0 is DR_ERR_INVALID_ARG there */
   const float* host_rho;     /* G*G tile probabilities, row-major (tile = ty * G + tx), > 0, summing to one (copied) */
 } dr_config;
 

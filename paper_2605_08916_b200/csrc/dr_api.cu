@@ -139,6 +139,8 @@ dr_status check_config(const dr_config* c) {
   if (c->rao_blackwell > 1) return fail(DR_ERR_INVALID_ARG, "rao_blackwell must be 0 or 1");
   if (c->a_mode > 1) return fail(DR_ERR_INVALID_ARG, "a_mode must be 0 or 1");
   if (c->rho_grid > 64) return fail(DR_ERR_INVALID_ARG, "rho_grid must be <= 64");
+  if (c->rho_grid && c->method == DR_PATH_TRACING)   // its samples are averaged with unit weight: a non-uniform first draw would bias the image
+    return fail(DR_ERR_INVALID_ARG, "rho_grid must be 0 for DR_PATH_TRACING (path tracing draws every sample uniformly)");
   if (c->rho_grid) {
     if (!c->host_rho) return fail(DR_ERR_INVALID_ARG, "rho_grid > 0 needs host_rho");
     double sum = 0.0;

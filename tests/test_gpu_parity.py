@@ -527,6 +527,10 @@ def test_sharded_chains_reproduce_the_unsharded_run(dr, torch_):
     parts = []
     for off in (0, 1000):
         ch = dr.Chains(gsc, "diffusion_restore", 1000, seed=4, p_lambda_override=0.05, chain_offset=off)
+    with pytest.raises(dr.DrError):          # path tracing has no regeneration density (include/dr.h rho_grid)
+        dr.Chains(gsc, "path_tracing", 16, rho=np.full((2, 2), 0.25, np.float32))
+    with pytest.raises(ValueError):          # not G x G values: refused before dr_chains_create reads past the array
+        dr.Chains(gsc, "metropolis_restore", 16, rho=np.full(6, 1.0 / 6.0, np.float32))
         ch.init(0)
         ch.step(4)
         parts.append((ch.download(), ch.accum.clone(), ch.stats()["tours"]))
