@@ -65,9 +65,11 @@ template <class Real> struct Scene {
       if (mats[tri_mat[t]].kind != MAT_EMITTER) continue;
       const V c = cross(e1[t], e2[t]);
       const Real a = Real(0.5) * std::sqrt(dot(c, c));
+      if (!(a > Real(0)) || !std::isfinite(a)) continue;   // DESIGN.md Q21: an emitter without area is not on the list (sampling by area gives it probability zero)
       light_total = light_total + a;
       light_tri.push_back(t); light_area.push_back(a); light_cdf.push_back(light_total);
     }
+    if (!(light_total > Real(0))) { light_tri.clear(); light_area.clear(); light_cdf.clear(); light_total = 0; }
   }
 
   uint32_t dim() const { return analytic ? 2u : (nee ? 4u : 2u) * L; }

@@ -248,6 +248,8 @@ class Chains:
         self.scene, self.method, self.N, self.d = scene, method, int(n_chains), scene.dim
         rho_arr = None if rho is None else np.ascontiguousarray(rho, dtype=np.float32).ravel()
         grid = 0 if rho is None else int(round(np.sqrt(rho_arr.size)))
+        if rho is not None and grid * grid != rho_arr.size:     # dr_chains_create reads G * G floats from host_rho
+            raise ValueError(f"rho must hold G x G tile probabilities, got {rho_arr.size} values")
         self.cfg = dr_config(method, self.N, stddev, c_tilde, dt, m, large_step_prob, p_lambda_override, seed, chain_offset,
                              int(bool(rao_blackwell)), int(a_mode), grid, None if rho is None else _np(rho_arr))
         nbytes = lib.dr_chains_state_bytes(scene.h, C.byref(self.cfg))

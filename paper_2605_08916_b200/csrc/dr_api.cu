@@ -441,12 +441,12 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
   }
   s->trace_smem = trace_stack_bytes(dev.stack_cap, kTraceBlock);
   s->wave_ok = stack_bytes + kWaveExtraSmem <= kMaxDynSmem;
-  e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (d->nee && !s->wave_ok) {   // next-event estimation has no per-segment loop to fall back on: refuse here, not at the first evaluation
     dr_scene_destroy(s);
     return fail(DR_ERR_UNSUPPORTED, "next-event estimation runs in k_wave only, and this BVH8 is too deep for k_wave's shared memory");
   }
+  e = cudaFuncSetAttribute(k_trace<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_trace<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
   if (e == cudaSuccess) e = wave_allow_smem<TraceBig>();
   if (e == cudaSuccess) e = wave_allow_smem<TraceSmall>();
   if (e != cudaSuccess) {
@@ -485,6 +485,7 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
       for (int x = 0; x < 3; ++x) { e1[x] = b[x] - a[x]; e2[x] = c[x] - a[x]; }
       cross(e1, e2, cr);
       const float area = 0.5f * std::sqrt(cr[0] * cr[0] + cr[1] * cr[1] + cr[2] * cr[2]);
+      if (!(area > 0.f) || !std::isfinite(area)) continue;   // a degenerate emitter has no normal and no area to sample: it is never picked (nor can a ray hit it)
       const float before = total;
       total = total + area;
       normalize(cr);
@@ -495,8 +496,9 @@ dr_status dr_scene_create(const dr_scene_desc* d, dr_scene** out) {
                              cr[0], cr[1], cr[2], before, m.emission[0], m.emission[1], m.emission[2], 0.f};
       lights.insert(lights.end(), rec, rec + 20);
     }
+    if (!(total > 0.f) || !std::isfinite(total)) lights.clear();   // no emitter area to sample: vertices make no emitter connection (dr_nee.cuh checks n_lights)
     dev.n_lights = (uint32_t)(lights.size() / 20);
-    dev.light_total = total;
+    dev.light_total = dev.n_lights ? total : 0.f;
     dev.lights = nullptr;
     if (dev.n_lights) {
       cudaError_t le = cudaMalloc(&s->d_lights, lights.size() * sizeof(float));
@@ -713,14 +715,14 @@ dr_status dr_chains_work_stats(dr_chains* c, uint64_t* host_out3, void* stream) 
   const dr_status r = launch_eval(nullptr, c->scene, next_ws(c, s), io, c->cp.N, c->cp.grad != 0, true, 0, s);
   if (r != DR_OK) return r;
   CUDA_TRY(cudaMemcpyAsync(host_out3, d.p, 24, cudaMemcpyDeviceToHost, s));
+  uint32_t wave_err = 0;
+  if (!c->scene->dev.analytic) CUDA_TRY(cudaMemcpyAsync(&wave_err, c->ws.ctl + kCtlWaveError, 4, cudaMemcpyDeviceToHost, s));
   CUDA_TRY(cudaStreamSynchronize(s));
+  if (wave_err & kErrTimeout) return fail(DR_ERR_CUDA, "k_wave's watchdog ended the counting evaluation: the counts are incomplete");
   return DR_OK;
 }
 
-  uint32_t wave_err = 0;
-  if (!c->scene->dev.analytic) CUDA_TRY(cudaMemcpyAsync(&wave_err, c->ws.ctl + kCtlWaveError, 4, cudaMemcpyDeviceToHost, s));
 dr_status dr_chains_stats(dr_chains* c, dr_stats* o, void* stream) {
-  if (wave_err & kErrTimeout) return fail(DR_ERR_CUDA, "k_wave's watchdog ended the counting evaluation: the counts are incomplete");
   if (!c || !o) return fail(DR_ERR_INVALID_ARG, "null argument");
   Counters h;
   CUDA_TRY(cudaMemcpyAsync(&h, c->st.ctr, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
@@ -870,14 +872,14 @@ dr_status eval_rows(const dr_scene* sc, const float* x, uint32_t n, float* f, fl
   if (f || p) k_fp_split<<<g, 256, 0, s>>>(he.f4.as<float4>(), p, f, n);
   if (grad) k_planes_to_rows<<<g, 256, 0, s>>>(he.gpl.as<float4>(), score, n, d, planes);
   CUDA_TRY(cudaGetLastError());
+  uint32_t wave_err = 0;   // k_wave's watchdog (dr_wave.cuh): an evaluation it ended has written partial results
+  if (!sc->dev.analytic) CUDA_TRY(cudaMemcpyAsync(&wave_err, he.ws.ctl + kCtlWaveError, 4, cudaMemcpyDeviceToHost, s));
   CUDA_TRY(cudaStreamSynchronize(s));  // the scratch buffers are freed on return
+  if (wave_err & kErrTimeout) return fail(DR_ERR_CUDA, "k_wave's watchdog ended the evaluation: the outputs are incomplete");
   return DR_OK;
 }
 }  // namespace
-  uint32_t wave_err = 0;   // k_wave's watchdog (dr_wave.cuh): an evaluation it ended has written partial results
-  if (!sc->dev.analytic) CUDA_TRY(cudaMemcpyAsync(&wave_err, he.ws.ctl + kCtlWaveError, 4, cudaMemcpyDeviceToHost, s));
 
-  if (wave_err & kErrTimeout) return fail(DR_ERR_CUDA, "k_wave's watchdog ended the evaluation: the outputs are incomplete");
 dr_status dr_eval_states(const dr_scene* sc, const float* x, uint32_t n, float* f, float* p, uint32_t* pix, float* score,
                          uint32_t* nrays, uint32_t* sig, void* stream) {
   return dr_eval_states_form(sc, x, n, f, p, pix, score, nrays, sig, 0, stream);

@@ -276,6 +276,36 @@ def test_teacher_forced_parity_with_nee(dr, oracle, torch_, method, case):
     _teacher_forced(dr, oracle, torch_, method, case)
 
 
+def test_an_emitter_without_area_is_never_sampled_on_the_gpu(dr, oracle, torch_):
+    """DESIGN.md Q21: zero-area emitters are not on the emitter list (the oracle's pin: test_oracle_nee.py).  Appending one
+    changes no evaluation, bit for bit; when it is the only emitter the scene is lit by the environment alone, no vertex
+    makes a connection, and the evaluation matches the oracle's like any other."""
+    import copy
+    from test_oracle_nee import degenerate_emitter_appended
+    base = _nee(S.cornell(width=32, height=32, max_path_len=4))
+    plus = degenerate_emitter_appended(base)
+    x = S.seeded_states(4000, base.dim, 21)
+    x[:2000, 6::4] = np.float32(1.0 - 2.0 ** -24)
+    xg = torch_.from_numpy(x).cuda()
+    a, b = dr.Scene(base).eval_states(xg, True), dr.Scene(plus).eval_states(xg, True)
+    for k in ("f", "p", "pix", "nrays", "sig", "g"):
+        assert torch_.equal(a[k], b[k]), k
+    assert int((a["p"][:2000] > 0).sum()) > 200
+    dark = copy.copy(plus)
+    dark.tri_material = plus.tri_material.copy()
+    dark.tri_material[:-1][plus.tri_material[:-1] == plus.tri_material[-1]] = 0
+    dark.env_radiance = (1.0, 0.5, 0.25)
+    g = dr.Scene(dark).eval_states(xg, True)
+    o = oracle.Scene(dark, oracle.F32).eval(x.astype(np.float64), True)
+    gf, gp, gg = g["f"].cpu().numpy(), g["p"].cpu().numpy(), g["g"].cpu().numpy()
+    assert np.isfinite(gf).all() and np.isfinite(gg).all() and not o["nonfinite"].any()
+    same = g["sig"].cpu().numpy().view(np.uint32) == o["sig"]
+    assert same.mean() > 0.999 and (gp[same] > 0).mean() > 0.3
+    assert np.array_equal(g["pix"].cpu().numpy()[same], o["pix"][same])
+    assert np.allclose(gf[same], o["f"][same], rtol=1e-4, atol=1e-6) and np.allclose(gp[same], o["p"][same], rtol=1e-4, atol=1e-6)
+    assert not gg.reshape(len(x), -1, 4)[:, :, 2:].any()     # no connection anywhere: the emitter coordinates carry no score
+
+
 EXTRA = [("path_tracing", {}), ("metropolis_restore", dict(rao_blackwell=True)), ("mala_restore", dict(rao_blackwell=True)),
          ("diffusion_restore", dict(rao_blackwell=True))]
 
@@ -497,6 +527,10 @@ def test_edge_cases(dr, torch_):
                 dict(rho=np.full((3, 3), 0.2, np.float32)), dict(rho=np.array([[0.5, 0.5], [0.0, 0.0]], np.float32))):
         with pytest.raises(dr.DrError):
             dr.Chains(gsc, "metropolis", 16, **bad)
+    with pytest.raises(dr.DrError):          # path tracing has no regeneration density (include/dr.h rho_grid)
+        dr.Chains(gsc, "path_tracing", 16, rho=np.full((2, 2), 0.25, np.float32))
+    with pytest.raises(ValueError):          # not G x G values: refused before dr_chains_create reads past the array
+        dr.Chains(gsc, "metropolis_restore", 16, rho=np.full(6, 1.0 / 6.0, np.float32))
     bad_desc = S.furnace()
     bad_desc.vertices = bad_desc.vertices.copy()
     bad_desc.vertices[0, 0] = np.inf
@@ -527,10 +561,6 @@ def test_sharded_chains_reproduce_the_unsharded_run(dr, torch_):
     parts = []
     for off in (0, 1000):
         ch = dr.Chains(gsc, "diffusion_restore", 1000, seed=4, p_lambda_override=0.05, chain_offset=off)
-    with pytest.raises(dr.DrError):          # path tracing has no regeneration density (include/dr.h rho_grid)
-        dr.Chains(gsc, "path_tracing", 16, rho=np.full((2, 2), 0.25, np.float32))
-    with pytest.raises(ValueError):          # not G x G values: refused before dr_chains_create reads past the array
-        dr.Chains(gsc, "metropolis_restore", 16, rho=np.full(6, 1.0 / 6.0, np.float32))
         ch.init(0)
         ch.step(4)
         parts.append((ch.download(), ch.accum.clone(), ch.stats()["tours"]))
@@ -809,6 +839,14 @@ try:
     print("no error")
 except dr.DrError as e:
     print("DrError", e.status, ch.lib_stats_timeouts() if hasattr(ch, "lib_stats_timeouts") else "")
+# the evaluation hook and the counting pass report the watchdog as well (no partial result returned as DR_OK)
+desc = S.closed_furnace()
+x = torch.from_numpy(S.seeded_states(64, desc.dim, 3)).cuda()
+try:
+    dr.Scene(desc).eval_states(x, False, form=2)
+    print("eval: no error")
+except dr.DrError as e:
+    print("eval DrError", e.status)
 """
 
 
@@ -825,12 +863,4 @@ def test_a_lost_ray_ends_in_an_error_not_in_a_hang(dr, tmp_path):
     r = subprocess.run([sys.executable, "-c", _LOST_RAY_SNIPPET.format(root=root)], env=dict(os.environ, DR_LIB=lib), capture_output=True,
                        text=True, timeout=120)
     assert r.returncode == 0 and f"DrError {dr.DR_ERR_CUDA}" in r.stdout, r.stdout + r.stderr
-# the evaluation hook and the counting pass report the watchdog as well (no partial result returned as DR_OK)
-desc = S.closed_furnace()
-x = torch.from_numpy(S.seeded_states(64, desc.dim, 3)).cuda()
-try:
-    dr.Scene(desc).eval_states(x, False, form=2)
-    print("eval: no error")
-except dr.DrError as e:
-    print("eval DrError", e.status)
     assert f"eval DrError {dr.DR_ERR_CUDA}" in r.stdout, r.stdout + r.stderr

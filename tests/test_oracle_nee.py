@@ -147,3 +147,46 @@ def test_score_matches_finite_differences_with_nee(oracle):
             assert np.allclose(e["g"][i], g2, rtol=1e-3, atol=1e-3 * (1 + np.abs(g2).max())), (desc.name, i, e["g"][i], g2)
         assert checked >= 15, (desc.name, checked)
         assert (np.abs(e["g"][lit]).max(1) > 0).mean() > 0.9              # with NEE the score is live on diffuse paths too
+
+
+def degenerate_emitter_appended(desc):
+    """The same scene with one more emitter triangle, of zero area (three times the same vertex), LAST in triangle order."""
+    d = copy.copy(desc)
+    light = int(np.flatnonzero(desc.materials[:, 0] == 3)[0])
+    nv = len(desc.vertices)
+    d.vertices = np.concatenate([desc.vertices, np.array([[0.5, 0.5, 0.5]], dtype=np.float32)])
+    d.indices = np.concatenate([desc.indices, np.array([[nv, nv, nv]], dtype=np.uint32)])
+    d.tri_material = np.concatenate([desc.tri_material, np.array([light], dtype=np.uint32)])
+    return d
+
+
+def test_an_emitter_without_area_is_never_sampled(oracle):
+    """DESIGN.md Q21 (emitters are drawn by area; PAPER.md L735, L757 leave the construction open): a zero-area emitter has
+    probability zero.  Appending one to a scene changes nothing, also with v1 at the top of [0, 1); and when it is the ONLY
+    emitter no vertex makes a connection: the evaluation is that of the direction sample alone, not 0/0."""
+    base = nee_scene(S.cornell(width=32, height=32, max_path_len=4))
+    plus = degenerate_emitter_appended(base)
+    x = S.seeded_states(4000, base.dim, 21).astype(np.float64)
+    x[:2000, 6::4] = 1.0 - 2.0 ** -24                      # v1 of every vertex at the top of [0, 1)
+    for prec in (oracle.F32, oracle.F64):
+        a = oracle.Scene(base, prec, use_bvh=False).eval(x, True)
+        b = oracle.Scene(plus, prec, use_bvh=False).eval(x, True)
+        assert not b["nonfinite"].any()
+        for k in ("f", "p", "pix", "sig", "g"):
+            assert np.array_equal(a[k], b[k]), k
+        assert (a["p"][:2000] > 0).sum() > 200             # the corner case is exercised on lit paths
+    # the only emitter has no area: light comes from the environment alone
+    dark = copy.copy(plus)
+    dark.tri_material = plus.tri_material.copy()
+    dark.tri_material[:-1][plus.tri_material[:-1] == plus.tri_material[-1]] = 0     # the ceiling light becomes a white wall
+    dark.env_radiance = (1.0, 0.5, 0.25)
+    plain = copy.copy(dark)
+    plain.nee = False
+    xp = np.ascontiguousarray(x.reshape(len(x), -1, 4)[:, :, :2].reshape(len(x), -1))   # (u1, u2) of every vertex
+    for prec in (oracle.F32, oracle.F64):
+        a = oracle.Scene(dark, prec, use_bvh=False).eval(x, True)
+        b = oracle.Scene(plain, prec, use_bvh=False).eval(xp, True)
+        assert not a["nonfinite"].any() and (a["p"] > 0).mean() > 0.3
+        assert np.array_equal(a["f"], b["f"]) and np.array_equal(a["pix"], b["pix"])
+        g = a["g"].reshape(len(x), -1, 4)
+        assert np.array_equal(np.ascontiguousarray(g[:, :, :2]).reshape(len(x), -1), b["g"]) and not g[:, :, 2:].any()
