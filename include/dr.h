@@ -112,6 +112,16 @@ typedef struct {
   const float* host_rho;     /* G*G tile probabilities, row-major (tile = ty * G + tx), > 0, summing to one (copied) */
 } dr_config;
 
+/* The paper's parameters for `method`, for C callers and the binding alike: zeroes *host_out, then sets method and
+ *   stddev           1e-2 for Metropolis and Metropolis-Restore, 5e-3 for the Langevin-based samplers; a stddev
+ *                    argument > 0 replaces it
+ *   large_step_prob  0.3 for plain Metropolis / MALA, 0 otherwise (L747)
+ *   dt = 1e-5 (L755), m = 64 (L754)
+ *   c_tilde          stddev^2 / 2 of the stddev in use: this build's default rotation strength (Q10; the paper gives none)
+ * n_chains, seed and the other fields stay zero for the caller to fill in.  DR_ERR_INVALID_ARG for an unknown method, a null
+ * pointer or a stddev that is not finite. */
+dr_status dr_config_default(int32_t method, double stddev, dr_config* host_out);
+
 typedef struct {
   uint64_t tours;            /* tourCount */
   uint64_t mutations;        /* Accumulate calls = chain-iterations, init included */

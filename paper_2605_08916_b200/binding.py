@@ -26,7 +26,7 @@ EXPORTS = [
     "dr_trace_rays", "dr_eval_states", "dr_philox_blocks", "dr_rng_transforms", "dr_resolve_image_sharded",
     "dr_eval_work_stats", "dr_profile_enable", "dr_profile_read", "dr_chains_work_stats", "dr_eval_states_form",
     "dr_chains_set_eval_form", "dr_frame_floats", "dr_pack_frame", "dr_resolve_image_packed",
-    "dr_bias_field", "dr_trace_rays_noalloc",
+    "dr_bias_field", "dr_trace_rays_noalloc", "dr_config_default",
 ]
 TRACE_NOALLOC_MAX_RAYS = 65536   # DR_TRACE_NOALLOC_MAX_RAYS of include/dr.h
 PROF_NAMES = ["propose", "raygen", "trace", "shade", "grad", "decide", "scan", "scatter", "resolve"]
@@ -100,6 +100,7 @@ def _load():
     L.dr_regen_queue_download.argtypes = [vp, vp, C.POINTER(u32), vp]
     L.dr_trace_rays.argtypes = [vp, vp, vp, u32, vp, vp, vp]
     L.dr_trace_rays_noalloc.argtypes = [vp, vp, vp, u32, vp, vp, vp]
+    L.dr_config_default.argtypes = [i32, C.c_double, vp]
     L.dr_eval_states.argtypes = [vp, vp, u32, vp, vp, vp, vp, vp, vp, vp]
     L.dr_eval_states_form.argtypes = [vp, vp, u32, vp, vp, vp, vp, vp, vp, i32, vp]
     L.dr_chains_set_eval_form.argtypes = [vp, i32]
@@ -236,15 +237,16 @@ class Scene:
 class Chains:
     """dr_chains_create over caller-owned torch memory + the per-frame calls."""
 
-    def __init__(self, scene: Scene, method, n_chains, stddev=None, c_tilde=None, dt=1e-5, m=64.0, large_step_prob=None,
+    def __init__(self, scene: Scene, method, n_chains, stddev=None, c_tilde=None, dt=None, m=None, large_step_prob=None,
                  p_lambda_override=0.0, seed=0, chain_offset=0, rao_blackwell=False, a_mode=0, rho=None):
         method = METHODS[method] if isinstance(method, str) else int(method)
-        if stddev is None:
-            stddev = 1e-2 if method in (0, 2) else 5e-3        # PAPER.md L747
-        if c_tilde is None:
-            c_tilde = 0.5 * stddev * stddev                     # DESIGN.md Q10
-        if large_step_prob is None:
-            large_step_prob = 0.3 if method in (0, 1) else 0.0  # PAPER.md L747
+        dflt = dr_config()                                      # the method's parameters live in the library (dr_config_default)
+        _check(lib.dr_config_default(method, 0.0 if stddev is None else float(stddev), C.byref(dflt)))
+        stddev = dflt.stddev if stddev is None else stddev
+        c_tilde = dflt.c_tilde if c_tilde is None else c_tilde
+        dt = dflt.dt if dt is None else dt
+        m = dflt.m if m is None else m
+        large_step_prob = dflt.large_step_prob if large_step_prob is None else large_step_prob
         self.scene, self.method, self.N, self.d = scene, method, int(n_chains), scene.dim
         rho_arr = None if rho is None else np.ascontiguousarray(rho, dtype=np.float32).ravel()
         grid = 0 if rho is None else int(round(np.sqrt(rho_arr.size)))

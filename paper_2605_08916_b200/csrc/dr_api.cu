@@ -550,6 +550,22 @@ dr_status dr_scene_get_info(const dr_scene* s, dr_scene_info* o) {
   return DR_OK;
 }
 
+dr_status dr_config_default(int32_t method, double stddev, dr_config* out) {
+  if (!out) return fail(DR_ERR_INVALID_ARG, "null argument");
+  if (method < 0 || method > DR_PATH_TRACING) return fail(DR_ERR_INVALID_ARG, "method out of range");
+  if (!std::isfinite(stddev)) return fail(DR_ERR_INVALID_ARG, "stddev must be finite");
+  std::memset(out, 0, sizeof(*out));
+  const bool random_walk = method == DR_METROPOLIS || method == DR_METROPOLIS_RESTORE;
+  const double s = stddev > 0.0 ? stddev : (random_walk ? 1e-2 : 5e-3);
+  out->method = method;
+  out->stddev = (float)s;
+  out->c_tilde = (float)(0.5 * s * s);                                                                  // DESIGN.md Q10, in double like the caller's own s^2 / 2 would be
+  out->dt = 1e-5f;                                                                                      // L755
+  out->m = 64.f;                                                                                        // L754
+  out->large_step_prob = (method == DR_METROPOLIS || method == DR_MALA) ? 0.3f : 0.f;                   // L747
+  return DR_OK;
+}
+
 size_t dr_chains_state_bytes(const dr_scene* s, const dr_config* c) {
   if (!s || check_config(c) != DR_OK) return 0;
   const bool grad = c->method == DR_MALA || c->method == DR_MALA_RESTORE || c->method == DR_DIFFUSION_RESTORE;

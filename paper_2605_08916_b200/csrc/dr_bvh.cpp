@@ -1,6 +1,7 @@
 // Host-side acceleration-structure build: binned-SAH BVH2, collapsed to a BVH8, children placed in octant
 // slots, child boxes quantised to 8 bits per plane (80-byte nodes, dr_types.h), emitted breadth-first so that
-// the top levels are contiguous (the traversal kernel stages them in shared memory).
+// the top levels are contiguous (they stay in L1 / L2; staging them in shared memory was measured in round 1 and
+// removed: profiles/r01f_k_trace_full.md, step r01e).
 // The paper uses a hardware ray-tracing pipeline; B200 has no RT cores, so the closest-hit
 // query of row a4 runs in software over this structure.  The compressed wide node with octant-ordered
 // traversal follows the published idea of Ylitie, Karras and Laine (HPG 2017), restated here from scratch.
@@ -335,7 +336,7 @@ void build_bvh8(const float* verts, uint32_t nv, const uint32_t* idx, uint32_t n
   // and Laine 2017): cost[n][i] = least SAH cost of representing the subtree of n by at most i + 1 roots (leaves of at most
   // kMaxLeafTris references, or BVH8 nodes), area(n) * kCostNode per node and area * refs * kCostTri per leaf.  The BVH2 is
   // built down to single references, so the programme also decides what a leaf is.  Otherwise: greedy, open the child of
-  // largest area until there are eight.  Measured on configs[3]: profiles/r02b_bvh_collapse.md.
+  // largest area until there are eight.  Measured on configs[3]: profiles/r02b_tuning.md (BVH collapse table).
   constexpr int kW = 8;
   const size_t nn2 = n2.size();
   std::vector<float> cost;          // [n * 7 + i], i = 0..6: at most i + 1 roots

@@ -6,8 +6,8 @@
 
 namespace dr {
 
-constexpr int kMaxPathLen = 16;        // L <= 16, d = 2L <= 32 (BASELINE.json configs[3])
-constexpr int kMaxPlanes = 8;          // d / 4 float4 planes
+constexpr int kMaxPathLen = 16;        // L <= 16: d = 2L <= 32 (BASELINE.json configs[3]), or d = 4L <= 64 with next-event estimation
+                                       // (Q21); the state is stored in d / 4 float4 planes (DevScene::planes)
 constexpr int kMaxMix = 16;
 constexpr int kMaxLeafTris = 3;        // triangles per leaf (three bits per slot in the node's triangle mask)
 constexpr int kMaxBvhDepth = 30;       // upper bound; what the traversal stacks in shared memory allow is checked by dr_scene_create

@@ -33,6 +33,32 @@ def test_binding_lists_the_same_names():
     assert ctypes.sizeof(binding.dr_scene_info) == 32
 
 
+def test_config_default_holds_the_papers_parameters():
+    """dr_config_default (host-only, no GPU): PAPER.md L747 (stddev 1e-2 for the random-walk samplers, 5e-3 for the Langevin-based
+    ones; large steps with probability 0.3 for plain Metropolis / MALA), L754-L755 (m = 64, dt = 1e-5), Q10 (c~ = s^2 / 2)."""
+    import numpy as np
+    from paper_2605_08916_b200 import build
+    build.build()
+    from paper_2605_08916_b200 import binding
+    lib = ctypes.CDLL(build.build())
+    lib.dr_config_default.argtypes = [ctypes.c_int32, ctypes.c_double, ctypes.c_void_p]
+    f32 = np.float32
+    for method in range(6):
+        c = binding.dr_config()
+        c.n_chains, c.seed, c.rho_grid = 7, 9, 3                      # overwritten: the call zeroes the struct first
+        assert lib.dr_config_default(method, 0.0, ctypes.byref(c)) == 0
+        s = 1e-2 if method in (0, 2) else 5e-3
+        assert c.method == method and f32(c.stddev) == f32(s) and f32(c.c_tilde) == f32(0.5 * s * s)
+        assert f32(c.dt) == f32(1e-5) and c.m == 64.0 and f32(c.large_step_prob) == f32(0.3 if method in (0, 1) else 0.0)
+        assert (c.n_chains, c.seed, c.chain_offset, c.rao_blackwell, c.a_mode, c.rho_grid, c.host_rho) == (0, 0, 0, 0, 0, 0, None)
+        assert c.p_lambda_override == 0.0
+        assert lib.dr_config_default(method, 0.02, ctypes.byref(c)) == 0   # the caller's step width, and the rotation that goes with it
+        assert f32(c.stddev) == f32(0.02) and f32(c.c_tilde) == f32(0.5 * 0.02 * 0.02)
+    c = binding.dr_config()
+    assert lib.dr_config_default(6, 0.0, ctypes.byref(c)) == -1 and lib.dr_config_default(-1, 0.0, ctypes.byref(c)) == -1
+    assert lib.dr_config_default(0, float("nan"), ctypes.byref(c)) == -1 and lib.dr_config_default(0, 0.0, None) == -1
+
+
 def test_product_path_does_not_touch_the_oracle():
     """The oracle is test infrastructure: nothing in the package or the inputs module imports it."""
     for folder in ("paper_2605_08916_b200", "dr_inputs"):

@@ -96,10 +96,11 @@ def test_trace_matches_oracle(dr, oracle, torch_, scene):
     hit = (~mism) & (otri >= 0)
     assert hit.sum() > 1000
     diag = float(np.linalg.norm(desc.vertices.max(0) - desc.vertices.min(0)))
-    assert np.all(np.abs(t[hit] - ot[hit]) <= 1e-5 * np.maximum(np.abs(ot[hit]), 0.25 * diag))   # fp32 Moeller-Trumbore on both sides
+    # fp32 Moeller-Trumbore on both sides: its error scales with the scene extent, not with t (Q8, measured fp32-vs-fp64 numbers there)
+    assert np.all(np.abs(t[hit] - ot[hit]) <= 1e-5 * np.maximum(np.abs(ot[hit]), 0.25 * diag))
     assert np.all(t[(~mism) & (otri < 0)] == -1.0)
     info = gsc.info()
-    assert info["n_tris"] == desc.n_tris and info["n_nodes"] >= 1 and info["smem_nodes"] <= 585
+    assert info["n_tris"] == desc.n_tris and info["n_nodes"] >= 1 and info["smem_nodes"] == 0
 
 
 def test_trace_degenerate_rays(dr, oracle, torch_):

@@ -100,7 +100,9 @@ def test_kill_probability_law(oracle):
     """Race of Alg. 1: P(killed) = kappa / (lambda + kappa).  Uniform target, kappa0 = p_lambda/(m dt)
     => 1/(m+1) per event (golden); also a non-trivial ratio with kappa = 4 lambda."""
     sc = oracle.Scene(uniform_scene(), oracle.F64)
-    for meth, m, want in [("diffusion_restore", 64.0, 1 / 65), ("metropolis_restore", 64.0, 1 / 65),
+    (m_gold, p_gold), = [(float(r[1]), float(r[2])) for r in rows("rates.txt") if r[0] == "kill_prob_uniform"]
+    assert m_gold == 64.0 and abs(p_gold - 1 / 65) < 1e-15
+    for meth, m, want in [("diffusion_restore", m_gold, p_gold), ("metropolis_restore", m_gold, p_gold),
                           ("mala_restore", 0.25, 0.8), ("diffusion_restore", 1.0, 0.5)]:
         ch = oracle.Chains(sc, meth, 20000, m=m, seed=11)
         ch.init(0)
@@ -111,6 +113,28 @@ def test_kill_probability_law(oracle):
         assert n == 20000 * 10
         frac = st["tours"] / n
         assert abs(frac - want) < 5 * np.sqrt(want * (1 - want) / n), (meth, frac, want)
+
+
+def test_killing_rate_is_kappa0_over_p_hat(oracle):
+    """kappa = kappa0 / p_hat for uniform rho; golden row S:L279: kappa0 = 4, p = 2 -> kappa = 2.  On a constant
+    target of luminance p with lambda = 1 (Metropolis-Restore) the race of Alg. 1 kills with probability
+    kappa / (1 + kappa), which the tour count of a run shows."""
+    (kappa0, p, kappa), = [tuple(float(v) for v in r[1:]) for r in rows("rates.txt") if r[0] == "kappa"]
+    assert kappa0 / p == kappa
+    desc = uniform_scene()
+    desc.env_radiance = (p, p, p)
+    sc = oracle.Scene(desc, oracle.F64)
+    ch = oracle.Chains(sc, "metropolis_restore", 20000, m=1.0, p_lambda_override=kappa0, seed=13)   # kappa0 = p_lambda / (m dt), dt := 1
+    ch.init(0)
+    assert np.allclose(ch.state()["p"], p, rtol=1e-12)
+    ch.step(9)
+    st = ch.stats()
+    assert np.isclose(st["kappa0"], kappa0, rtol=1e-12) and st["lambda"] == 1.0
+    n, want = st["mutations"], kappa / (1.0 + kappa)
+    assert abs(st["tours"] / n - want) < 5 * np.sqrt(want * (1 - want) / n), (st["tours"] / n, want)
+    # and the sampled weights: E[dtau] = 1 / (lambda + kappa), so sum w / p_hat over the run = n / ((1 + kappa) p) within 5 s.e.
+    acc = ch.accum()[:, 3].sum()
+    assert abs(acc / n * (1.0 + kappa) * p - 1.0) < 5 / np.sqrt(n), acc
 
 
 def test_uniform_target_resolves_to_one_and_tours_are_geometric(oracle):
