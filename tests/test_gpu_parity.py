@@ -307,6 +307,76 @@ def test_an_emitter_without_area_is_never_sampled_on_the_gpu(dr, oracle, torch_)
     assert not gg.reshape(len(x), -1, 4)[:, :, 2:].any()     # no connection anywhere: the emitter coordinates carry no score
 
 
+# ---- Q18: non-finite f or score -> zero-contribution state, counted -------------------------------------------------------
+def test_q18_overflowing_f_is_zeroed_on_the_same_states(dr, oracle, torch_):
+    """DESIGN.md Q18.  The oracle's branch is pinned by fp64 in test_oracle_q18.py; here the kernels
+    (finish_path, k_grad) against it on the closed box with albedo 2 and a 1e38 emitter: the same states are zeroed, with and
+    without the score, and the chain counters agree."""
+    from test_oracle_q18 import overflow_box
+    desc = overflow_box()
+    gsc, osc = dr.Scene(desc), oracle.Scene(desc, oracle.F32)
+    x = S.seeded_states(4000, desc.dim, 31)
+    for want_score in (False, True):
+        g = gsc.eval_states(torch_.from_numpy(x).cuda(), want_score)
+        o = osc.eval(x.astype(np.float64), want_score)
+        same = g["sig"].cpu().numpy().view(np.uint32) == o["sig"]
+        assert same.mean() > 0.999
+        gf, gp = g["f"].cpu().numpy(), g["p"].cpu().numpy()
+        flagged = o["nonfinite"].astype(bool)
+        assert flagged[same].sum() > 500
+        assert not gf[same & flagged].any() and not gp[same & flagged].any()               # zeroed where the oracle zeroes
+        keep = same & ~flagged
+        assert np.array_equal(gp[keep] > 0, o["p"][keep] > 0) and (gp[keep] > 0).sum() > 300  # and nowhere else
+        assert np.allclose(gf[keep], o["f"][keep], rtol=1e-4) and np.isfinite(gf).all()
+        if want_score:
+            gg = g["g"].cpu().numpy()
+            assert not gg[same & flagged].any() and np.isfinite(gg).all()
+    # counters and one step of plain Metropolis with fresh uniform proposals: same decisions
+    N = 3000
+    kw = dict(seed=5, large_step_prob=1.0)
+    for method in ("metropolis", "mala"):
+        gch, och = dr.Chains(gsc, method, N, **kw), oracle.Chains(osc, method, N, **kw)
+        gch.init(1)
+        och.init(1)
+        gst, ost = gch.stats(), och.stats()
+        assert gst["nonfinite"] == ost["nonfinite"] > 500
+        assert np.isclose(gst["p_lambda"], ost["p_lambda"], rtol=2e-6)
+        gch.step(1)
+        och.step(1)
+        gs, os_ = gch.download(), och.state()
+        assert gch.stats()["nonfinite"] == och.stats()["nonfinite"] > ost["nonfinite"]
+        assert (gs["x"].astype(np.float64) == os_["x"]).all()                                # large steps only: the states are exact uniforms
+        assert np.array_equal(gch.last_step()[0].astype(bool), och.last()[0].astype(bool))
+        assert np.allclose(gs["p"], os_["p"], rtol=1e-5)
+        assert np.isfinite(gch.accum.cpu().numpy()).all()
+
+
+def test_q18_overflowing_score_is_zeroed_like_the_oracle(dr, oracle, torch_):
+    """Only the score overflows (GGX room, 1e38 emitters).  The oracle differentiates forwards, k_grad backwards, so fp32 leaves
+    its range at slightly different points of the two computations: the states are compared by what fp64 says about them.  Both
+    sides zero every state whose |grad p| exceeds FLT_MAX by a factor 16 and none below FLT_MAX / 16; in between either may."""
+    from test_oracle_q18 import FLT_MAX, bright_ggx_room
+    desc = bright_ggx_room()
+    gsc, o32, o64 = dr.Scene(desc), oracle.Scene(desc, oracle.F32), oracle.Scene(desc, oracle.F64)
+    x = S.seeded_states(60000, desc.dim, 32)
+    g = gsc.eval_states(torch_.from_numpy(x).cuda(), True)
+    a, b = o32.eval(x.astype(np.float64), True), o64.eval(x.astype(np.float64), True)
+    gf, gp, gg = g["f"].cpu().numpy(), g["p"].cpu().numpy(), g["g"].cpu().numpy()
+    assert np.isfinite(gf).all() and np.isfinite(gg).all()
+    same = (g["sig"].cpu().numpy().view(np.uint32) == b["sig"]) & (a["sig"] == b["sig"])
+    grad_p = np.abs(b["g"]).max(1) * (b["p"] + 1e-8)
+    lit = same & (b["p"] > 0)
+    g_flag, o_flag = lit & (gp == 0), lit & a["nonfinite"].astype(bool)
+    must, must_not = lit & (grad_p > 16 * FLT_MAX), lit & (grad_p < FLT_MAX / 16)
+    print(f"Q18 score overflow: gpu zeroed {g_flag.sum()}, oracle zeroed {o_flag.sum()}, both {(g_flag & o_flag).sum()}, "
+          f"|grad p| > 16 FLT_MAX: {must.sum()}, in between: {(lit & ~must & ~must_not).sum()}")
+    assert g_flag[must].all() and o_flag[must].all() and not g_flag[must_not].any() and not o_flag[must_not].any()
+    assert must_not.sum() > 1000 and (g_flag | o_flag).sum() >= 10
+    assert not gf[g_flag].any() and not gg[g_flag].any()
+    keep = lit & ~g_flag & ~o_flag
+    assert np.allclose(gf[keep], a["f"][keep], rtol=1e-4)
+
+
 EXTRA = [("path_tracing", {}), ("metropolis_restore", dict(rao_blackwell=True)), ("mala_restore", dict(rao_blackwell=True)),
          ("diffusion_restore", dict(rao_blackwell=True))]
 
