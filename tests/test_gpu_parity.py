@@ -6,7 +6,7 @@ from dr_inputs import scenes as S
 
 pytestmark = pytest.mark.gpu
 
-from gpu_util import METHODS, compare_bulk, compare_states, min_image  # noqa: E402
+from gpu_util import METHODS, compare_bulk, compare_states, min_image, three_way  # noqa: E402
 
 
 @pytest.fixture(scope="module")
@@ -204,25 +204,25 @@ def test_eval_matches_oracle(dr, oracle, torch_, scene):
     assert div.mean() < 1e-3, div.sum()                                         # near-threshold decisions: counted
     ok = ~div
     assert (g["nrays"][ok] == e["nrays"][ok]).all()
+    stddev = 5e-3
+    relp = np.abs(g["p"] - e["p"]) / np.maximum(e["p"], 1e-8)
+    relf = (np.abs(g["f"] - e["f"]) / np.maximum(np.abs(e["f"]), 1e-8)).max(1)
+    badg = (np.abs(g["g"] - e["g"]) > 1e-4 * np.abs(e["g"]) + 2e-4 / stddev).any(1)
     if scene.endswith("_nee"):
         # a connection that grazes the emitter (cos_l -> 0) or is very short divides by a cancelled quantity: fp32 on either
-        # side then carries a relative error far above its usual 1e-7.  Such states are counted with the diverged ones.
-        ill = np.abs(g["p"] - e["p"]) > 1e-4 * np.maximum(e["p"], 1e-8)
-        assert (div | ill).mean() < 1e-3, (div.sum(), ill.sum())
-        ok &= ~ill
-    rel = np.abs(g["p"][ok] - e["p"][ok]) / np.maximum(e["p"][ok], 1e-8)
-    assert rel.max() <= 1e-4, rel.max()
-    relf = np.abs(g["f"][ok] - e["f"][ok]) / np.maximum(np.abs(e["f"][ok]), 1e-8)
-    assert relf.max() <= 1e-4
-    stddev = 5e-3
-    tol = 1e-4 * np.abs(e["g"][ok]) + 2e-4 / stddev
-    bad = np.abs(g["g"][ok] - e["g"][ok]) > tol
-    if scene.endswith("_nee"):      # the same near-singular connections, seen through the derivative of 1 / cos_l and 1 / r^2
-        assert (div.sum() + ill.sum() + bad.any(1).sum()) < 1e-3 * n, (div.sum(), ill.sum(), bad.any(1).sum())
-        rel_g = np.abs(g["g"][ok] - e["g"][ok])[bad] / np.abs(e["g"][ok][bad])
-        assert (rel_g < 5e-2).all(), rel_g                                      # and even there a relative error of per cent
-    else:
-        assert not bad.any(), (int(bad.sum()), float(np.abs(g["g"][ok] - e["g"][ok]).max()))
+        # side then carries a relative error far above its usual 1e-7.  Every state whose values differ is judged against the
+        # fp64 oracle (gpu_util.three_way): ill-conditioned or on a decision boundary of the fp64 path -> counted; else a defect.
+        idx = np.flatnonzero(ok & ((relp > 1e-4) | (relf > 1e-4) | badg))
+        if len(idx):
+            ill, other, e_gpu, e_orc, sens = three_way(oracle.Scene(desc, oracle.F64), dict(g, x=x), dict(e, x=x.astype(np.float64)), idx, stddev)
+            defect = ~(ill | other)
+            print(f"{scene}: {int(div.sum())} discrete, {int(ill.sum())} ill-conditioned, {int(other.sum())} on an fp64 decision boundary")
+            assert not defect.any(), (idx[defect][:8], e_gpu[defect][:8], e_orc[defect][:8], sens[defect][:8])
+        assert div.sum() + len(idx) < 1e-3 * n, (div.sum(), len(idx))
+        ok[idx] = False
+    assert relp[ok].max() <= 1e-4, relp[ok].max()
+    assert relf[ok].max() <= 1e-4
+    assert not badg[ok].any(), (int(badg[ok].sum()), float(np.abs(g["g"][ok] - e["g"][ok]).max()))
     if scene in ("mini_machines", "ggx_room") or scene.endswith("_nee"):
         assert (np.abs(e["g"][ok]).max(1) > 0).sum() > 20                       # the score path is exercised
     if scene.endswith("_nee"):
@@ -500,8 +500,8 @@ def _teacher_forced(dr, oracle, torch_, method, case, **kw):
     assert np.isclose(gst["p_lambda"], ost["p_lambda"], rtol=2e-6) and np.isclose(gst["kappa0"], ost["kappa0"], rtol=2e-6)
     assert gst["mutations"] == ost["mutations"] == N
     g_last, o_last = gch.last_step(), och.last()
-    fold = bool(getattr(desc, "nee", False))
-    div, rep = compare_states(gs, os_, g_last, o_last, stddev, fold_outliers=fold)
+    osc64 = oracle.Scene(desc, oracle.F64) if getattr(desc, "nee", False) else None   # judges value differences three ways (gpu_util.three_way)
+    div, rep = compare_states(gs, os_, g_last, o_last, stddev, osc64=osc64)
     assert div.mean() < 1e-3, rep
     nr_g, nr_o = gsc.eval_states(torch_.from_numpy(gs["x"]).cuda(), False)["nrays"].cpu().numpy(), osc.eval(os_["x"], False)["nrays"]
     assert gst["rays"] == int(nr_g.sum()) and ost["rays"] == int(nr_o.sum()) and (nr_g[~div] == nr_o[~div]).all()   # closest-hit queries: counted exactly
@@ -520,7 +520,7 @@ def _teacher_forced(dr, oracle, torch_, method, case, **kw):
         och.step(1)
         gs, os_ = gch.download(), och.state()
         g_last, o_last = gch.last_step(), och.last()
-        div, rep = compare_states(gs, os_, g_last, o_last, stddev, fold_outliers=fold)
+        div, rep = compare_states(gs, os_, g_last, o_last, stddev, osc64=osc64)
         worst = max(worst, rep["frac"])
         assert div.mean() < 1e-3, (method, name, burst, rep)
         compare_bulk(gch, och, gs, os_, g_last, o_last, div, gch.stats()["tours"] - t0g, och.stats()["tours"] - t0o)
@@ -715,10 +715,20 @@ def test_whole_ensemble_teacher_forced_step(dr, oracle, torch_, case):
     states, decisions, queue, tourCount and accumulation buffer are compared with the oracle's (Q15)."""
     name, make, N, seed, method = case
     desc, gsc, osc = _full_scene(dr, oracle, name, make)
-    gch = dr.Chains(gsc, method, N, seed=seed)
     och = oracle.Chains(osc, method, N, seed=seed)
-    gch.init(0)
     och.init(0)
+    # Teacher forcing covers the run's constants too: kappa0 = p_lambda / (m dt) comes from the bootstrap over the init states, and
+    # the handful of init states that diverge or are ill-conditioned move the GPU's own p_lambda by 3e-5 .. 6e-5 relative, which
+    # then sits in EVERY weight of the step (measured with next-event estimation: dw = dp + 3.08e-5 on all chains).  The bootstrap itself is compared below
+    # and, at 2e-6, in _teacher_forced; the step under test takes the oracle's p_lambda like it takes the oracle's state.
+    own = dr.Chains(gsc, method, N, seed=seed)
+    own.init(0)
+    p_lambda = och.stats()["p_lambda"]
+    assert np.isclose(own.stats()["p_lambda"], p_lambda, rtol=1e-4)   # a mean over every init state, the few diverged ones included (Cornell box: 6e-5)
+    del own
+    gch = dr.Chains(gsc, method, N, seed=seed, p_lambda_override=p_lambda)
+    gch.init(0)
+    assert np.isclose(gch.stats()["kappa0"], och.stats()["kappa0"], rtol=1e-6)
     och.step(2)
     gch.upload(och.state(), 2)
     gch.accum.zero_()
@@ -728,13 +738,13 @@ def test_whole_ensemble_teacher_forced_step(dr, oracle, torch_, case):
     och.step(1)
     gs, os_ = gch.download(), och.state()
     g_last, o_last = gch.last_step(), och.last()
-    div, rep = compare_states(gs, os_, g_last, o_last, float(gch.cfg.stddev), fold_outliers=name.endswith("_nee"))
+    osc64 = oracle.Scene(desc, oracle.F64) if name.endswith("_nee") else None
+    div, rep = compare_states(gs, os_, g_last, o_last, float(gch.cfg.stddev), osc64=osc64)
     print(f"{name}/{method}: {rep}")
-    # < 0.1 % of the chains per step (B: north_star).  One case is above it and says so: Diffusion Restore with next-event
-    # estimation on the full machines geometry, where every chain takes a fresh 20-ray evaluation each step: 7e-4 discrete
-    # differences + 7e-4 states whose score (up to 1e5 near a 1 / r^2 or 1 / cos_l singularity) or contribution is
-    # ill-conditioned in fp32 on either side (Q15); measured 1.45e-3, bound 2e-3.
-    assert div.mean() < (2e-3 if (name, method) == ("machines_nee", "diffusion_restore") else 1e-3), rep
+    # < 0.1 % of the chains per step take other discrete decisions (B: north_star), every case.  With next-event estimation the
+    # states whose values differ are judged against fp64 one by one (gpu_util.three_way: a defect fails inside compare_states);
+    # the ill-conditioned ones and those on a decision boundary of the fp64 path are counted apart, each under 0.1 % too.
+    assert rep["discrete_frac"] < 1e-3 and rep["ill_frac"] < 1e-3 and rep["fp64_other_path"] < 1e-3 * N, rep
     compare_bulk(gch, och, gs, os_, g_last, o_last, div, gch.stats()["tours"] - t0g, och.stats()["tours"] - t0o)
 
 
